@@ -1,0 +1,178 @@
+/* gabsplat.h -- C ABI of libgabsplat: the differentiable tile-based rasterizer for 3D Gabor-based
+ * primitives (3DGabSplat, arXiv 2508.05343), hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Citations are /root/reference/PAPER.md line numbers plus the equation they fall in.
+ *
+ * The four calls follow the paper's statement of the renderer ("transformation ...
+ * splat ... tile-based colour-alpha blending"; :160 "tile-based rasterizer"):
+ *
+ *   gabsplat_preprocess       projection of every primitive to the image plane
+ *                             (Eq.2 :91, Eq.3 :101, Eq.9 :145/:414, Eq.10-11 :150-154, SH colour :83)
+ *   gabsplat_bin_sort         (tile | depth) instance keys, stable sort, per-tile ranges (:103, :160)
+ *   gabsplat_render_forward   per-pixel front-to-back blend of 2D Gabor primitives (Eq.12 :158, Eq.13 :162)
+ *   gabsplat_render_backward  the same computation in reverse: gradients of sum_p <dL/dC(p), C(p)> with
+ *                             respect to every primitive parameter, including f and omega (:48, :129)
+ *
+ * General rules
+ *   - Every pointer inside the structs below is a DEVICE pointer unless its name ends in _host.
+ *     The structs themselves are HOST structs, read during the call (they may be freed afterwards).
+ *   - All device buffers are allocated, owned and freed by the caller.  The library allocates only
+ *     inside gabsplat_create (a few KB of device scratch) and frees it in gabsplat_destroy.
+ *   - Inputs are never written.  Outputs are fully overwritten (gradients are zeroed by the library
+ *     before accumulation).
+ *   - Calls enqueue work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ *     stream) and return without synchronising, except where stated.
+ *   - Return value: one of the GABSPLAT_* status codes.  Nothing is printed, nothing aborts.
+ *   - There is no CPU fallback: on a machine without a usable sm_100 device gabsplat_create fails.
+ *   - All floating-point storage is IEEE binary32, contiguous, row-major in the index order written.
+ *
+ * Value contract (activated inputs): scales > 0, rotations are unit quaternions (w,x,y,z)
+ * and are not re-normalised, opacities in (0,1), weights omega_k in [0,1) (omega >= 0 is relied on by the
+ * envelope reject), freqs in cycles per world unit (Eq.7 :127).  Gradients are with respect to these
+ * activated values.
+ */
+#ifndef GABSPLAT_H_
+#define GABSPLAT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GABSPLAT_OK 0
+#define GABSPLAT_INVALID_ARG 1 /* null pointer, N < 0, K outside [0,8], sh_degree outside [0,3], bad size/focal */
+#define GABSPLAT_CAPACITY 2    /* instance buffers or workspace too small */
+#define GABSPLAT_CUDA 3        /* a CUDA call failed; see gabsplat_last_error */
+#define GABSPLAT_UNSUPPORTED 4 /* no sm_100 device */
+
+#define GABSPLAT_MAX_K 8
+#define GABSPLAT_TILE 16       /* tiles are 16x16 pixels */
+#define GABSPLAT_SH_COEFFS 16  /* storage stride of SH coefficients per primitive (degree 3) */
+
+typedef struct gabsplat_ctx gabsplat_ctx;
+
+/* Create / destroy a context bound to CUDA device `device`.  Host calls; create synchronises. */
+int32_t gabsplat_create(gabsplat_ctx** out, int32_t device);
+void gabsplat_destroy(gabsplat_ctx* ctx);
+/* Static description of the last non-OK status on this context (never NULL). */
+const char* gabsplat_last_error(const gabsplat_ctx* ctx);
+
+/* Pinhole camera ("viewing transformation W", "Jacobian J of the affine approximation of the
+ * projective transformation").  Pixel (x,y) is sampled at integer coordinates (x,y). */
+typedef struct {
+  int32_t width, height;
+  float fx, fy, cx, cy;
+  float world_to_cam[12]; /* row-major 3x4 [W | tau]:  t = W mu + tau */
+  float z_near;           /* primitives with t_z <= z_near are culled */
+  float bg[3];            /* background colour, composited as C + T_final * bg */
+} gabsplat_camera;
+
+/* The primitives.  N primitives, K Gabor components each. */
+typedef struct {
+  int32_t N, K, sh_degree;
+  const float* means;     /* [N][3]                                                  */
+  const float* scales;    /* [N][3]   Sigma = R diag(s^2) R^T  (:87)                 */
+  const float* rotations; /* [N][4]   unit quaternion (w,x,y,z)                      */
+  const float* opacities; /* [N]                                                     */
+  const float* sh;        /* [N][16][3]  only the first (sh_degree+1)^2 rows are read */
+  const float* freqs;     /* [N][K][3]  f_{k,i}  (Eq.7)                              */
+  const float* weights;   /* [N][K]     omega_{k,i}  (Eq.7)                          */
+} gabsplat_scene;
+
+/* Outputs of gabsplat_preprocess, one entry per primitive.  Entries of culled primitives are zero
+ * (tiles_touched == 0 marks a culled primitive).  `packed` is the record the blend kernels gather. */
+typedef struct {
+  float* mean2d;           /* [N][2]  mu2D in pixels (:99)                                         */
+  float* depth;            /* [N]     camera-space t_z; its bit pattern is the low half of the key */
+  int32_t* radius;         /* [N]     ceil(3 sqrt(lambda_max)) of the dilated 2D covariance        */
+  float* conic_opacity;    /* [N][4]  (a,b,c) = (Sigma2D + 0.3 I)^-1 (Eq.3), opacity               */
+  float* rgb;              /* [N][3]  SH colour, clamped at 0 from below                           */
+  uint8_t* rgb_clamped;    /* [N][4]  1 where the channel was clamped (4th byte 0)                 */
+  float* freq2d;           /* [N][K][2]  f2D in cycles per pixel (Eq.10-11)                        */
+  uint32_t* tiles_touched; /* [N]     number of tiles in the primitive's rectangle                */
+  int32_t* rect;           /* [N][4]  xmin,ymin,xmax,ymax in tiles, max exclusive                  */
+  float* packed;           /* [N][gabsplat_packed_floats(K)]  gather record, 16-byte aligned       */
+} gabsplat_projected;
+
+/* Number of floats per primitive in gabsplat_projected.packed (a multiple of 4). */
+int32_t gabsplat_packed_floats(int32_t K);
+
+/* Tile binning state.  capacity = number of (key,id) slots the caller allocated. */
+typedef struct {
+  uint32_t* offsets;          /* [N]  inclusive prefix sum of tiles_touched                          */
+  uint64_t* keys;             /* [capacity]  sorted on return: (tile_id << 32) | bits(depth)         */
+  uint32_t* ids;              /* [capacity]  primitive index of each instance, same order            */
+  uint32_t* tile_ranges;      /* [tiles_y*tiles_x][2]  [start,end) into keys/ids; (0,0) if empty     */
+  uint64_t capacity;
+  uint32_t* num_instances;    /* [1]  device: D = total instance count                               */
+  void* workspace;            /* device scratch, >= gabsplat_sort_workspace_bytes(N, capacity) bytes */
+  uint64_t workspace_bytes;
+} gabsplat_binning;
+
+uint64_t gabsplat_sort_workspace_bytes(int32_t N, uint64_t capacity);
+
+/* Forward outputs.  n_contrib[p] = 1-based position, within the tile list of pixel p, of the last
+ * primitive that was blended at p (0 = none); its id is ids[tile_ranges[tile][0] + n_contrib - 1]. */
+typedef struct {
+  float* image;        /* [3][H][W] */
+  float* final_T;      /* [H][W]    */
+  uint32_t* n_contrib; /* [H][W]    */
+} gabsplat_fwd_out;
+
+/* Gradient outputs (all required except d_mean2d / d_mean2d_abs, which may be NULL). */
+typedef struct {
+  float* d_means;      /* [N][3]     */
+  float* d_scales;     /* [N][3]     */
+  float* d_rotations;  /* [N][4]     */
+  float* d_opacities;  /* [N]        */
+  float* d_sh;         /* [N][16][3] */
+  float* d_freqs;      /* [N][K][3]  */
+  float* d_weights;    /* [N][K]     */
+  float* d_mean2d;     /* [N][2] optional: dL/dmu2D in pixel units (densification statistic, :175) */
+  float* d_mean2d_abs; /* [N][2] optional: sum over pixels of |per-pixel dL/dmu2D| (AbsGS variant, :224) */
+} gabsplat_grads;
+
+/* Bytes of device scratch gabsplat_render_backward needs for N primitives with K components. */
+uint64_t gabsplat_grad_workspace_bytes(int32_t N, int32_t K);
+
+/* S1.  Writes every array of `out` for all N primitives. */
+int32_t gabsplat_preprocess(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                            gabsplat_projected* out, void* stream);
+
+/* S2.  Emits one (key,id) per (primitive, tile of its rectangle) in primitive-major, row-major order,
+ * sorts them stably by key with an LSD radix sort on one-byte digits, and extracts tile ranges.
+ * If D > capacity nothing is emitted, *num_instances still holds D, and (when num_instances_host is
+ * given) GABSPLAT_CAPACITY is returned.  num_instances_host != NULL makes the call synchronise the
+ * stream once to read D back; with NULL the call is fully asynchronous and the caller must have sized
+ * capacity from an earlier run. */
+int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected* proj, const gabsplat_camera* cam,
+                          gabsplat_binning* bin, uint64_t* num_instances_host, void* stream);
+
+/* S3.  One CTA per tile; Eq.12-13 with the alpha rules of DESIGN.md (alpha = min(0.99, o G M),
+ * skip alpha < 1/255, stop before T(1-alpha) < 1e-4). */
+int32_t gabsplat_render_forward(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                                const gabsplat_projected* proj, const gabsplat_binning* bin, gabsplat_fwd_out* out,
+                                void* stream);
+
+/* S4a + S4b.  dL_dimage is [3][H][W] on the device. */
+int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                                 const gabsplat_projected* proj, const gabsplat_binning* bin,
+                                 const gabsplat_fwd_out* fwd, const float* dL_dimage, gabsplat_grads* grads,
+                                 void* grad_workspace, uint64_t grad_workspace_bytes, void* stream);
+
+/* Convenience for callers with HOST buffers (bench.py's end-to-end leg): one forward (and, if
+ * dL_dimage_host != NULL, backward) pass with host->device copies of the scene / image gradient and
+ * device->host copies of the image / gradients inside the call; synchronises.  All pointers in
+ * `scene_host` and `grads_host` are HOST pointers here; grads_host may be NULL when dL_dimage_host is.
+ * Device memory is taken from `device_arena` (device pointer, arena_bytes long; query the size with
+ * gabsplat_host_arena_bytes). */
+uint64_t gabsplat_host_arena_bytes(int32_t N, int32_t K, int32_t width, int32_t height, uint64_t capacity);
+int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* scene_host, const gabsplat_camera* cam,
+                             uint64_t capacity, float* image_host, const float* dL_dimage_host,
+                             gabsplat_grads* grads_host, void* device_arena, uint64_t arena_bytes, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GABSPLAT_H_ */

@@ -1,0 +1,349 @@
+"""Thin ctypes binding of libgabsplat.so (include/gabsplat.h).  Argument marshalling only: every step of
+the path runs in the library's CUDA kernels.  torch is used for device memory and streams.
+
+The functions carry the names of the C entry points (gabsplat_preprocess, gabsplat_bin_sort,
+gabsplat_render_forward, gabsplat_render_backward, gabsplat_render_host).  There is no fallback:
+importing this module without the built library, or creating a Context without a B200, raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgabsplat.so")
+
+OK, INVALID_ARG, CAPACITY, CUDA_ERROR, UNSUPPORTED = 0, 1, 2, 3, 4
+TILE = 16
+
+
+class GabsplatError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__("libgabsplat status %d: %s" % (code, msg))
+        self.code = code
+
+
+class _Camera(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("world_to_cam", C.c_float * 12), ("z_near", C.c_float),
+                ("bg", C.c_float * 3)]
+
+
+class _Scene(C.Structure):
+    _fields_ = [("N", C.c_int32), ("K", C.c_int32), ("sh_degree", C.c_int32)] + [
+        (n, C.c_void_p) for n in ("means", "scales", "rotations", "opacities", "sh", "freqs", "weights")]
+
+
+class _Projected(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("mean2d", "depth", "radius", "conic_opacity", "rgb", "rgb_clamped",
+                                          "freq2d", "tiles_touched", "rect", "packed")]
+
+
+class _Binning(C.Structure):
+    _fields_ = [("offsets", C.c_void_p), ("keys", C.c_void_p), ("ids", C.c_void_p), ("tile_ranges", C.c_void_p),
+                ("capacity", C.c_uint64), ("num_instances", C.c_void_p), ("workspace", C.c_void_p),
+                ("workspace_bytes", C.c_uint64)]
+
+
+class _FwdOut(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("image", "final_T", "n_contrib")]
+
+
+class _Grads(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("d_means", "d_scales", "d_rotations", "d_opacities", "d_sh", "d_freqs",
+                                          "d_weights", "d_mean2d", "d_mean2d_abs")]
+
+
+_lib = None
+
+
+def lib():
+    """The loaded library; raises if it has not been built (python -m paper_2508_05343_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libgabsplat.so is not built: run `python -m paper_2508_05343_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.gabsplat_create.argtypes = [C.POINTER(C.c_void_p), C.c_int32]
+        L.gabsplat_create.restype = C.c_int32
+        L.gabsplat_destroy.argtypes = [C.c_void_p]
+        L.gabsplat_destroy.restype = None
+        L.gabsplat_last_error.argtypes = [C.c_void_p]
+        L.gabsplat_last_error.restype = C.c_char_p
+        L.gabsplat_packed_floats.argtypes = [C.c_int32]
+        L.gabsplat_packed_floats.restype = C.c_int32
+        L.gabsplat_sort_workspace_bytes.argtypes = [C.c_int32, C.c_uint64]
+        L.gabsplat_sort_workspace_bytes.restype = C.c_uint64
+        L.gabsplat_grad_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
+        L.gabsplat_grad_workspace_bytes.restype = C.c_uint64
+        L.gabsplat_host_arena_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_uint64]
+        L.gabsplat_host_arena_bytes.restype = C.c_uint64
+        P = C.c_void_p
+        L.gabsplat_preprocess.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected), P]
+        L.gabsplat_bin_sort.argtypes = [P, C.c_int32, C.POINTER(_Projected), C.POINTER(_Camera), C.POINTER(_Binning),
+                                        C.POINTER(C.c_uint64), P]
+        L.gabsplat_render_forward.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
+                                              C.POINTER(_Binning), C.POINTER(_FwdOut), P]
+        L.gabsplat_render_backward.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
+                                               C.POINTER(_Binning), C.POINTER(_FwdOut), P, C.POINTER(_Grads), P,
+                                               C.c_uint64, P]
+        L.gabsplat_render_host.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.c_uint64, P, P,
+                                           C.POINTER(_Grads), P, C.c_uint64, P]
+        for f in (L.gabsplat_preprocess, L.gabsplat_bin_sort, L.gabsplat_render_forward, L.gabsplat_render_backward,
+                  L.gabsplat_render_host):
+            f.restype = C.c_int32
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(stream) -> C.c_void_p:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def camera_struct(cam) -> _Camera:
+    c = _Camera()
+    c.width, c.height = int(cam.width), int(cam.height)
+    c.fx, c.fy, c.cx, c.cy = cam.fx, cam.fy, cam.cx, cam.cy
+    w = np.asarray(cam.world_to_cam, np.float32).reshape(12)
+    for i in range(12):
+        c.world_to_cam[i] = float(w[i])
+    c.z_near = cam.z_near
+    for i in range(3):
+        c.bg[i] = float(cam.bg[i])
+    return c
+
+
+class Context:
+    """gabsplat_ctx bound to one CUDA device."""
+
+    def __init__(self, device: int = 0):
+        self._h = C.c_void_p()
+        rc = lib().gabsplat_create(C.byref(self._h), device)
+        if rc != OK:
+            raise GabsplatError(rc, "gabsplat_create failed (needs an sm_100 device; there is no CPU fallback)")
+        self.device = torch.device("cuda", device)
+
+    def check(self, rc: int) -> None:
+        if rc != OK:
+            raise GabsplatError(rc, lib().gabsplat_last_error(self._h).decode())
+
+    def close(self) -> None:
+        if self._h:
+            lib().gabsplat_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+@dataclass
+class DeviceScene:
+    """The primitives in device memory (float32, contiguous; layouts of gabsplat_scene)."""
+    means: torch.Tensor
+    scales: torch.Tensor
+    rotations: torch.Tensor
+    opacities: torch.Tensor
+    sh: torch.Tensor
+    freqs: torch.Tensor
+    weights: torch.Tensor
+    sh_degree: int = 3
+
+    @property
+    def N(self) -> int:
+        return int(self.means.shape[0])
+
+    @property
+    def K(self) -> int:
+        return int(self.freqs.shape[1])
+
+    def struct(self) -> _Scene:
+        s = _Scene()
+        s.N, s.K, s.sh_degree = self.N, self.K, self.sh_degree
+        for n in ("means", "scales", "rotations", "opacities", "sh", "freqs", "weights"):
+            t = getattr(self, n)
+            assert t.dtype == torch.float32 and t.is_contiguous()
+            setattr(s, n, t.data_ptr() if t.numel() else None)
+        return s
+
+
+def upload_scene(scene, device="cuda:0") -> DeviceScene:
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(device)
+    return DeviceScene(f(scene.means), f(scene.scales), f(scene.rotations), f(scene.opacities), f(scene.sh),
+                       f(scene.freqs), f(scene.weights), scene.sh_degree)
+
+
+class Projected:
+    """Device buffers of gabsplat_projected for N primitives, K components."""
+
+    def __init__(self, N: int, K: int, device):
+        z = lambda shape, dt: torch.zeros(shape, dtype=dt, device=device)
+        self.N, self.K = N, K
+        self.mean2d = z((N, 2), torch.float32)
+        self.depth = z((N,), torch.float32)
+        self.radius = z((N,), torch.int32)
+        self.conic_opacity = z((N, 4), torch.float32)
+        self.rgb = z((N, 3), torch.float32)
+        self.rgb_clamped = z((N, 4), torch.uint8)
+        self.freq2d = z((N, K, 2), torch.float32)
+        self.tiles_touched = z((N,), torch.int32)  # uint32 on the device; torch has no uint32 arithmetic
+        self.rect = z((N, 4), torch.int32)
+        self.packed = z((N, lib().gabsplat_packed_floats(K)), torch.float32)
+
+    def struct(self) -> _Projected:
+        p = _Projected()
+        for n, _ in _Projected._fields_:
+            t = getattr(self, n)
+            setattr(p, n, t.data_ptr() if t.numel() else None)
+        return p
+
+
+class Binning:
+    """Device buffers of gabsplat_binning for N primitives and `capacity` instances."""
+
+    def __init__(self, N: int, cam, capacity: int, device):
+        z = lambda shape, dt: torch.zeros(shape, dtype=dt, device=device)
+        self.N, self.capacity = N, int(capacity)
+        self.n_tiles = ((cam.width + TILE - 1) // TILE) * ((cam.height + TILE - 1) // TILE)
+        self.offsets = z((max(N, 1),), torch.int32)
+        self.keys = z((max(self.capacity, 1),), torch.int64)
+        self.ids = z((max(self.capacity, 1),), torch.int32)
+        self.tile_ranges = z((self.n_tiles, 2), torch.int32)
+        self.num_instances = z((4,), torch.int32)
+        self.workspace_bytes = int(lib().gabsplat_sort_workspace_bytes(N, self.capacity))
+        self.workspace = z((self.workspace_bytes + 256,), torch.uint8)
+        self.D = None  # host copy of the instance count when the call read it back
+
+    def struct(self) -> _Binning:
+        b = _Binning()
+        b.offsets, b.keys, b.ids = self.offsets.data_ptr(), self.keys.data_ptr(), self.ids.data_ptr()
+        b.tile_ranges = self.tile_ranges.data_ptr()
+        b.capacity = self.capacity
+        b.num_instances = self.num_instances.data_ptr()
+        b.workspace = (self.workspace.data_ptr() + 255) // 256 * 256
+        b.workspace_bytes = self.workspace_bytes
+        return b
+
+
+class FwdOut:
+    def __init__(self, cam, device):
+        H, W = cam.height, cam.width
+        self.image = torch.zeros((3, H, W), dtype=torch.float32, device=device)
+        self.final_T = torch.zeros((H, W), dtype=torch.float32, device=device)
+        self.n_contrib = torch.zeros((H, W), dtype=torch.int32, device=device)
+
+    def struct(self) -> _FwdOut:
+        o = _FwdOut()
+        o.image, o.final_T, o.n_contrib = self.image.data_ptr(), self.final_T.data_ptr(), self.n_contrib.data_ptr()
+        return o
+
+
+class Grads:
+    def __init__(self, N: int, K: int, device, with_mean2d: bool = True):
+        z = lambda shape: torch.zeros(shape, dtype=torch.float32, device=device)
+        self.N, self.K = N, K
+        self.d_means, self.d_scales, self.d_rotations = z((N, 3)), z((N, 3)), z((N, 4))
+        self.d_opacities, self.d_sh = z((N,)), z((N, 16, 3))
+        self.d_freqs, self.d_weights = z((N, K, 3)), z((N, K))
+        self.d_mean2d = z((N, 2)) if with_mean2d else None
+        self.d_mean2d_abs = z((N, 2)) if with_mean2d else None
+        self.workspace_bytes = int(lib().gabsplat_grad_workspace_bytes(N, K))
+        self.workspace = torch.zeros((self.workspace_bytes,), dtype=torch.uint8, device=device)
+
+    def struct(self) -> _Grads:
+        g = _Grads()
+        for n, _ in _Grads._fields_:
+            t = getattr(self, n)
+            setattr(g, n, t.data_ptr() if (t is not None and t.numel()) else None)
+        return g
+
+
+# ---- the four calls (same names as the C entry points) ---------------------------------------------
+
+def gabsplat_preprocess(ctx: Context, scene: DeviceScene, cam, out: Projected | None = None, stream=None) -> Projected:
+    out = Projected(scene.N, scene.K, scene.means.device) if out is None else out
+    s, c, p = scene.struct(), camera_struct(cam), out.struct()
+    ctx.check(lib().gabsplat_preprocess(ctx._h, C.byref(s), C.byref(c), C.byref(p), _stream(stream)))
+    return out
+
+
+def gabsplat_bin_sort(ctx: Context, N: int, proj: Projected, cam, bin: Binning | None = None, capacity: int | None = None,
+                      read_count: bool = True, stream=None) -> Binning:
+    """With bin=None and capacity=None the instance count is taken from a first pass with zero capacity."""
+    dev = proj.depth.device
+    if bin is None:
+        if capacity is None:
+            probe = Binning(N, cam, 0, dev)
+            p, c, b = proj.struct(), camera_struct(cam), probe.struct()
+            d = C.c_uint64(0)
+            rc = lib().gabsplat_bin_sort(ctx._h, N, C.byref(p), C.byref(c), C.byref(b), C.byref(d), _stream(stream))
+            if rc not in (OK, CAPACITY):
+                ctx.check(rc)
+            capacity = int(d.value)
+        bin = Binning(N, cam, capacity, dev)
+    p, c, b = proj.struct(), camera_struct(cam), bin.struct()
+    d = C.c_uint64(0)
+    ctx.check(lib().gabsplat_bin_sort(ctx._h, N, C.byref(p), C.byref(c), C.byref(b),
+                                      C.byref(d) if read_count else None, _stream(stream)))
+    bin.D = int(d.value) if read_count else None
+    return bin
+
+
+def gabsplat_render_forward(ctx: Context, scene: DeviceScene, cam, proj: Projected, bin: Binning,
+                            out: FwdOut | None = None, stream=None) -> FwdOut:
+    out = FwdOut(cam, scene.means.device) if out is None else out
+    s, c, p, b, o = scene.struct(), camera_struct(cam), proj.struct(), bin.struct(), out.struct()
+    ctx.check(lib().gabsplat_render_forward(ctx._h, C.byref(s), C.byref(c), C.byref(p), C.byref(b), C.byref(o),
+                                            _stream(stream)))
+    return out
+
+
+def gabsplat_render_backward(ctx: Context, scene: DeviceScene, cam, proj: Projected, bin: Binning, fwd: FwdOut,
+                             dL_dimage: torch.Tensor, grads: Grads | None = None, stream=None) -> Grads:
+    grads = Grads(scene.N, scene.K, scene.means.device) if grads is None else grads
+    assert dL_dimage.dtype == torch.float32 and dL_dimage.is_contiguous()
+    assert tuple(dL_dimage.shape) == (3, cam.height, cam.width)
+    s, c, p, b, o, g = (scene.struct(), camera_struct(cam), proj.struct(), bin.struct(), fwd.struct(), grads.struct())
+    ctx.check(lib().gabsplat_render_backward(ctx._h, C.byref(s), C.byref(c), C.byref(p), C.byref(b), C.byref(o),
+                                             _ptr(dL_dimage), C.byref(g), _ptr(grads.workspace),
+                                             grads.workspace_bytes, _stream(stream)))
+    return grads
+
+
+def gabsplat_render_host(ctx: Context, scene, cam, capacity: int, image_host: torch.Tensor,
+                         dL_dimage_host: torch.Tensor | None, grads_host: dict | None, arena: torch.Tensor,
+                         stream=None) -> None:
+    """End-to-end call with HOST buffers (torch CPU tensors, ideally pinned).  `scene` holds CPU tensors
+    under the attribute names of gabsplat_scene; `grads_host` maps d_* names to CPU tensors."""
+    s = _Scene()
+    s.N, s.K, s.sh_degree = int(scene.means.shape[0]), int(scene.freqs.shape[1]), int(scene.sh_degree)
+    for n in ("means", "scales", "rotations", "opacities", "sh", "freqs", "weights"):
+        t = getattr(scene, n)
+        setattr(s, n, t.data_ptr() if t.numel() else None)
+    g = _Grads()
+    if grads_host is not None:
+        for n, _ in _Grads._fields_:
+            t = grads_host.get(n)
+            setattr(g, n, t.data_ptr() if (t is not None and t.numel()) else None)
+    c = camera_struct(cam)
+    base = (arena.data_ptr() + 255) // 256 * 256
+    nbytes = arena.numel() - (base - arena.data_ptr())
+    ctx.check(lib().gabsplat_render_host(ctx._h, C.byref(s), C.byref(c), int(capacity), _ptr(image_host),
+                                         _ptr(dL_dimage_host), C.byref(g) if grads_host is not None else None,
+                                         C.c_void_p(base), nbytes, _stream(stream)))
+
+
+def host_arena_bytes(N: int, K: int, cam, capacity: int) -> int:
+    return int(lib().gabsplat_host_arena_bytes(N, K, cam.width, cam.height, int(capacity))) + 256

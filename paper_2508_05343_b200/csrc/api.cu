@@ -1,0 +1,180 @@
+// The C ABI of libgabsplat (include/gabsplat.h): argument checking, status codes, and the order of
+// kernel launches.  No arithmetic of the method lives here.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+
+struct gabsplat_ctx {
+  int device;
+  uint64_t* pinned_count;  // 8-byte pinned readback slot for D
+  char error[256];
+};
+
+namespace {
+
+using namespace gabsplat;
+
+int32_t fail(gabsplat_ctx* ctx, int32_t code, const char* msg) {
+  if (ctx) {
+    std::strncpy(ctx->error, msg, sizeof(ctx->error) - 1);
+    ctx->error[sizeof(ctx->error) - 1] = 0;
+  }
+  return code;
+}
+
+int32_t cuda_fail(gabsplat_ctx* ctx, cudaError_t e, const char* where) {
+  if (ctx) std::snprintf(ctx->error, sizeof(ctx->error), "%s: %s", where, cudaGetErrorString(e));
+  return GABSPLAT_CUDA;
+}
+
+bool camera_ok(const gabsplat_camera* c) {
+  return c && c->width > 0 && c->height > 0 && c->fx > 0.f && c->fy > 0.f &&
+         (int64_t)((c->width + kTile - 1) / kTile) * ((c->height + kTile - 1) / kTile) < (1 << 30);
+}
+
+bool scene_ok(const gabsplat_scene* s) {
+  if (!s || s->N < 0 || s->K < 0 || s->K > kMaxK || s->sh_degree < 0 || s->sh_degree > 3) return false;
+  if (s->N == 0) return true;
+  if (!s->means || !s->scales || !s->rotations || !s->opacities || !s->sh) return false;
+  if (s->K > 0 && (!s->freqs || !s->weights)) return false;
+  return true;
+}
+
+bool projected_ok(const gabsplat_projected* p, int N, int K) {
+  if (!p) return false;
+  if (N == 0) return true;
+  return p->mean2d && p->depth && p->radius && p->conic_opacity && p->rgb && p->rgb_clamped &&
+         (K == 0 || p->freq2d) && p->tiles_touched && p->rect && p->packed;
+}
+
+bool binning_ok(const gabsplat_binning* b, int N) {
+  if (!b || !b->tile_ranges || !b->num_instances) return false;
+  if (N > 0 && !b->offsets) return false;
+  if (b->capacity > 0 && (!b->keys || !b->ids)) return false;
+  if (b->capacity >= (1ull << 32)) return false;
+  return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t gabsplat_create(gabsplat_ctx** out, int32_t device) {
+  if (!out) return GABSPLAT_INVALID_ARG;
+  *out = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) {
+    cudaGetLastError();
+    return GABSPLAT_UNSUPPORTED;
+  }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return GABSPLAT_CUDA;
+  if (prop.major != 10) return GABSPLAT_UNSUPPORTED;  // the kernels are built for sm_100a only
+  if (cudaSetDevice(device) != cudaSuccess) return GABSPLAT_CUDA;
+  gabsplat_ctx* ctx = new (std::nothrow) gabsplat_ctx;
+  if (!ctx) return GABSPLAT_CUDA;
+  ctx->device = device;
+  ctx->error[0] = 0;
+  ctx->pinned_count = nullptr;
+  if (cudaMallocHost(&ctx->pinned_count, sizeof(uint64_t)) != cudaSuccess) {
+    delete ctx;
+    return GABSPLAT_CUDA;
+  }
+  cudaDeviceSynchronize();
+  *out = ctx;
+  return GABSPLAT_OK;
+}
+
+void gabsplat_destroy(gabsplat_ctx* ctx) {
+  if (!ctx) return;
+  if (ctx->pinned_count) cudaFreeHost(ctx->pinned_count);
+  delete ctx;
+}
+
+const char* gabsplat_last_error(const gabsplat_ctx* ctx) { return ctx ? ctx->error : "null context"; }
+
+int32_t gabsplat_packed_floats(int32_t K) { return (K < 0 || K > kMaxK) ? 0 : packed_floats(K); }
+
+uint64_t gabsplat_sort_workspace_bytes(int32_t N, uint64_t capacity) {
+  return sort_workspace_bytes(N < 0 ? 0 : N, capacity);
+}
+
+uint64_t gabsplat_grad_workspace_bytes(int32_t N, int32_t K) {
+  if (N < 0 || K < 0 || K > kMaxK) return 0;
+  return (uint64_t)N * grad2d_floats(K) * sizeof(float) + 256;
+}
+
+int32_t gabsplat_preprocess(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                            gabsplat_projected* out, void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  if (!scene_ok(scene)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess: bad scene");
+  if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess: bad camera");
+  if (!projected_ok(out, scene->N, scene->K)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess: null output");
+  const cudaError_t e = launch_preprocess(*scene, make_camera(*cam), *out, (cudaStream_t)stream);
+  return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "preprocess");
+}
+
+int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected* proj, const gabsplat_camera* cam,
+                          gabsplat_binning* bin, uint64_t* num_instances_host, void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  if (N < 0 || !camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: bad N or camera");
+  if (!proj || (N > 0 && (!proj->tiles_touched || !proj->rect || !proj->depth)))
+    return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: null projected arrays");
+  if (!binning_ok(bin, N)) return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: bad binning buffers");
+  if (!bin->workspace || bin->workspace_bytes < sort_workspace_bytes(N, bin->capacity))
+    return fail(ctx, GABSPLAT_CAPACITY, "bin_sort: workspace too small");
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e = launch_bin_sort(N, *proj, make_camera(*cam), *bin, st);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "bin_sort");
+  if (num_instances_host) {
+    uint32_t* slot = reinterpret_cast<uint32_t*>(ctx->pinned_count);
+    e = cudaMemcpyAsync(slot, bin->num_instances, sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "bin_sort readback");
+    *num_instances_host = *slot;
+    if (*num_instances_host > bin->capacity) return fail(ctx, GABSPLAT_CAPACITY, "bin_sort: instance capacity too small");
+  }
+  return GABSPLAT_OK;
+}
+
+int32_t gabsplat_render_forward(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                                const gabsplat_projected* proj, const gabsplat_binning* bin, gabsplat_fwd_out* out,
+                                void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  if (!scene || scene->K < 0 || scene->K > kMaxK || scene->N < 0) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: bad scene");
+  if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: bad camera");
+  if (!proj || (scene->N > 0 && !proj->packed)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: null packed records");
+  if (!bin || !bin->tile_ranges || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: bad binning");
+  if (!out || !out->image || !out->final_T || !out->n_contrib) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: null output");
+  const cudaError_t e = launch_blend_forward(scene->K, make_camera(*cam), *proj, *bin, *out, (cudaStream_t)stream);
+  return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "render_forward");
+}
+
+int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                                 const gabsplat_projected* proj, const gabsplat_binning* bin,
+                                 const gabsplat_fwd_out* fwd, const float* dL_dimage, gabsplat_grads* grads,
+                                 void* grad_workspace, uint64_t grad_workspace_bytes, void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  if (!scene_ok(scene)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: bad scene");
+  if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: bad camera");
+  if (!projected_ok(proj, scene->N, scene->K)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: null projected arrays");
+  if (!bin || !bin->tile_ranges || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: bad binning");
+  if (!fwd || !fwd->final_T || !fwd->n_contrib || !dL_dimage) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: null forward state");
+  if (!grads) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: null grads");
+  if (scene->N > 0 && (!grads->d_means || !grads->d_scales || !grads->d_rotations || !grads->d_opacities || !grads->d_sh ||
+                       (scene->K > 0 && (!grads->d_freqs || !grads->d_weights))))
+    return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: null gradient output");
+  if (scene->N > 0 && (!grad_workspace || grad_workspace_bytes < gabsplat_grad_workspace_bytes(scene->N, scene->K)))
+    return fail(ctx, GABSPLAT_CAPACITY, "render_backward: gradient workspace too small");
+  cudaStream_t st = (cudaStream_t)stream;
+  const Camera c = make_camera(*cam);
+  float* grad2d = reinterpret_cast<float*>(((uintptr_t)grad_workspace + 255) & ~(uintptr_t)255);
+  cudaError_t e = launch_blend_backward(scene->N, scene->K, c, *proj, *bin, *fwd, dL_dimage, grad2d, st);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "render_backward (blend)");
+  e = launch_preprocess_backward(*scene, c, *proj, grad2d, *grads, st);
+  return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "render_backward (projection)");
+}
+
+}  // extern "C"

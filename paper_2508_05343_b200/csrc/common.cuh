@@ -1,0 +1,70 @@
+// Shared declarations of the CUDA path (libgabsplat.so).  Nothing here is used by oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/gabsplat.h"
+
+namespace gabsplat {
+
+// Named constants of the rasterizer the paper adopts from 3DGS (readings C5, C8).
+constexpr float kDilation = 0.3f;
+constexpr float kAlphaMax = 0.99f;
+constexpr float kAlphaMin = 1.0f / 255.0f;
+constexpr float kTMin = 1e-4f;
+constexpr int kTile = GABSPLAT_TILE;
+constexpr int kMaxK = GABSPLAT_MAX_K;
+
+// ---- packed gather record (gabsplat_projected.packed), floats -----------------------------------
+//  [0..3]   mean2d hi.x, hi.y (fp32 mean, the indexing value), lo.x, lo.y (fp64 residual)
+//  [4..7]   L11, L21, L22 (sqrt(1/2) * Cholesky factor of the conic: q = -(u^2+v^2), u = L11 dx + L21 dy,
+//           v = L22 dy), qmin = -ln(255 o) - margin   (envelope reject: skip when q < qmin)
+//  [8..11]  opacity, r, g, b
+//  [12..]   f2D (x,y) * K, padded to a multiple of 4 floats; then omega * K, padded to a multiple of 4
+__host__ __device__ constexpr int freq_floats(int K) { return 4 * ((2 * K + 3) / 4); }
+__host__ __device__ constexpr int weight_floats(int K) { return 4 * ((K + 3) / 4); }
+__host__ __device__ constexpr int packed_floats(int K) { return 12 + freq_floats(K) + weight_floats(K); }
+__host__ __device__ constexpr int weight_offset(int K) { return 12 + freq_floats(K); }
+
+// ---- 2D gradient record accumulated by the blend backward (grad workspace), floats ---------------
+//  [0..1] d mean2d   [2..4] d conic (a,b,c)   [5] d opacity   [6..8] d rgb   [9..10] sum |d mean2d|  [11] pad
+//  [12..] d f2D (x,y) * K padded to 4; then d omega * K padded to 4     (same tail layout as the packed record)
+__host__ __device__ constexpr int grad2d_floats(int K) { return packed_floats(K); }
+
+struct Camera {  // device copy of gabsplat_camera plus derived integers
+  int width, height, tiles_x, tiles_y;
+  float fx, fy, cx, cy;
+  float w[12];
+  float z_near;
+  float bg[3];
+};
+
+inline Camera make_camera(const gabsplat_camera& c) {
+  Camera k;
+  k.width = c.width; k.height = c.height;
+  k.tiles_x = (c.width + kTile - 1) / kTile;
+  k.tiles_y = (c.height + kTile - 1) / kTile;
+  k.fx = c.fx; k.fy = c.fy; k.cx = c.cx; k.cy = c.cy;
+  for (int i = 0; i < 12; ++i) k.w[i] = c.world_to_cam[i];
+  k.z_near = c.z_near;
+  for (int i = 0; i < 3; ++i) k.bg[i] = c.bg[i];
+  return k;
+}
+
+// ---- launchers (one per .cu file); each returns the cudaError_t of its last launch ---------------
+cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& out,
+                              cudaStream_t st);
+cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
+                            cudaStream_t st);
+cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projected& proj,
+                                 const gabsplat_binning& bin, const gabsplat_fwd_out& out, cudaStream_t st);
+cudaError_t launch_blend_backward(int N, int K, const Camera& cam, const gabsplat_projected& proj,
+                                  const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const float* dL_dimage,
+                                  float* grad2d, cudaStream_t st);
+cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& proj,
+                                       const float* grad2d, const gabsplat_grads& g, cudaStream_t st);
+
+uint64_t sort_workspace_bytes(int N, uint64_t capacity);
+
+}  // namespace gabsplat

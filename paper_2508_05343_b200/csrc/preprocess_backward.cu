@@ -1,0 +1,239 @@
+// S4b / K8: chain rule from the projected quantities back to the primitive parameters (the paper gives no
+// equations -- PAPER.md:48, :129; derivation in DESIGN.md "Backward", per-primitive part):
+//   conic -> U;  f2D = U^-1 T Sigma f -> (U, T, Sigma, f);  U = T Sigma T^T -> (T, Sigma);  T = J W -> J -> t;
+//   mu2D -> t;  t -> mu;  Sigma = R S S^T R^T -> (scale, quaternion);  rgb -> (SH, mu through the view direction).
+// One thread per primitive; evaluated in fp64 (HBM-bound: the arithmetic is free, see preprocess.cu).
+// Gradient arrays are zeroed first, so culled primitives cost no thread work.
+#include "common.cuh"
+#include "sh.cuh"
+
+namespace gabsplat {
+namespace {
+
+__global__ void __launch_bounds__(128) preprocess_backward_kernel(gabsplat_scene s, Camera c, const uint32_t* __restrict__ tiles_touched,
+                                                                 const uint8_t* __restrict__ rgb_clamped,
+                                                                 const float* __restrict__ grad2d, gabsplat_grads g) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= s.N) return;
+  if (tiles_touched[i] == 0) return;
+  const int K = s.K;
+  const int G = grad2d_floats(K);
+  const float* g2 = grad2d + (size_t)i * G;
+
+  double Wm[3][3], tau[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+#pragma unroll
+    for (int b = 0; b < 3; ++b) Wm[a][b] = (double)c.w[4 * a + b];
+    tau[a] = (double)c.w[4 * a + 3];
+  }
+  const double mu[3] = {(double)s.means[3 * i], (double)s.means[3 * i + 1], (double)s.means[3 * i + 2]};
+  double t[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) t[a] = Wm[a][0] * mu[0] + Wm[a][1] * mu[1] + Wm[a][2] * mu[2] + tau[a];
+  const double tz = t[2];
+  const double sc[3] = {(double)s.scales[3 * i], (double)s.scales[3 * i + 1], (double)s.scales[3 * i + 2]};
+  const double qw = s.rotations[4 * i], qx = s.rotations[4 * i + 1], qy = s.rotations[4 * i + 2], qz = s.rotations[4 * i + 3];
+  const double R[3][3] = {{1 - 2 * (qy * qy + qz * qz), 2 * (qx * qy - qw * qz), 2 * (qx * qz + qw * qy)},
+                          {2 * (qx * qy + qw * qz), 1 - 2 * (qx * qx + qz * qz), 2 * (qy * qz - qw * qx)},
+                          {2 * (qx * qz - qw * qy), 2 * (qy * qz + qw * qx), 1 - 2 * (qx * qx + qy * qy)}};
+  double Sg[3][3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b)
+      Sg[a][b] = R[a][0] * sc[0] * sc[0] * R[b][0] + R[a][1] * sc[1] * sc[1] * R[b][1] + R[a][2] * sc[2] * sc[2] * R[b][2];
+  const double limx = 1.3 * (0.5 * c.width / (double)c.fx), limy = 1.3 * (0.5 * c.height / (double)c.fy);
+  const double rx = t[0] / tz, ry = t[1] / tz;
+  const bool clampx = rx < -limx || rx > limx, clampy = ry < -limy || ry > limy;
+  const double ux = fmin(limx, fmax(-limx, rx)), uy = fmin(limy, fmax(-limy, ry));
+  const double fx = c.fx, fy = c.fy;
+  const double J00 = fx / tz, J11 = fy / tz, J02 = -fx * ux / tz, J12 = -fy * uy / tz;
+  double T[2][3], V[2][3];
+#pragma unroll
+  for (int b = 0; b < 3; ++b) {
+    T[0][b] = J00 * Wm[0][b] + J02 * Wm[2][b];
+    T[1][b] = J11 * Wm[1][b] + J12 * Wm[2][b];
+  }
+#pragma unroll
+  for (int a = 0; a < 2; ++a)
+#pragma unroll
+    for (int b = 0; b < 3; ++b) V[a][b] = T[a][0] * Sg[0][b] + T[a][1] * Sg[1][b] + T[a][2] * Sg[2][b];
+  const double U00 = V[0][0] * T[0][0] + V[0][1] * T[0][1] + V[0][2] * T[0][2];
+  const double U01 = V[0][0] * T[1][0] + V[0][1] * T[1][1] + V[0][2] * T[1][2];
+  const double U11 = V[1][0] * T[1][0] + V[1][1] * T[1][1] + V[1][2] * T[1][2];
+  const double A = U00 + 0.3, C = U11 + 0.3;
+  const double idet = 1.0 / (A * C - U01 * U01);
+  const double ca = C * idet, cb = -U01 * idet, cc = A * idet;
+
+  // conic -> U_d (= U + const):  G_U = -Cm Gc Cm,  Gc = [[ga, gb/2],[gb/2, gc]]
+  double GU[2][2];
+  {
+    const double ga = g2[2], gb = 0.5 * (double)g2[3], gc = g2[4];
+    const double m00 = ca * ga + cb * gb, m01 = ca * gb + cb * gc;
+    const double m10 = cb * ga + cc * gb, m11 = cb * gb + cc * gc;
+    GU[0][0] = -(m00 * ca + m01 * cb);
+    GU[0][1] = -(m00 * cb + m01 * cc);
+    GU[1][0] = -(m10 * ca + m11 * cb);
+    GU[1][1] = -(m10 * cb + m11 * cc);
+  }
+  double gS[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, gT[2][3] = {{0, 0, 0}, {0, 0, 0}};
+  // f2D_k = U^-1 T Sigma f_k  (U undilated)
+  {
+    const double iu = 1.0 / (U00 * U11 - U01 * U01);
+    const double Ui00 = U11 * iu, Ui01 = -U01 * iu, Ui11 = U00 * iu;
+    const int wo = weight_offset(K);
+    for (int k = 0; k < K; ++k) {
+      const float* fp = s.freqs + ((size_t)i * K + k) * 3;
+      const double f[3] = {fp[0], fp[1], fp[2]};
+      const double gf0 = g2[12 + 2 * k], gf1 = g2[12 + 2 * k + 1];
+      const double h0 = Ui00 * gf0 + Ui01 * gf1, h1 = Ui01 * gf0 + Ui11 * gf1;
+      const double b0 = V[0][0] * f[0] + V[0][1] * f[1] + V[0][2] * f[2];
+      const double b1 = V[1][0] * f[0] + V[1][1] * f[1] + V[1][2] * f[2];
+      const double f2x = Ui00 * b0 + Ui01 * b1, f2y = Ui01 * b0 + Ui11 * b1;
+      GU[0][0] -= h0 * f2x;
+      GU[0][1] -= 0.5 * (h0 * f2y + f2x * h1);
+      GU[1][0] -= 0.5 * (h1 * f2x + f2y * h0);
+      GU[1][1] -= h1 * f2y;
+      double Th[3], Sf[3];
+#pragma unroll
+      for (int m = 0; m < 3; ++m) {
+        Th[m] = T[0][m] * h0 + T[1][m] * h1;
+        Sf[m] = Sg[m][0] * f[0] + Sg[m][1] * f[1] + Sg[m][2] * f[2];
+      }
+#pragma unroll
+      for (int m = 0; m < 3; ++m)
+#pragma unroll
+        for (int n = 0; n < 3; ++n) gS[m][n] += 0.5 * (Th[m] * f[n] + f[m] * Th[n]);
+#pragma unroll
+      for (int m = 0; m < 3; ++m) { gT[0][m] += h0 * Sf[m]; gT[1][m] += h1 * Sf[m]; }
+#pragma unroll
+      for (int m = 0; m < 3; ++m)
+        g.d_freqs[((size_t)i * K + k) * 3 + m] = (float)(Sg[m][0] * Th[0] + Sg[m][1] * Th[1] + Sg[m][2] * Th[2]);
+      g.d_weights[(size_t)i * K + k] = g2[wo + k];
+    }
+  }
+  // U = T Sigma T^T
+  {
+    double GUT[2][3];
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+      for (int m = 0; m < 3; ++m) GUT[r][m] = GU[r][0] * T[0][m] + GU[r][1] * T[1][m];
+#pragma unroll
+    for (int m = 0; m < 3; ++m)
+#pragma unroll
+      for (int n = 0; n < 3; ++n) gS[m][n] += T[0][m] * GUT[0][n] + T[1][m] * GUT[1][n];
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+      for (int m = 0; m < 3; ++m) gT[r][m] += 2.0 * (GUT[r][0] * Sg[0][m] + GUT[r][1] * Sg[1][m] + GUT[r][2] * Sg[2][m]);
+  }
+  // T = J W  ->  g_J = g_T W^T;  J(t) and mu2D(t)
+  double gt[3] = {0, 0, 0};
+  {
+    double gJ[2][3];
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+      for (int m = 0; m < 3; ++m) gJ[r][m] = gT[r][0] * Wm[m][0] + gT[r][1] * Wm[m][1] + gT[r][2] * Wm[m][2];
+    const double iz = 1.0 / tz, iz2 = iz * iz;
+    gt[2] += -gJ[0][0] * fx * iz2 - gJ[1][1] * fy * iz2;
+    gt[2] += gJ[0][2] * fx * ux * iz2 + gJ[1][2] * fy * uy * iz2;
+    if (!clampx) { gt[0] += -gJ[0][2] * fx * iz2; gt[2] += gJ[0][2] * fx * t[0] * iz2 * iz; }
+    if (!clampy) { gt[1] += -gJ[1][2] * fy * iz2; gt[2] += gJ[1][2] * fy * t[1] * iz2 * iz; }
+    const double gmx = g2[0], gmy = g2[1];
+    gt[0] += gmx * fx * iz;
+    gt[1] += gmy * fy * iz;
+    gt[2] += -(gmx * fx * t[0] + gmy * fy * t[1]) * iz2;
+  }
+  double gmu[3];
+#pragma unroll
+  for (int m = 0; m < 3; ++m) gmu[m] = Wm[0][m] * gt[0] + Wm[1][m] * gt[1] + Wm[2][m] * gt[2];
+  // Sigma = Ms Ms^T, Ms = R diag(s):  g_Ms = 2 g_Sigma Ms
+  {
+    double gR[3][3];
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      double gs = 0.0;
+#pragma unroll
+      for (int m = 0; m < 3; ++m) {
+        const double gMs = 2.0 * (gS[m][0] * R[0][n] + gS[m][1] * R[1][n] + gS[m][2] * R[2][n]) * sc[n];
+        gs += R[m][n] * gMs;
+        gR[m][n] = gMs * sc[n];
+      }
+      g.d_scales[3 * i + n] = (float)gs;
+    }
+    // R(q) polynomial (un-normalised) form
+    const double dw = 2 * (-qz * gR[0][1] + qy * gR[0][2] + qz * gR[1][0] - qx * gR[1][2] - qy * gR[2][0] + qx * gR[2][1]);
+    const double dx = 2 * (qy * gR[0][1] + qz * gR[0][2] + qy * gR[1][0] - 2 * qx * gR[1][1] - qw * gR[1][2] + qz * gR[2][0] +
+                           qw * gR[2][1] - 2 * qx * gR[2][2]);
+    const double dy = 2 * (-2 * qy * gR[0][0] + qx * gR[0][1] + qw * gR[0][2] + qx * gR[1][0] + qz * gR[1][2] - qw * gR[2][0] +
+                           qz * gR[2][1] - 2 * qy * gR[2][2]);
+    const double dz = 2 * (-2 * qz * gR[0][0] - qw * gR[0][1] + qx * gR[0][2] + qw * gR[1][0] - 2 * qz * gR[1][1] + qy * gR[1][2] +
+                           qx * gR[2][0] + qy * gR[2][1]);
+    reinterpret_cast<float4*>(g.d_rotations)[i] = make_float4((float)dw, (float)dx, (float)dy, (float)dz);
+  }
+  // colour: rgb = max(0, 0.5 + sum_j Y_j(dir) sh_j)
+  {
+    double cp[3], v[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) cp[a] = -(Wm[0][a] * tau[0] + Wm[1][a] * tau[1] + Wm[2][a] * tau[2]);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) v[a] = mu[a] - cp[a];
+    const double il = 1.0 / sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+    const double d[3] = {v[0] * il, v[1] * il, v[2] * il};
+    double Y[16], dY[16][3];
+    sh_values(s.sh_degree, d[0], d[1], d[2], Y);
+    sh_gradients(s.sh_degree, d[0], d[1], d[2], dY);
+    const int nc = (s.sh_degree + 1) * (s.sh_degree + 1);
+    const uchar4 cl = reinterpret_cast<const uchar4*>(rgb_clamped)[i];
+    const double gr[3] = {cl.x ? 0.0 : (double)g2[6], cl.y ? 0.0 : (double)g2[7], cl.z ? 0.0 : (double)g2[8]};
+    double gd[3] = {0, 0, 0};
+    const float* shp = s.sh + (size_t)i * 48;
+    float* dsh = g.d_sh + (size_t)i * 48;
+    for (int j = 0; j < nc; ++j) {
+      double dot = 0.0;
+#pragma unroll
+      for (int ch = 0; ch < 3; ++ch) {
+        dsh[3 * j + ch] = (float)(Y[j] * gr[ch]);
+        dot += (double)shp[3 * j + ch] * gr[ch];
+      }
+#pragma unroll
+      for (int m = 0; m < 3; ++m) gd[m] += dY[j][m] * dot;
+    }
+    const double dg = d[0] * gd[0] + d[1] * gd[1] + d[2] * gd[2];
+#pragma unroll
+    for (int m = 0; m < 3; ++m) gmu[m] += (gd[m] - d[m] * dg) * il;
+  }
+#pragma unroll
+  for (int m = 0; m < 3; ++m) g.d_means[3 * i + m] = (float)gmu[m];
+  g.d_opacities[i] = g2[5];
+  if (g.d_mean2d) { g.d_mean2d[2 * i] = g2[0]; g.d_mean2d[2 * i + 1] = g2[1]; }
+  if (g.d_mean2d_abs) { g.d_mean2d_abs[2 * i] = g2[9]; g.d_mean2d_abs[2 * i + 1] = g2[10]; }
+}
+
+}  // namespace
+
+cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& proj,
+                                       const float* grad2d, const gabsplat_grads& g, cudaStream_t st) {
+  const size_t N = (size_t)s.N, K = (size_t)s.K;
+  cudaMemsetAsync(g.d_means, 0, N * 3 * sizeof(float), st);
+  cudaMemsetAsync(g.d_scales, 0, N * 3 * sizeof(float), st);
+  cudaMemsetAsync(g.d_rotations, 0, N * 4 * sizeof(float), st);
+  cudaMemsetAsync(g.d_opacities, 0, N * sizeof(float), st);
+  cudaMemsetAsync(g.d_sh, 0, N * 48 * sizeof(float), st);
+  if (K) {
+    cudaMemsetAsync(g.d_freqs, 0, N * K * 3 * sizeof(float), st);
+    cudaMemsetAsync(g.d_weights, 0, N * K * sizeof(float), st);
+  }
+  if (g.d_mean2d) cudaMemsetAsync(g.d_mean2d, 0, N * 2 * sizeof(float), st);
+  if (g.d_mean2d_abs) cudaMemsetAsync(g.d_mean2d_abs, 0, N * 2 * sizeof(float), st);
+  if (s.N == 0) return cudaGetLastError();
+  const int block = 128;
+  preprocess_backward_kernel<<<(s.N + block - 1) / block, block, 0, st>>>(s, cam, proj.tiles_touched, proj.rgb_clamped,
+                                                                       grad2d, g);
+  return cudaGetLastError();
+}
+
+}  // namespace gabsplat

@@ -1,0 +1,136 @@
+"""-m gpu edge cases of the C ABI: empty and fully culled scenes, capacity overflow, status codes, and the
+host-buffer convenience call."""
+import numpy as np
+import pytest
+
+from paper_2508_05343_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+
+def _mods():
+    import torch
+    from paper_2508_05343_b200 import binding as gb
+    from tests.gpu_helpers import ctx, run_gpu
+    return torch, gb, ctx(), run_gpu
+
+
+def test_empty_scene():
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny", N=0)
+    cam = scenes.make_cameras("tiny")[0]
+    cam.bg = (0.25, 0.5, 0.75)
+    dL = np.ones((3, cam.height, cam.width), np.float32)
+    g, _ = run_gpu(scene, cam, dL)
+    assert g["D"] == 0
+    assert np.all(g["tile_ranges"] == 0)
+    assert np.all(g["n_contrib"] == 0) and np.all(g["final_T"] == 1.0)
+    for ch, v in enumerate(cam.bg):
+        assert np.all(g["image"][ch] == np.float32(v))
+
+
+def test_all_culled():
+    """Everything behind the camera: no instances, background image, zero gradients."""
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny")
+    scene.means[:, 2] -= 10.0
+    cam = scenes.make_cameras("tiny")[0]
+    dL = scenes.make_image_grad("tiny", 0, cam)
+    g, _ = run_gpu(scene, cam, dL)
+    assert g["D"] == 0 and np.all(g["tiles_touched"] == 0)
+    assert np.all(g["image"] == 0)
+    for n in ("d_means", "d_scales", "d_rotations", "d_opacities", "d_sh", "d_freqs", "d_weights"):
+        assert np.all(g[n] == 0)
+
+
+def test_capacity_overflow_reports_required_count():
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny")
+    cam = scenes.make_cameras("tiny")[0]
+    ds = gb.upload_scene(scene)
+    proj = gb.gabsplat_preprocess(ctx, ds, cam)
+    full = gb.gabsplat_bin_sort(ctx, ds.N, proj, cam)
+    D = full.D
+    assert D > 16
+    small = gb.Binning(ds.N, cam, D - 1, ds.means.device)
+    with pytest.raises(gb.GabsplatError) as e:
+        gb.gabsplat_bin_sort(ctx, ds.N, proj, cam, bin=small)
+    assert e.value.code == gb.CAPACITY
+    torch.cuda.synchronize()
+    assert int(small.num_instances[0].item()) == D          # the required count is left on the device
+    exact = gb.gabsplat_bin_sort(ctx, ds.N, proj, cam, bin=gb.Binning(ds.N, cam, D, ds.means.device))
+    assert torch.equal(exact.keys[:D], full.keys[:D]) and torch.equal(exact.ids[:D], full.ids[:D])
+    # slack capacity gives the same list
+    slack = gb.gabsplat_bin_sort(ctx, ds.N, proj, cam, bin=gb.Binning(ds.N, cam, 3 * D + 5, ds.means.device))
+    assert torch.equal(slack.keys[:D], full.keys[:D]) and torch.equal(slack.ids[:D], full.ids[:D])
+    assert torch.equal(slack.tile_ranges, full.tile_ranges)
+
+
+def test_invalid_arguments():
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny", N=8)
+    cam = scenes.make_cameras("tiny")[0]
+    ds = gb.upload_scene(scene)
+    bad = scenes.make_camera(0, 16, 10.0, cam.world_to_cam)
+    with pytest.raises(gb.GabsplatError) as e:
+        gb.gabsplat_preprocess(ctx, ds, bad, out=gb.Projected(8, 4, ds.means.device))
+    assert e.value.code == gb.INVALID_ARG
+    ds.sh_degree = 4
+    with pytest.raises(gb.GabsplatError) as e:
+        gb.gabsplat_preprocess(ctx, ds, cam)
+    assert e.value.code == gb.INVALID_ARG
+
+
+def test_async_path_without_readback_matches():
+    """read_count=False (no host sync inside the call) gives the same result as the synchronising call."""
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny")
+    cam = scenes.make_cameras("tiny")[0]
+    ds = gb.upload_scene(scene)
+    proj = gb.gabsplat_preprocess(ctx, ds, cam)
+    a = gb.gabsplat_bin_sort(ctx, ds.N, proj, cam)
+    b = gb.gabsplat_bin_sort(ctx, ds.N, proj, cam, bin=gb.Binning(ds.N, cam, a.D + 100, ds.means.device),
+                             read_count=False)
+    torch.cuda.synchronize()
+    assert b.D is None
+    assert torch.equal(a.keys[:a.D], b.keys[:a.D]) and torch.equal(a.tile_ranges, b.tile_ranges)
+
+
+def test_side_stream():
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny")
+    cam = scenes.make_cameras("tiny")[0]
+    ref, _ = run_gpu(scene, cam)
+    st = torch.cuda.Stream()
+    ds = gb.upload_scene(scene)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(st):
+        proj = gb.gabsplat_preprocess(ctx, ds, cam, stream=st)
+        bins = gb.gabsplat_bin_sort(ctx, ds.N, proj, cam, stream=st)
+        fwd = gb.gabsplat_render_forward(ctx, ds, cam, proj, bins, stream=st)
+    st.synchronize()
+    assert np.array_equal(fwd.image.cpu().numpy(), ref["image"])
+
+
+def test_render_host_matches_device_path():
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny")
+    cam = scenes.make_cameras("tiny")[0]
+    dL = scenes.make_image_grad("tiny", 0, cam)
+    ref, _ = run_gpu(scene, cam, dL)
+
+    class H:
+        pass
+    h = H()
+    for n in ("means", "scales", "rotations", "opacities", "sh", "freqs", "weights"):
+        setattr(h, n, torch.from_numpy(getattr(scene, n)).pin_memory())
+    h.sh_degree = 3
+    cap = ref["D"] + 10
+    arena = torch.zeros(gb.host_arena_bytes(scene.N, scene.K, cam, cap), dtype=torch.uint8, device="cuda")
+    img = torch.zeros((3, cam.height, cam.width), dtype=torch.float32).pin_memory()
+    names = ("d_means", "d_scales", "d_rotations", "d_opacities", "d_sh", "d_freqs", "d_weights")
+    grads = {n: torch.zeros(ref[n].shape, dtype=torch.float32).pin_memory() for n in names}
+    gb.gabsplat_render_host(ctx, h, cam, cap, img, torch.from_numpy(dL).pin_memory(), grads, arena)
+    assert np.array_equal(img.numpy(), ref["image"])
+    for n in names:
+        assert np.allclose(grads[n].numpy(), ref[n], rtol=1e-4, atol=1e-6 * np.abs(ref[n]).max())
