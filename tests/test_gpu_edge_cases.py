@@ -11,7 +11,7 @@ pytestmark = pytest.mark.gpu
 def _mods():
     import torch
     from paper_2508_05343_b200 import binding as gb
-    from tests.gpu_helpers import ctx, run_gpu
+    from gpu_helpers import ctx, run_gpu
     return torch, gb, ctx(), run_gpu
 
 

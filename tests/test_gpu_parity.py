@@ -21,7 +21,7 @@ def _oracle():
 
 
 def _gpu(scene, cam, dL=None):
-    from tests.gpu_helpers import run_gpu
+    from gpu_helpers import run_gpu
     return run_gpu(scene, cam, dL)[0]
 
 
@@ -70,7 +70,7 @@ def check_forward(g, o, report=None):
 
 def check_gradients(g, o):
     worst = {}
-    from tests.gpu_helpers import rel_inf
+    from gpu_helpers import rel_inf
     for name in ("d_means", "d_scales", "d_rotations", "d_opacities", "d_sh", "d_freqs", "d_weights", "d_mean2d"):
         worst[name] = rel_inf(g[name], o[name])
     worst["d_mean2d_abs"] = rel_inf(g["d_mean2d_abs"], o["d_absmean2d"])
@@ -172,7 +172,7 @@ def test_partition_of_unity_full_size():
     """Property that holds at any size (reading C23): all colours = background = 1 gives image == 1."""
     import torch
     from paper_2508_05343_b200 import binding as gb
-    from tests.gpu_helpers import ctx
+    from gpu_helpers import ctx
     scene = scenes.make_scene("unbounded", N=200000)
     cam = scenes.make_cameras("unbounded")[1]
     cam.bg = (1.0, 1.0, 1.0)
