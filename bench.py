@@ -1,0 +1,439 @@
+#!/usr/bin/env python
+"""bench.py -- the hot path of 3DGabSplat (forward + backward of the tile rasterizer) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config unbounded] [--impl ours|reference]
+
+One STEP = one pass of the whole hot path (S1 preprocess, S2 bin+sort, S3 blend forward, S4a blend backward,
+S4b projection backward -- SURVEY.md 8(a)) over one camera view of the synthetic scene; consecutive steps
+cycle through the config's 8 seeded views.  The headline workload is BASELINE.json configs[2] ("unbounded":
+1M primitives, K=4, 1297x840), the configuration its `metric` is quoted on.  Metric: forward+backward
+Mpix/s = pixels per view / time per view (forward-only ms/frame is reported beside it).
+
+Prints ONE JSON line (see DESIGN.md "Measurement" for every field).  `--impl reference` times the CPU
+oracle (oracle/, test infrastructure) on the host cores instead: this repository's stand-in for a reference
+implementation, since the paper ships no code.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "fwd+bwd Mpix/s per view (fwd ms/frame and fwd+bwd ms/view beside it) at 1M Gabor primitives, 1297x840"
+UNIT = "Mpix/s"
+
+# ALU roofline constants: 148 SMs x 4 sub-partitions x 32 lanes x 1.965 GHz FP32-pipe
+# lane-instructions per second; MUFU: 16 lanes per SM per clock.
+SM_COUNT, SM_HZ = 148, 1.965e9
+FP32_PEAK = SM_COUNT * 128 * SM_HZ      # lane-instructions / s
+MUFU_PEAK = SM_COUNT * 16 * SM_HZ       # lane-ops / s
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=64)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="unbounded", choices=["tiny", "object", "unbounded", "large"])
+    ap.add_argument("--K", type=int, default=None, help="filter-bank size override (config 5, the K sweep)")
+    ap.add_argument("--zero-weights", action="store_true", help="config 5's all-omega-zero case")
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (profiling runs)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
+    ap.add_argument("--forward-only", action="store_true", help="a step is S1-S3 only (config 2 is forward only)")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    return 6650.0, "fallback"
+
+
+# ----------------------------------------------------------------------------------------------------
+# clocks: nvidia-smi sampled in a thread while the timed region runs
+# ----------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for s in self.samples:
+            f = [x.strip() for x in s.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------------------------------
+# the CPU oracle legs (cpu_baseline of our arm; the whole of --impl reference)
+# ----------------------------------------------------------------------------------------------------
+def crop_camera(cam, y0: int, rows: int):
+    """The same view restricted to image rows [y0, y0+rows): a camera with a shifted principal point."""
+    from paper_2508_05343_b200 import scenes
+    return scenes.Camera(cam.width, rows, cam.fx, cam.fy, cam.cx, float(np.float32(cam.cy - y0)), cam.world_to_cam,
+                         cam.z_near, cam.bg)
+
+
+def oracle_view(orc, scene, cam, dL, backward: bool) -> float:
+    t0 = time.perf_counter()
+    if backward:
+        orc.render_backward(scene, cam, dL)     # runs its own forward first
+    else:
+        orc.render_forward(scene, cam)
+    return time.perf_counter() - t0
+
+
+def run_reference(args, name, scene, cams, rank) -> dict:
+    """--impl reference: the oracle as it stands, on the host cores; each step a band of rows of one view."""
+    from oracle import gabsplat_oracle as orc
+    from paper_2508_05343_b200 import scenes
+    backward = not args.forward_only
+    cores = orc.max_threads()
+    H, W = cams[0].height, cams[0].width
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    cal_rows = min(H, 32)
+    y_mid = max(0, (H // 2) // 16 * 16 - 16)
+    dL0 = scenes.make_image_grad(name, 0, cams[0])
+    t_cal = oracle_view(orc, scene, crop_camera(cams[0], y_mid, cal_rows), dL0[:, y_mid:y_mid + cal_rows], backward)
+    rows = int(min(H, max(16, cal_rows * int(budget / max(t_cal, 1e-6)))))
+    rows = H if rows >= H else rows // 16 * 16
+    times = []
+    for i in range(args.warmup + args.steps):
+        v = i % len(cams)
+        y0 = 0 if rows >= H else (y_mid if y_mid + rows <= H else 0)
+        cam = crop_camera(cams[v], y0, rows) if rows < H else cams[v]
+        dL = scenes.make_image_grad(name, v, cams[v])[:, y0:y0 + rows]
+        dt = oracle_view(orc, scene, cam, np.ascontiguousarray(dL), backward)
+        if i >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    value = rows * W / 1e6 / (ms / 1e3)
+    sample = "rows [%d,%d) of each 1297x840-style view (%d of %d rows) rendered as a cropped camera, %s" % (
+        y0, y0 + rows, rows, H, "forward+backward" if backward else "forward")
+    return {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic (seeded; DESIGN.md 'Input recipe')",
+        "config": workload_config(args, name, scene, cams[0]),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+
+
+def workload_config(args, name, scene, cam) -> dict:
+    return {"workload": "%s: N=%d primitives, K=%d, SH degree 3, %dx%d, 8 seeded views, %s" % (
+                name, scene.N, scene.K, cam.width, cam.height,
+                "forward" if args.forward_only else "forward+backward"),
+            "config_name": name, "N": scene.N, "K": scene.K, "width": cam.width, "height": cam.height,
+            "zero_weights": bool(args.zero_weights),
+            "l2_policy": "inputs larger than L2 (scene %.0f MB + gradients %.0f MB per step vs 126 MB L2)" % (
+                scene.N * (59 + 4 * scene.K) * 4 / 1e6, scene.N * (59 + 4 * scene.K) * 4 / 1e6)}
+
+
+# ----------------------------------------------------------------------------------------------------
+# rooflines
+# ----------------------------------------------------------------------------------------------------
+def stage_work(K, N, stats, tiles, passes) -> dict:
+    """Algorithmic work of every stage for one view."""
+    n_vis, D = stats["n_visible"], stats["D"]
+    E, P, B, Pb, Eb = stats["examined"], stats["envelope"], stats["blended"], stats["envelope_le_last"], stats["walked"]
+    par = (59 + 4 * K) * 4
+    w = {}
+    w["preprocess"] = ("hbm", N * 16 + n_vis * (par - 12 + 49 + 8 * K - 4))
+    w["scan"] = ("hbm", 8 * N)
+    w["duplicate"] = ("hbm", 4 * N + 20 * n_vis + 12 * D)
+    w["sort"] = ("hbm", D * (8 + passes * 24))
+    w["ranges"] = ("hbm", 8 * D + 8 * tiles)
+    w["preprocess_backward"] = ("hbm", n_vis * (par + (9 + 3 * K) * 4) + N * par)
+    # blend: FP32-pipe lane-instructions and MUFU lane-ops
+    f_fp32 = 9 * E + (4 * K + 10) * P
+    f_mufu = (1 + K) * P
+    b_fp32 = 9 * Eb + (4 * K + 10) * Pb + (10 * K + 45) * B
+    b_mufu = (1 + K) * Pb + K * B
+    w["blend_forward"] = ("alu", f_fp32, f_mufu)
+    w["blend_backward"] = ("alu", b_fp32, b_mufu)
+    return w
+
+
+def roofline_entry(work, ms, hbm_peak, peak_kind) -> dict:
+    t = ms / 1e3
+    if work[0] == "hbm":
+        ach = work[1] / t / 1e9
+        return {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                "traffic": None, "peak_kind": peak_kind, "algorithmic_bytes": int(work[1])}
+    fp32, mufu = work[1], work[2]
+    t_peak = max(fp32 / FP32_PEAK, mufu / MUFU_PEAK)
+    ach = fp32 / t / 1e12
+    return {"bound": "alu", "achieved": ach, "peak": FP32_PEAK / 1e12, "unit": "Tinstr/s (FP32-pipe lane-instructions)",
+            "frac": t_peak / t, "traffic": None, "peak_kind": "derived: 148 SM x 128 lanes x 1.965 GHz; MUFU 16 lanes/SM",
+            "algorithmic_fp32_instr": int(fp32), "algorithmic_mufu_ops": int(mufu),
+            "time_at_peak_ms": 1e3 * t_peak}
+
+
+# ----------------------------------------------------------------------------------------------------
+# our arm
+# ----------------------------------------------------------------------------------------------------
+def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
+    import torch
+    from paper_2508_05343_b200 import binding as gb, scenes
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    ctx = gb.Context(local_rank)
+    backward = not args.forward_only
+    N, K = scene.N, scene.K
+    V = len(cams)
+    H, W = cams[0].height, cams[0].width
+    tiles = cams[0].tiles_x * cams[0].tiles_y
+    passes = (32 + max(1, (tiles - 1).bit_length()) + 7) // 8
+
+    ds = gb.upload_scene(scene, dev)
+    dLs = [torch.from_numpy(scenes.make_image_grad(name, v, cams[v])).to(dev) for v in range(V)] if backward else None
+    proj = gb.Projected(N, K, dev)
+
+    # dry run per view (untimed): instance counts for the capacity, and the roofline numerators
+    stats = []
+    probe = gb.Binning(N, cams[0], 0, dev)
+    Ds = []
+    for v in range(V):
+        gb.gabsplat_preprocess(ctx, ds, cams[v], proj)
+        b = gb.gabsplat_bin_sort(ctx, N, proj, cams[v], capacity=None)
+        Ds.append(b.D)
+        fwd = gb.gabsplat_render_forward(ctx, ds, cams[v], proj, b)
+        cnt = gb.gabsplat_count_pairs(ctx, ds, cams[v], proj, b).to(torch.int64).reshape(-1, 4).sum(0).tolist()
+        stats.append({"n_visible": int((proj.tiles_touched != 0).sum().item()), "D": b.D, "examined": cnt[0],
+                      "envelope": cnt[1], "blended": cnt[2], "envelope_le_last": cnt[3],
+                      "walked": int(fwd.n_contrib.to(torch.int64).sum().item())})
+        del b, fwd
+    del probe
+    capacity = max(Ds)
+    bins = gb.Binning(N, cams[0], capacity, dev)
+    fwd = gb.FwdOut(cams[0], dev)
+    grads = gb.Grads(N, K, dev, with_mean2d=False) if backward else None
+
+    my_view = lambda i: (i + rank) % V
+
+    def step(i, do_backward):
+        v = my_view(i)
+        gb.gabsplat_preprocess(ctx, ds, cams[v], proj)
+        gb.gabsplat_bin_sort(ctx, N, proj, cams[v], bin=bins, read_count=False)
+        gb.gabsplat_render_forward(ctx, ds, cams[v], proj, bins, fwd)
+        if do_backward:
+            gb.gabsplat_render_backward(ctx, ds, cams[v], proj, bins, fwd, dLs[v], grads)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(n, do_backward, with_stage_timing):
+        for i in range(args.warmup):
+            step(i, do_backward)
+        barrier()
+        if with_stage_timing:
+            gb.gabsplat_timing_enable(ctx, True)
+        l0 = gb.gabsplat_kernel_launches()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(n):
+            step(i, do_backward)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        launches = gb.gabsplat_kernel_launches() - l0
+        recs = gb.gabsplat_timing_read(ctx) if with_stage_timing else []
+        gb.gabsplat_timing_enable(ctx, False)
+        if dist is not None:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, launches, recs
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    total_ms, launches, recs = timed(args.steps, backward, True)
+    clocks = sampler.stop() if rank == 0 else None
+    fwd_ms, _, _ = timed(args.steps, False, False) if backward else (total_ms, 0, [])
+    ms_per_step = total_ms / args.steps
+    value = world * H * W / 1e6 / (ms_per_step / 1e3)
+
+    # per-stage means over the timed region; the views of the timed steps weight the numerators
+    stage_ms = {}
+    for s, ms in recs:
+        stage_ms.setdefault(s, []).append(ms)
+    views_timed = [my_view(i) for i in range(args.steps)]
+    mean_stats = {k: float(np.mean([stats[v][k] for v in views_timed])) for k in stats[0]}
+    hbm_peak, peak_kind = peaks()
+    work = stage_work(K, N, mean_stats, tiles, passes)
+    per_stage = {}
+    for s, lst in stage_ms.items():
+        m = float(np.mean(lst))
+        per_stage[s] = {"ms": m, "share": m * len(lst) / args.steps / ms_per_step, **roofline_entry(work[s], m, hbm_peak, peak_kind)}
+    dominant = max(per_stage, key=lambda s: per_stage[s]["ms"])
+    roofline = {"kernel": dominant, **{k: per_stage[dominant][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
+                "peak_kind": per_stage[dominant]["peak_kind"]}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")   # ncu-measured DRAM bytes per launch, if recorded
+    if os.path.exists(traffic_file):
+        with open(traffic_file) as f:
+            tr = json.load(f)
+        for s in per_stage:
+            if s in tr.get(name, {}):
+                per_stage[s]["traffic"] = tr[name][s]
+        roofline["traffic"] = per_stage[dominant]["traffic"]
+
+    # end to end through the C ABI with HOST buffers (gabsplat_render_host): H2D of the scene and dL/dimage,
+    # D2H of the image and the gradients, all inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        class HostScene:
+            pass
+        hs = HostScene()
+        for n in ("means", "scales", "rotations", "opacities", "sh", "freqs", "weights"):
+            setattr(hs, n, pin(getattr(scene, n)))
+        hs.sh_degree = scene.sh_degree
+        img_h = torch.zeros((3, H, W), dtype=torch.float32).pin_memory()
+        dL_h = [pin(scenes.make_image_grad(name, v, cams[v])) for v in range(V)] if backward else None
+        g_h = None
+        if backward:
+            g_h = {"d_means": (N, 3), "d_scales": (N, 3), "d_rotations": (N, 4), "d_opacities": (N,),
+                   "d_sh": (N, 16, 3), "d_freqs": (N, K, 3), "d_weights": (N, K)}
+            g_h = {k: torch.zeros(s, dtype=torch.float32).pin_memory() for k, s in g_h.items()}
+        del bins, fwd, grads, proj
+        torch.cuda.empty_cache()
+        arena = torch.zeros((gb.host_arena_bytes(N, K, cams[0], capacity),), dtype=torch.uint8, device=dev)
+        n_e2e = max(1, min(args.steps, 8))
+
+        def e2e_step(i):
+            v = my_view(i)
+            gb.gabsplat_render_host(ctx, hs, cams[v], capacity, img_h, dL_h[v] if backward else None, g_h, arena)
+
+        for i in range(min(args.warmup, 3)):
+            e2e_step(i)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(n_e2e):
+            e2e_step(i)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        par_bytes = N * (59 + 4 * K) * 4
+        e2e = {"value": world * H * W / 1e6 / (ms / n_e2e / 1e3), "unit": UNIT, "ms_per_step": ms / n_e2e, "steps": n_e2e,
+               "h2d_bytes_per_step": par_bytes + (3 * H * W * 4 if backward else 0),
+               "d2h_bytes_per_step": 3 * H * W * 4 + (par_bytes if backward else 0),
+               "api": "gabsplat_render_host (pinned host buffers in, image + gradients out)"}
+
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return None
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic (seeded; DESIGN.md 'Input recipe')",
+        "config": workload_config(args, name, scene, cams[0]),
+        "fwd_ms_per_frame": fwd_ms / args.steps, "fwd_bwd_ms_per_view": ms_per_step if backward else None,
+        "fwd_mpix_per_s": world * H * W / 1e6 / (fwd_ms / args.steps / 1e3),
+        "roofline": roofline, "roofline_per_stage": per_stage,
+        "work_per_view": {k: mean_stats[k] for k in mean_stats},
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "multi_gpu": "replicas only: each rank renders its own views of a replicated scene, no data-path collective",
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import gabsplat_oracle as orc
+        dL0 = scenes.make_image_grad(name, 0, cams[0])
+        dt = oracle_view(orc, scene, cams[0], dL0, backward)
+        out["cpu_baseline"] = {"value": H * W / 1e6 / dt, "unit": UNIT, "cores": orc.max_threads(), "kind": "oracle",
+                               "ms_per_view": 1e3 * dt,
+                               "sample": "view 0 of the same workload, full frame, %s, run once" % (
+                                   "forward+backward" if backward else "forward")}
+    return out
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference" and rank != 0:
+        return 0
+    from paper_2508_05343_b200 import scenes
+    name = args.config
+    scene = scenes.make_scene(name, K=args.K, zero_weights=args.zero_weights)
+    cams = scenes.make_cameras(name)
+    if len(cams) == 1:
+        cams = cams * 8
+    if args.impl == "reference":
+        out = run_reference(args, name, scene, cams, rank)
+    else:
+        out = run_ours(args, name, scene, cams, rank, world, local_rank)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -172,6 +172,39 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* scene_host
                              uint64_t capacity, float* image_host, const float* dL_dimage_host,
                              gabsplat_grads* grads_host, void* device_arena, uint64_t arena_bytes, void* stream);
 
+/* ---- instrumentation (used by bench.py and the tests; none of it is needed to render) ----------------
+ *
+ * Per-stage device timing.  While enabled, every stage launched by the four calls above is bracketed by a
+ * pair of CUDA events recorded on the stream of the call.  gabsplat_timing_read waits for the recorded
+ * events, writes up to max_records (stage id, elapsed milliseconds) pairs in launch order, stores the
+ * number of records that existed in *n_records, and clears the record list.  Host calls. */
+#define GABSPLAT_STAGE_PREPROCESS 0      /* S1  projection kernel                                   */
+#define GABSPLAT_STAGE_SCAN 1            /* S2a prefix sum of tiles_touched                          */
+#define GABSPLAT_STAGE_DUPLICATE 2       /* S2b key emission                                        */
+#define GABSPLAT_STAGE_SORT 3            /* S2c all radix passes                                    */
+#define GABSPLAT_STAGE_RANGES 4          /* S2d tile ranges (incl. clearing them)                   */
+#define GABSPLAT_STAGE_BLEND_FORWARD 5   /* S3                                                      */
+#define GABSPLAT_STAGE_BLEND_BACKWARD 6  /* S4a (incl. zeroing the 2D gradient records)             */
+#define GABSPLAT_STAGE_PREPROCESS_BACKWARD 7 /* S4b (incl. zeroing the gradient outputs)             */
+#define GABSPLAT_STAGE_COUNT 8
+int32_t gabsplat_timing_enable(gabsplat_ctx* ctx, int32_t on);
+int32_t gabsplat_timing_read(gabsplat_ctx* ctx, int32_t* stage_ids_host, float* ms_host, int32_t max_records,
+                             int32_t* n_records_host);
+
+/* Number of CUDA kernels this library has launched in this process so far (host counter). */
+uint64_t gabsplat_kernel_launches(void);
+
+/* Per-pixel work counters of the forward blend, the numerators of the blend kernels' roofline
+ * (DESIGN.md "Rooflines"): counters is a DEVICE array [H][W][4] of
+ *   [0] pairs examined  -- list entries visited before the pixel stopped (the stopping entry included),
+ *   [1] pairs that pass the envelope test o G >= 1/255 (the ones whose K cosines must be evaluated),
+ *   [2] pairs blended,
+ *   [3] envelope-passing pairs at list positions <= the last contributor (what the backward re-evaluates).
+ * Same arguments as gabsplat_render_forward; runs a counting variant of the blend kernel. */
+int32_t gabsplat_count_pairs(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                             const gabsplat_projected* proj, const gabsplat_binning* bin, uint32_t* counters,
+                             void* stream);
+
 #ifdef __cplusplus
 }
 #endif

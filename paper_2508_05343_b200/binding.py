@@ -94,8 +94,15 @@ def lib():
                                                C.c_uint64, P]
         L.gabsplat_render_host.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.c_uint64, P, P,
                                            C.POINTER(_Grads), P, C.c_uint64, P]
+        L.gabsplat_kernel_launches.argtypes = []
+        L.gabsplat_kernel_launches.restype = C.c_uint64
+        L.gabsplat_timing_enable.argtypes = [P, C.c_int32]
+        L.gabsplat_timing_read.argtypes = [P, C.POINTER(C.c_int32), C.POINTER(C.c_float), C.c_int32,
+                                           C.POINTER(C.c_int32)]
+        L.gabsplat_count_pairs.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
+                                           C.POINTER(_Binning), P, P]
         for f in (L.gabsplat_preprocess, L.gabsplat_bin_sort, L.gabsplat_render_forward, L.gabsplat_render_backward,
-                  L.gabsplat_render_host):
+                  L.gabsplat_render_host, L.gabsplat_timing_enable, L.gabsplat_timing_read, L.gabsplat_count_pairs):
             f.restype = C.c_int32
         _lib = L
     return _lib
@@ -343,6 +350,37 @@ def gabsplat_render_host(ctx: Context, scene, cam, capacity: int, image_host: to
     ctx.check(lib().gabsplat_render_host(ctx._h, C.byref(s), C.byref(c), int(capacity), _ptr(image_host),
                                          _ptr(dL_dimage_host), C.byref(g) if grads_host is not None else None,
                                          C.c_void_p(base), nbytes, _stream(stream)))
+
+
+STAGES = ("preprocess", "scan", "duplicate", "sort", "ranges", "blend_forward", "blend_backward",
+          "preprocess_backward")
+
+
+def gabsplat_kernel_launches() -> int:
+    return int(lib().gabsplat_kernel_launches())
+
+
+def gabsplat_timing_enable(ctx: Context, on: bool) -> None:
+    ctx.check(lib().gabsplat_timing_enable(ctx._h, 1 if on else 0))
+
+
+def gabsplat_timing_read(ctx: Context, max_records: int = 1 << 16) -> list[tuple[str, float]]:
+    """(stage name, milliseconds) of every stage launched since timing was enabled / last read."""
+    ids = (C.c_int32 * max_records)()
+    ms = (C.c_float * max_records)()
+    n = C.c_int32(0)
+    ctx.check(lib().gabsplat_timing_read(ctx._h, ids, ms, max_records, C.byref(n)))
+    return [(STAGES[ids[i]], float(ms[i])) for i in range(min(n.value, max_records))]
+
+
+def gabsplat_count_pairs(ctx: Context, scene: DeviceScene, cam, proj: Projected, bin: Binning, stream=None) -> torch.Tensor:
+    """[H][W][4] int32 per-pixel counters (examined, past the envelope test, blended, past the envelope
+    test at positions <= the last contributor)."""
+    out = torch.zeros((cam.height, cam.width, 4), dtype=torch.int32, device=scene.means.device)
+    s, c, p, b = scene.struct(), camera_struct(cam), proj.struct(), bin.struct()
+    ctx.check(lib().gabsplat_count_pairs(ctx._h, C.byref(s), C.byref(c), C.byref(p), C.byref(b), _ptr(out),
+                                         _stream(stream)))
+    return out
 
 
 def host_arena_bytes(N: int, K: int, cam, capacity: int) -> int:

@@ -9,8 +9,13 @@
 struct gabsplat_ctx {
   int device;
   uint64_t* pinned_count;  // 8-byte pinned readback slot for D
+  gabsplat::StageTimer timer;
   char error[256];
 };
+
+namespace gabsplat {
+unsigned long long g_kernel_launches = 0;
+}
 
 namespace {
 
@@ -90,6 +95,7 @@ int32_t gabsplat_create(gabsplat_ctx** out, int32_t device) {
 void gabsplat_destroy(gabsplat_ctx* ctx) {
   if (!ctx) return;
   if (ctx->pinned_count) cudaFreeHost(ctx->pinned_count);
+  ctx->timer.destroy();
   delete ctx;
 }
 
@@ -112,7 +118,9 @@ int32_t gabsplat_preprocess(gabsplat_ctx* ctx, const gabsplat_scene* scene, cons
   if (!scene_ok(scene)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess: bad scene");
   if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess: bad camera");
   if (!projected_ok(out, scene->N, scene->K)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess: null output");
+  ctx->timer.begin(GABSPLAT_STAGE_PREPROCESS, (cudaStream_t)stream);
   const cudaError_t e = launch_preprocess(*scene, make_camera(*cam), *out, (cudaStream_t)stream);
+  ctx->timer.end((cudaStream_t)stream);
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "preprocess");
 }
 
@@ -126,7 +134,7 @@ int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected
   if (!bin->workspace || bin->workspace_bytes < sort_workspace_bytes(N, bin->capacity))
     return fail(ctx, GABSPLAT_CAPACITY, "bin_sort: workspace too small");
   cudaStream_t st = (cudaStream_t)stream;
-  cudaError_t e = launch_bin_sort(N, *proj, make_camera(*cam), *bin, st);
+  cudaError_t e = launch_bin_sort(N, *proj, make_camera(*cam), *bin, ctx->timer, st);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "bin_sort");
   if (num_instances_host) {
     uint32_t* slot = reinterpret_cast<uint32_t*>(ctx->pinned_count);
@@ -148,7 +156,9 @@ int32_t gabsplat_render_forward(gabsplat_ctx* ctx, const gabsplat_scene* scene, 
   if (!proj || (scene->N > 0 && !proj->packed)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: null packed records");
   if (!bin || !bin->tile_ranges || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: bad binning");
   if (!out || !out->image || !out->final_T || !out->n_contrib) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: null output");
+  ctx->timer.begin(GABSPLAT_STAGE_BLEND_FORWARD, (cudaStream_t)stream);
   const cudaError_t e = launch_blend_forward(scene->K, make_camera(*cam), *proj, *bin, *out, (cudaStream_t)stream);
+  ctx->timer.end((cudaStream_t)stream);
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "render_forward");
 }
 
@@ -171,10 +181,54 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
   cudaStream_t st = (cudaStream_t)stream;
   const Camera c = make_camera(*cam);
   float* grad2d = reinterpret_cast<float*>(((uintptr_t)grad_workspace + 255) & ~(uintptr_t)255);
+  ctx->timer.begin(GABSPLAT_STAGE_BLEND_BACKWARD, st);
   cudaError_t e = launch_blend_backward(scene->N, scene->K, c, *proj, *bin, *fwd, dL_dimage, grad2d, st);
+  ctx->timer.end(st);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "render_backward (blend)");
+  ctx->timer.begin(GABSPLAT_STAGE_PREPROCESS_BACKWARD, st);
   e = launch_preprocess_backward(*scene, c, *proj, grad2d, *grads, st);
+  ctx->timer.end(st);
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "render_backward (projection)");
+}
+
+uint64_t gabsplat_kernel_launches(void) { return g_kernel_launches; }
+
+int32_t gabsplat_timing_enable(gabsplat_ctx* ctx, int32_t on) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  ctx->timer.on = on != 0;
+  ctx->timer.reset();
+  return GABSPLAT_OK;
+}
+
+int32_t gabsplat_timing_read(gabsplat_ctx* ctx, int32_t* stage_ids_host, float* ms_host, int32_t max_records,
+                             int32_t* n_records_host) {
+  if (!ctx || !n_records_host || max_records < 0 || (max_records > 0 && (!stage_ids_host || !ms_host)))
+    return GABSPLAT_INVALID_ARG;
+  StageTimer& tm = ctx->timer;
+  *n_records_host = (int32_t)tm.recs.size();
+  for (size_t i = 0; i < tm.recs.size() && (int32_t)i < max_records; ++i) {
+    cudaError_t e = cudaEventSynchronize(tm.recs[i].b);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, tm.recs[i].a, tm.recs[i].b);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "timing_read");
+    stage_ids_host[i] = tm.recs[i].stage;
+    ms_host[i] = ms;
+  }
+  tm.reset();
+  return GABSPLAT_OK;
+}
+
+int32_t gabsplat_count_pairs(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                             const gabsplat_projected* proj, const gabsplat_binning* bin, uint32_t* counters,
+                             void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  if (!scene || scene->K < 0 || scene->K > kMaxK || scene->N < 0) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: bad scene");
+  if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: bad camera");
+  if (!proj || (scene->N > 0 && !proj->packed)) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: null packed records");
+  if (!bin || !bin->tile_ranges || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: bad binning");
+  if (!counters) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: null output");
+  const cudaError_t e = launch_count_pairs(scene->K, make_camera(*cam), *proj, *bin, counters, (cudaStream_t)stream);
+  return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "count_pairs");
 }
 
 }  // extern "C"

@@ -128,11 +128,15 @@ void device_scan(const u32* in, u32* out, u32 n, u32* sums, u32* total_out, cuda
   const u32 nb = scan_blocks(n);
   if (nb == 0) {
     scan_of_sums<<<1, kScanThreads, 0, st>>>(sums, 0, total_out);
+    launched();
     return;
   }
   scan_block_sums<<<nb, kScanThreads, 0, st>>>(in, n, sums);
+  launched();
   scan_of_sums<<<1, kScanThreads, 0, st>>>(sums, nb, total_out);
+  launched();
   scan_apply<INCLUSIVE><<<nb, kScanThreads, 0, st>>>(in, n, sums, out);
+  launched();
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -338,14 +342,19 @@ Workspace carve(void* base, int N, u64 capacity) {
 uint64_t sort_workspace_bytes(int N, uint64_t capacity) { return carve(nullptr, N, capacity).bytes; }
 
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
-                            cudaStream_t st) {
+                            StageTimer& tm, cudaStream_t st) {
   const Workspace ws = carve(bin.workspace, N, bin.capacity);
   const int ntiles = cam.tiles_x * cam.tiles_y;
-  cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
   // K2
+  tm.begin(GABSPLAT_STAGE_SCAN, st);
   device_scan<true>(proj.tiles_touched, bin.offsets, (u32)N, ws.scan_sums, bin.num_instances, st);
-  if (N == 0 || bin.capacity == 0) return cudaGetLastError();
+  tm.end(st);
+  if (N == 0 || bin.capacity == 0) {
+    cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
+    return cudaGetLastError();
+  }
   clamp_count_kernel<<<1, 1, 0, st>>>(ws.sort_count, bin.num_instances, bin.capacity);
+  launched();
   // number of one-byte passes: 32 depth bits + bits of the largest tile id
   int tile_bits = 0;
   while ((1 << tile_bits) < ntiles) ++tile_bits;
@@ -354,22 +363,33 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   u32* vbuf[2] = {bin.ids, ws.ids_alt};
   int cur = passes & 1;  // an odd number of passes starts in the alternate buffer so the result lands in bin.keys
   // K3
+  tm.begin(GABSPLAT_STAGE_DUPLICATE, st);
   duplicate_kernel<<<(N + kDupThreads - 1) / kDupThreads, kDupThreads, 0, st>>>(
       N, cam.tiles_x, bin.offsets, proj.tiles_touched, reinterpret_cast<const int4*>(proj.rect), proj.depth,
       bin.num_instances, bin.capacity, kbuf[cur], vbuf[cur]);
+  launched();
+  tm.end(st);
   // K4
+  tm.begin(GABSPLAT_STAGE_SORT, st);
   const u32 nblocks = (u32)((bin.capacity + kSortTile - 1) / kSortTile);
   for (int p = 0; p < passes; ++p) {
     const int shift = 8 * p;
     sort_histogram<<<nblocks, kSortThreads, 0, st>>>(kbuf[cur], ws.sort_count, ws.table, nblocks, shift);
+    launched();
     device_scan<false>(ws.table, ws.table, 256u * nblocks, ws.scan_sums, nullptr, st);
     sort_scatter<<<nblocks, kSortThreads, 0, st>>>(kbuf[cur], vbuf[cur], kbuf[cur ^ 1], vbuf[cur ^ 1], ws.sort_count,
                                                    ws.table, nblocks, shift);
+    launched();
     cur ^= 1;
   }
+  tm.end(st);
   // K5
+  tm.begin(GABSPLAT_STAGE_RANGES, st);
+  cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
   tile_ranges_kernel<<<148 * 8, 256, 0, st>>>(bin.keys, bin.num_instances, bin.capacity,
                                               reinterpret_cast<uint2*>(bin.tile_ranges));
+  launched();
+  tm.end(st);
   return cudaGetLastError();
 }
 

@@ -150,6 +150,7 @@ cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const ga
   blend_backward_kernel<K><<<ntiles, kBlock, 0, st>>>(cam, reinterpret_cast<const uint2*>(bin.tile_ranges), bin.ids,
                                                        reinterpret_cast<const float4*>(proj.packed), fwd.final_T,
                                                        fwd.n_contrib, dL, grad2d);
+  launched();
   return cudaGetLastError();
 }
 

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "../../include/gabsplat.h"
 
 namespace gabsplat {
@@ -52,13 +54,54 @@ inline Camera make_camera(const gabsplat_camera& c) {
   return k;
 }
 
+// ---- optional per-stage device timing (gabsplat_timing_enable / gabsplat_timing_read) -------------
+// When enabled, every stage is bracketed by a pair of CUDA events recorded on the stream of the call;
+// the records are read back (elapsed ms per stage launch) by gabsplat_timing_read.
+struct StageTimer {
+  struct Rec { int stage; cudaEvent_t a, b; };
+  bool on = false;
+  std::vector<cudaEvent_t> pool;
+  size_t used = 0;
+  std::vector<Rec> recs;
+  cudaEvent_t take() {
+    if (used == pool.size()) {
+      cudaEvent_t e = nullptr;
+      cudaEventCreate(&e);
+      pool.push_back(e);
+    }
+    return pool[used++];
+  }
+  void begin(int stage, cudaStream_t st) {
+    if (!on) return;
+    Rec r{stage, take(), take()};
+    cudaEventRecord(r.a, st);
+    recs.push_back(r);
+  }
+  void end(cudaStream_t st) {
+    if (!on || recs.empty()) return;
+    cudaEventRecord(recs.back().b, st);
+  }
+  void reset() { recs.clear(); used = 0; }
+  void destroy() {
+    for (cudaEvent_t e : pool) cudaEventDestroy(e);
+    pool.clear();
+    reset();
+  }
+};
+
+// Number of kernels launched by this library since it was loaded (gabsplat_kernel_launches).
+extern unsigned long long g_kernel_launches;
+inline void launched(int n = 1) { g_kernel_launches += (unsigned long long)n; }
+
 // ---- launchers (one per .cu file); each returns the cudaError_t of its last launch ---------------
 cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& out,
                               cudaStream_t st);
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
-                            cudaStream_t st);
+                            StageTimer& tm, cudaStream_t st);
 cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projected& proj,
                                  const gabsplat_binning& bin, const gabsplat_fwd_out& out, cudaStream_t st);
+cudaError_t launch_count_pairs(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
+                               uint32_t* counters, cudaStream_t st);
 cudaError_t launch_blend_backward(int N, int K, const Camera& cam, const gabsplat_projected& proj,
                                   const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const float* dL_dimage,
                                   float* grad2d, cudaStream_t st);

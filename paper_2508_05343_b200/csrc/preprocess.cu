@@ -254,6 +254,7 @@ cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const 
   if (s.N == 0) return cudaSuccess;
   const int block = 256;
   preprocess_kernel<<<(s.N + block - 1) / block, block, 0, st>>>(s, cam, out);
+  launched();
   return cudaGetLastError();
 }
 

@@ -233,6 +233,7 @@ cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& ca
   const int block = 128;
   preprocess_backward_kernel<<<(s.N + block - 1) / block, block, 0, st>>>(s, cam, proj.tiles_touched, proj.rgb_clamped,
                                                                        grad2d, g);
+  launched();
   return cudaGetLastError();
 }
 

@@ -183,3 +183,38 @@ def test_partition_of_unity_full_size():
     fwd = gb.gabsplat_render_forward(ctx(), ds, cam, proj, bins)
     torch.cuda.synchronize()
     assert float((fwd.image - 1.0).abs().max()) < 2e-5
+
+
+def test_pair_counters_and_stage_timing():
+    """gabsplat_count_pairs (the roofline numerators) against the oracle's per-pixel counters, and the stage
+    timer: one record per stage per call, in launch order."""
+    import torch
+    from paper_2508_05343_b200 import binding as gb
+    from gpu_helpers import ctx
+    orc = _oracle()
+    scene = scenes.make_scene("tiny")
+    cam = scenes.make_cameras("tiny")[0]
+    dL = scenes.make_image_grad("tiny", 0, cam)
+    c = ctx()
+    ds = gb.upload_scene(scene)
+    l0 = gb.gabsplat_kernel_launches()
+    gb.gabsplat_timing_enable(c, True)
+    proj = gb.gabsplat_preprocess(c, ds, cam)
+    bins = gb.gabsplat_bin_sort(c, ds.N, proj, cam, capacity=8192)
+    fwd = gb.gabsplat_render_forward(c, ds, cam, proj, bins)
+    gb.gabsplat_render_backward(c, ds, cam, proj, bins, fwd, torch.from_numpy(dL).cuda())
+    recs = gb.gabsplat_timing_read(c)
+    gb.gabsplat_timing_enable(c, False)
+    assert [r[0] for r in recs] == list(gb.STAGES)
+    assert all(ms > 0 for _, ms in recs)
+    assert gb.gabsplat_kernel_launches() - l0 >= len(gb.STAGES)
+    assert gb.gabsplat_timing_read(c) == []
+    cnt = gb.gabsplat_count_pairs(c, ds, cam, proj, bins).cpu().numpy().astype(np.int64)
+    o = orc.render_forward(scene, cam)
+    dec = np.minimum(o["margin"][..., 0], o["margin"][..., 1]) > DELTA
+    oc = o["counters"].astype(np.int64)
+    assert np.array_equal(cnt[..., 0][dec], oc[..., 0][dec])          # examined
+    assert np.array_equal(cnt[..., 2][dec], oc[..., 2][dec])          # blended
+    # the envelope test is a threshold on exp(): equal up to borderline pairs
+    assert abs(int(cnt[..., 1].sum()) - int(oc[..., 1].sum())) <= 1e-3 * oc[..., 1].sum()
+    assert np.all(cnt[..., 3] <= cnt[..., 1]) and np.all(cnt[..., 2] <= cnt[..., 3])
