@@ -182,7 +182,7 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
   const Camera c = make_camera(*cam);
   float* grad2d = reinterpret_cast<float*>(((uintptr_t)grad_workspace + 255) & ~(uintptr_t)255);
   ctx->timer.begin(GABSPLAT_STAGE_BLEND_BACKWARD, st);
-  cudaError_t e = launch_blend_backward(scene->N, scene->K, c, *proj, *bin, *fwd, dL_dimage, grad2d, st);
+  cudaError_t e = launch_blend_backward(scene->N, scene->K, grads->d_mean2d_abs != nullptr, c, *proj, *bin, *fwd, dL_dimage, grad2d, st);
   ctx->timer.end(st);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "render_backward (blend)");
   ctx->timer.begin(GABSPLAT_STAGE_PREPROCESS_BACKWARD, st);

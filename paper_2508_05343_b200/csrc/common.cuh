@@ -20,19 +20,19 @@ constexpr int kMaxK = GABSPLAT_MAX_K;
 
 // ---- packed gather record (gabsplat_projected.packed), floats -----------------------------------
 //  [0..3]   mean2d hi.x, hi.y (fp32 mean, the indexing value), lo.x, lo.y (fp64 residual)
-//  [4..7]   L11, L21, L22 (sqrt(1/2) * Cholesky factor of the conic: q = -(u^2+v^2), u = L11 dx + L21 dy,
+//  [4..7]   L11, L21, L22 (sqrt(1/2) * Cholesky factor of the conic: q = -(u^2 + v^2), u = L11 dx + L21 dy,
 //           v = L22 dy), qmin = -ln(255 o) - margin   (envelope reject: skip when q < qmin)
 //  [8..11]  opacity, r, g, b
-//  [12..]   f2D (x,y) * K, padded to a multiple of 4 floats; then omega * K, padded to a multiple of 4
-__host__ __device__ constexpr int freq_floats(int K) { return 4 * ((2 * K + 3) / 4); }
-__host__ __device__ constexpr int weight_floats(int K) { return 4 * ((K + 3) / 4); }
-__host__ __device__ constexpr int packed_floats(int K) { return 12 + freq_floats(K) + weight_floats(K); }
-__host__ __device__ constexpr int weight_offset(int K) { return 12 + freq_floats(K); }
+//  [12..]   tail: 2 pi f2D (x,y) * K (radians per pixel), then omega * K; padded to a multiple of 4 floats
+__host__ __device__ constexpr int tail_floats(int K) { return 4 * ((3 * K + 3) / 4); }
+__host__ __device__ constexpr int packed_floats(int K) { return 12 + tail_floats(K); }
 
 // ---- 2D gradient record accumulated by the blend backward (grad workspace), floats ---------------
-//  [0..1] d mean2d   [2..4] d conic (a,b,c)   [5] d opacity   [6..8] d rgb   [9..10] sum |d mean2d|  [11] pad
-//  [12..] d f2D (x,y) * K padded to 4; then d omega * K padded to 4     (same tail layout as the packed record)
-__host__ __device__ constexpr int grad2d_floats(int K) { return packed_floats(K); }
+//  [0..1] d mean2d   [2..4] d conic (a,b,c)   [5] d opacity   [6..8] d rgb
+//  [9..9+2K) d (2 pi f2D) (x,y) * K   [9+2K..9+3K) d omega * K   [9+3K..11+3K) sum |d mean2d| (AbsGS statistic)
+//  padded to a multiple of 4 floats
+__host__ __device__ constexpr int grad2d_values(int K) { return 11 + 3 * K; }
+__host__ __device__ constexpr int grad2d_floats(int K) { return 4 * ((grad2d_values(K) + 3) / 4); }
 
 struct Camera {  // device copy of gabsplat_camera plus derived integers
   int width, height, tiles_x, tiles_y;
@@ -102,7 +102,7 @@ cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projec
                                  const gabsplat_binning& bin, const gabsplat_fwd_out& out, cudaStream_t st);
 cudaError_t launch_count_pairs(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
                                uint32_t* counters, cudaStream_t st);
-cudaError_t launch_blend_backward(int N, int K, const Camera& cam, const gabsplat_projected& proj,
+cudaError_t launch_blend_backward(int N, int K, bool want_abs, const Camera& cam, const gabsplat_projected& proj,
                                   const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const float* dL_dimage,
                                   float* grad2d, cudaStream_t st);
 cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& proj,

@@ -229,21 +229,20 @@ __global__ void __launch_bounds__(256) preprocess_kernel(gabsplat_scene s, Camer
   // frequencies: f2D_k = U^-1 T Sigma f_k  (U undilated)
   {
     const double iu = 1.0 / (U00 * U11 - U01 * U01);
-    const int wo = weight_offset(K);
+    const double two_pi = 6.283185307179586476925286766559;
     for (int k = 0; k < K; ++k) {
       const float* f = s.freqs + ((size_t)i * K + k) * 3;
       const double f0 = f[0], f1 = f[1], f2 = f[2];
       const double g0 = V[0][0] * f0 + V[0][1] * f1 + V[0][2] * f2;
       const double g1 = V[1][0] * f0 + V[1][1] * f1 + V[1][2] * f2;
-      const float fx2 = (float)((U11 * g0 - U01 * g1) * iu), fy2 = (float)((U00 * g1 - U01 * g0) * iu);
-      out.freq2d[((size_t)i * K + k) * 2] = fx2;
-      out.freq2d[((size_t)i * K + k) * 2 + 1] = fy2;
-      rec[12 + 2 * k] = fx2;
-      rec[12 + 2 * k + 1] = fy2;
-      rec[wo + k] = s.weights[(size_t)i * K + k];
+      const double fx2 = (U11 * g0 - U01 * g1) * iu, fy2 = (U00 * g1 - U01 * g0) * iu;
+      out.freq2d[((size_t)i * K + k) * 2] = (float)fx2;
+      out.freq2d[((size_t)i * K + k) * 2 + 1] = (float)fy2;
+      rec[12 + 2 * k] = (float)(two_pi * fx2);      // the blend kernels work in radians per pixel
+      rec[12 + 2 * k + 1] = (float)(two_pi * fy2);
+      rec[12 + 2 * K + k] = s.weights[(size_t)i * K + k];
     }
-    for (int k = 2 * K; k < freq_floats(K); ++k) rec[12 + k] = 0.f;
-    for (int k = K; k < weight_floats(K); ++k) rec[wo + k] = 0.f;
+    for (int k = 3 * K; k < tail_floats(K); ++k) rec[12 + k] = 0.f;
   }
 }
 

@@ -82,11 +82,12 @@ __global__ void __launch_bounds__(128) preprocess_backward_kernel(gabsplat_scene
   {
     const double iu = 1.0 / (U00 * U11 - U01 * U01);
     const double Ui00 = U11 * iu, Ui01 = -U01 * iu, Ui11 = U00 * iu;
-    const int wo = weight_offset(K);
+    const int wo = 9 + 2 * K;
+    const double two_pi = 6.283185307179586476925286766559;  // grad2d holds d/d(2 pi f2D)
     for (int k = 0; k < K; ++k) {
       const float* fp = s.freqs + ((size_t)i * K + k) * 3;
       const double f[3] = {fp[0], fp[1], fp[2]};
-      const double gf0 = g2[12 + 2 * k], gf1 = g2[12 + 2 * k + 1];
+      const double gf0 = two_pi * (double)g2[9 + 2 * k], gf1 = two_pi * (double)g2[9 + 2 * k + 1];
       const double h0 = Ui00 * gf0 + Ui01 * gf1, h1 = Ui01 * gf0 + Ui11 * gf1;
       const double b0 = V[0][0] * f[0] + V[0][1] * f[1] + V[0][2] * f[2];
       const double b1 = V[1][0] * f[0] + V[1][1] * f[1] + V[1][2] * f[2];
@@ -210,7 +211,7 @@ __global__ void __launch_bounds__(128) preprocess_backward_kernel(gabsplat_scene
   for (int m = 0; m < 3; ++m) g.d_means[3 * i + m] = (float)gmu[m];
   g.d_opacities[i] = g2[5];
   if (g.d_mean2d) { g.d_mean2d[2 * i] = g2[0]; g.d_mean2d[2 * i + 1] = g2[1]; }
-  if (g.d_mean2d_abs) { g.d_mean2d_abs[2 * i] = g2[9]; g.d_mean2d_abs[2 * i + 1] = g2[10]; }
+  if (g.d_mean2d_abs) { g.d_mean2d_abs[2 * i] = g2[9 + 3 * K]; g.d_mean2d_abs[2 * i + 1] = g2[10 + 3 * K]; }
 }
 
 }  // namespace

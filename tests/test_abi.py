@@ -39,7 +39,7 @@ def test_size_queries(lib):
     lib.gabsplat_sort_workspace_bytes.restype = C.c_uint64
     lib.gabsplat_sort_workspace_bytes.argtypes = [C.c_int32, C.c_uint64]
     lib.gabsplat_grad_workspace_bytes.restype = C.c_uint64
-    assert [lib.gabsplat_packed_floats(k) for k in (0, 1, 2, 4, 8)] == [12, 20, 20, 24, 36]
+    assert [lib.gabsplat_packed_floats(k) for k in (0, 1, 2, 4, 8)] == [12, 16, 20, 24, 36]
     assert lib.gabsplat_packed_floats(9) == 0 and lib.gabsplat_packed_floats(-1) == 0
     a = lib.gabsplat_sort_workspace_bytes(1000, 10_000)
     b = lib.gabsplat_sort_workspace_bytes(1000, 20_000)
