@@ -190,8 +190,13 @@ def stage_work(K, N, stats, tiles, passes) -> dict:
     w = {}
     w["preprocess"] = ("hbm", N * 16 + n_vis * (par - 12 + 49 + 8 * K - 4))
     w["scan"] = ("hbm", 8 * N)
-    w["duplicate"] = ("hbm", 4 * N + 20 * n_vis + 12 * D)
-    w["sort"] = ("hbm", D * (8 + passes * 24))
+    # S2 as built: the LSD sort of the 64-bit keys is split into the 4 depth digits, sorted on
+    # the N primitives (read 4 B for the histogram, then 8 B in + 8 B out per pass), and the tile digits, sorted
+    # on the D instances (4 B histogram read; 8 B in + 8 B out per pass, the last pass 8 B in + 4 B depth gather
+    # + 12 B out); the duplication writes 8 B per instance
+    w["depth_sort"] = ("hbm", N * (4 + 4 * 16))
+    w["duplicate"] = ("hbm", 8 * N + 20 * n_vis + 8 * D)
+    w["sort"] = ("hbm", D * (4 + (passes - 1) * 16 + 24))
     w["ranges"] = ("hbm", 8 * D + 8 * tiles)
     w["preprocess_backward"] = ("hbm", n_vis * (par + (9 + 3 * K) * 4) + N * par)
     # blend: FP32-pipe lane-instructions and MUFU lane-ops
@@ -240,7 +245,7 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     V = len(cams)
     H, W = cams[0].height, cams[0].width
     tiles = cams[0].tiles_x * cams[0].tiles_y
-    passes = (32 + max(1, (tiles - 1).bit_length()) + 7) // 8
+    passes = (max(1, (tiles - 1).bit_length()) + 7) // 8     # one-byte passes on the tile id
 
     ds = gb.upload_scene(scene, dev)
     dLs = [torch.from_numpy(scenes.make_image_grad(name, v, cams[v])).to(dev) for v in range(V)] if backward else None
@@ -323,8 +328,8 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     work = stage_work(K, N, mean_stats, tiles, passes)
     per_stage = {}
     for s, lst in stage_ms.items():
-        m = float(np.mean(lst))
-        per_stage[s] = {"ms": m, "share": m * len(lst) / args.steps / ms_per_step, **roofline_entry(work[s], m, hbm_peak, peak_kind)}
+        m = float(np.sum(lst)) / args.steps          # per step (a stage may launch in several pieces)
+        per_stage[s] = {"ms": m, "share": m / ms_per_step, **roofline_entry(work[s], m, hbm_peak, peak_kind)}
     dominant = max(per_stage, key=lambda s: per_stage[s]["ms"])
     roofline = {"kernel": dominant, **{k: per_stage[dominant][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
                 "peak_kind": per_stage[dominant]["peak_kind"]}

@@ -100,7 +100,7 @@ int32_t gabsplat_packed_floats(int32_t K);
 
 /* Tile binning state.  capacity = number of (key,id) slots the caller allocated. */
 typedef struct {
-  uint32_t* offsets;          /* [N]  inclusive prefix sum of tiles_touched                          */
+  uint32_t* offsets;          /* [N]  inclusive prefix sum of tiles_touched taken in depth order     */
   uint64_t* keys;             /* [capacity]  sorted on return: (tile_id << 32) | bits(depth)         */
   uint32_t* ids;              /* [capacity]  primitive index of each instance, same order            */
   uint32_t* tile_ranges;      /* [tiles_y*tiles_x][2]  [start,end) into keys/ids; (0,0) if empty     */
@@ -140,8 +140,10 @@ uint64_t gabsplat_grad_workspace_bytes(int32_t N, int32_t K);
 int32_t gabsplat_preprocess(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
                             gabsplat_projected* out, void* stream);
 
-/* S2.  Emits one (key,id) per (primitive, tile of its rectangle) in primitive-major, row-major order,
- * sorts them stably by key with an LSD radix sort on one-byte digits, and extracts tile ranges.
+/* S2.  Builds the list of (key,id) instances, one per (primitive, tile of its rectangle), ordered by key with
+ * ties by primitive index -- the result of a stable LSD radix sort on one-byte digits of the keys emitted in
+ * primitive-major order (the depth digits are sorted on the primitives before duplication, the tile digits on
+ * the instances after it) -- and extracts tile ranges.
  * If D > capacity nothing is emitted, *num_instances still holds D, and (when num_instances_host is
  * given) GABSPLAT_CAPACITY is returned.  num_instances_host != NULL makes the call synchronise the
  * stream once to read D back; with NULL the call is fully asynchronous and the caller must have sized
@@ -181,12 +183,13 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* scene_host
 #define GABSPLAT_STAGE_PREPROCESS 0      /* S1  projection kernel                                   */
 #define GABSPLAT_STAGE_SCAN 1            /* S2a prefix sum of tiles_touched                          */
 #define GABSPLAT_STAGE_DUPLICATE 2       /* S2b key emission                                        */
-#define GABSPLAT_STAGE_SORT 3            /* S2c all radix passes                                    */
+#define GABSPLAT_STAGE_SORT 3            /* S2c radix passes on the tile digits (over the instances) */
 #define GABSPLAT_STAGE_RANGES 4          /* S2d tile ranges (incl. clearing them)                   */
 #define GABSPLAT_STAGE_BLEND_FORWARD 5   /* S3                                                      */
 #define GABSPLAT_STAGE_BLEND_BACKWARD 6  /* S4a (incl. zeroing the 2D gradient records)             */
 #define GABSPLAT_STAGE_PREPROCESS_BACKWARD 7 /* S4b (incl. zeroing the gradient outputs)             */
-#define GABSPLAT_STAGE_COUNT 8
+#define GABSPLAT_STAGE_DEPTH_SORT 8      /* S2c radix passes on the depth digits (over the primitives) */
+#define GABSPLAT_STAGE_COUNT 9
 int32_t gabsplat_timing_enable(gabsplat_ctx* ctx, int32_t on);
 int32_t gabsplat_timing_read(gabsplat_ctx* ctx, int32_t* stage_ids_host, float* ms_host, int32_t max_records,
                              int32_t* n_records_host);

@@ -353,7 +353,9 @@ def gabsplat_render_host(ctx: Context, scene, cam, capacity: int, image_host: to
 
 
 STAGES = ("preprocess", "scan", "duplicate", "sort", "ranges", "blend_forward", "blend_backward",
-          "preprocess_backward")
+          "preprocess_backward", "depth_sort")          # indexed by GABSPLAT_STAGE_*
+LAUNCH_ORDER = ("preprocess", "depth_sort", "scan", "duplicate", "sort", "ranges", "blend_forward", "blend_backward",
+                "preprocess_backward")
 
 
 def gabsplat_kernel_launches() -> int:

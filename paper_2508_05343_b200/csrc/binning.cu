@@ -1,10 +1,17 @@
 // S2 / K2-K5: tile binning.  (PAPER.md:103 "sorted by depth", :160 "tile-based rasterizer".)
-//   K2  inclusive prefix sum of tiles_touched                       -> offsets, D
-//   K3  one (key,id) per (primitive, tile of its rectangle), primitive-major, row-major over the rectangle,
-//       key = (tile << 32) | bits(depth)
-//   K4  stable LSD radix sort of the pairs on one-byte digits (in-house; no library sort)
+// The result is the list of (primitive, tile) instances ordered by the 64-bit key (tile << 32) | bits(depth),
+// ties by primitive index -- exactly what a stable LSD radix sort of the keys on one-byte digits gives -- plus
+// the [start,end) range of every tile.  The LSD passes are split around the duplication step so that the four
+// depth digits are sorted on the N primitives, not on the D >> N instances:
+//   A   keys = bits(depth) (culled primitives: 0xffffffff), 4 stable one-byte passes over the N primitives
+//       -> `order`: primitives front to back, ties by index
+//   K2  inclusive prefix sum of tiles_touched taken in that order               -> offsets, D
+//   K3  one (tile,id) per (primitive, tile of its rectangle), emitted in depth order, row-major over the rectangle
+//   B   ceil(tile_bits / 8) stable one-byte passes on the tile id over the D instances; the last pass writes the
+//       64-bit key (tile | depth gathered by id) and the id
 //   K5  [start,end) of every tile in the sorted list
-// Everything is integer work; the result must equal std::stable_sort of the keys bit for bit.
+// LSD order is preserved: digits 0-3 (depth) before digits 4.. (tile), every pass stable.  Everything is
+// integer work; the result must equal std::stable_sort of the 64-bit keys bit for bit.
 // The instance count D lives on the device: every kernel is launched on a grid sized from the caller's
 // capacity and returns early past D, so the whole stage runs without a host round trip.
 #include "common.cuh"
@@ -17,6 +24,7 @@ typedef uint64_t u64;
 
 // ------------------------------------------------------------------------------------------------
 // Device-wide prefix sum of u32 (three launches: block sums, scan of the sums, block scans).
+// GATHER: element i of the input is in[idx[i]].
 // ------------------------------------------------------------------------------------------------
 constexpr int kScanThreads = 256;
 constexpr int kScanItems = 16;
@@ -53,16 +61,35 @@ __device__ __forceinline__ u32 block_exclusive_scan(u32 v, u32* total) {
   return r;
 }
 
-__global__ void __launch_bounds__(kScanThreads) scan_block_sums(const u32* __restrict__ in, u32 n, u32* __restrict__ sums) {
-  const u32 base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
-  u32 s = 0;
+template <bool GATHER>
+__device__ __forceinline__ void scan_load(const u32* __restrict__ in, const u32* __restrict__ idx, u32 base, u32 n,
+                                          u32 (&v)[kScanItems]) {
   if (base + kScanItems <= n) {
-    const uint4* p = reinterpret_cast<const uint4*>(in + base);
+    const uint4* p = reinterpret_cast<const uint4*>((GATHER ? idx : in) + base);
 #pragma unroll
-    for (int j = 0; j < kScanItems / 4; ++j) { const uint4 v = p[j]; s += v.x + v.y + v.z + v.w; }
+    for (int j = 0; j < kScanItems / 4; ++j) {
+      const uint4 x = p[j];
+      v[4 * j] = x.x; v[4 * j + 1] = x.y; v[4 * j + 2] = x.z; v[4 * j + 3] = x.w;
+    }
+    if (GATHER) {
+#pragma unroll
+      for (int j = 0; j < kScanItems; ++j) v[j] = __ldg(in + v[j]);
+    }
   } else {
-    for (int j = 0; j < kScanItems; ++j) if (base + j < n) s += in[base + j];
+#pragma unroll
+    for (int j = 0; j < kScanItems; ++j) v[j] = base + j < n ? (GATHER ? __ldg(in + idx[base + j]) : in[base + j]) : 0;
   }
+}
+
+template <bool GATHER>
+__global__ void __launch_bounds__(kScanThreads) scan_block_sums(const u32* __restrict__ in, const u32* __restrict__ idx, u32 n,
+                                                                 u32* __restrict__ sums) {
+  const u32 base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+  u32 v[kScanItems];
+  scan_load<GATHER>(in, idx, base, n, v);
+  u32 s = 0;
+#pragma unroll
+  for (int j = 0; j < kScanItems; ++j) s += v[j];
   u32 total;
   block_exclusive_scan(s, &total);
   if (threadIdx.x == 0) sums[blockIdx.x] = total;
@@ -82,23 +109,12 @@ __global__ void __launch_bounds__(kScanThreads) scan_of_sums(u32* __restrict__ s
   if (threadIdx.x == 0 && total_out) *total_out = carry;
 }
 
-template <bool INCLUSIVE>
-__global__ void __launch_bounds__(kScanThreads) scan_apply(const u32* __restrict__ in, u32 n, const u32* __restrict__ sums,
-                                                            u32* __restrict__ out) {
+template <bool INCLUSIVE, bool GATHER>
+__global__ void __launch_bounds__(kScanThreads) scan_apply(const u32* __restrict__ in, const u32* __restrict__ idx, u32 n,
+                                                            const u32* __restrict__ sums, u32* __restrict__ out) {
   const u32 base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
   u32 v[kScanItems];
-  const bool full = base + kScanItems <= n;
-  if (full) {
-    const uint4* p = reinterpret_cast<const uint4*>(in + base);
-#pragma unroll
-    for (int j = 0; j < kScanItems / 4; ++j) {
-      const uint4 x = p[j];
-      v[4 * j] = x.x; v[4 * j + 1] = x.y; v[4 * j + 2] = x.z; v[4 * j + 3] = x.w;
-    }
-  } else {
-#pragma unroll
-    for (int j = 0; j < kScanItems; ++j) v[j] = base + j < n ? in[base + j] : 0;
-  }
+  scan_load<GATHER>(in, idx, base, n, v);
   u32 s = 0;
 #pragma unroll
   for (int j = 0; j < kScanItems; ++j) s += v[j];
@@ -110,7 +126,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply(const u32* __restrict
     run += v[j];
     v[j] = INCLUSIVE ? run : e;
   }
-  if (full) {
+  if (base + kScanItems <= n) {
     uint4* q = reinterpret_cast<uint4*>(out + base);
 #pragma unroll
     for (int j = 0; j < kScanItems / 4; ++j) q[j] = make_uint4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
@@ -122,103 +138,166 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply(const u32* __restrict
 
 inline u32 scan_blocks(u32 n) { return (n + kScanTile - 1) / kScanTile; }
 
-// sums must hold scan_blocks(n) u32.  in/out must be 16-byte aligned.  in == out is allowed.
-template <bool INCLUSIVE>
-void device_scan(const u32* in, u32* out, u32 n, u32* sums, u32* total_out, cudaStream_t st) {
+// sums must hold scan_blocks(n) u32.  in/out/idx must be 16-byte aligned.  in == out is allowed (not with GATHER).
+template <bool INCLUSIVE, bool GATHER>
+void device_scan(const u32* in, const u32* idx, u32* out, u32 n, u32* sums, u32* total_out, cudaStream_t st) {
   const u32 nb = scan_blocks(n);
   if (nb == 0) {
     scan_of_sums<<<1, kScanThreads, 0, st>>>(sums, 0, total_out);
     launched();
     return;
   }
-  scan_block_sums<<<nb, kScanThreads, 0, st>>>(in, n, sums);
-  launched();
+  scan_block_sums<GATHER><<<nb, kScanThreads, 0, st>>>(in, idx, n, sums);
   scan_of_sums<<<1, kScanThreads, 0, st>>>(sums, nb, total_out);
-  launched();
-  scan_apply<INCLUSIVE><<<nb, kScanThreads, 0, st>>>(in, n, sums, out);
-  launched();
+  scan_apply<INCLUSIVE, GATHER><<<nb, kScanThreads, 0, st>>>(in, idx, n, sums, out);
+  launched(3);
 }
 
 // ------------------------------------------------------------------------------------------------
-// K3: duplicate.  One block per 256 primitives; the block's instances are emitted cooperatively so that
-// writes are coalesced and a primitive covering thousands of tiles is shared by the whole block.
+// A: depth keys of the primitives.  Culled primitives (tiles_touched == 0) sort to the end.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __restrict__ tiles_touched,
+                                                         const float* __restrict__ depth, u32* __restrict__ keys,
+                                                         u32* __restrict__ vals, u32* __restrict__ count) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) *count = (u32)N;
+  if (i >= N) return;
+  keys[i] = tiles_touched[i] ? __float_as_uint(depth[i]) : 0xffffffffu;
+  vals[i] = (u32)i;
+}
+
+// ------------------------------------------------------------------------------------------------
+// K3: duplicate, balanced by OUTPUT: one block per kDupChunk consecutive instances (in depth order the
+// front-most primitives cover thousands of tiles each and sit next to each other, so a block per 256
+// primitives would serialise them).  The block finds the first primitive rank of its chunk with a cooperative
+// 256-ary search over `offsets`, stages the chunk's slice of `offsets` / `order` in shared memory, and every
+// instance locates its primitive by a binary search there.  Emits the tile id (sort key of stage B) and the
+// primitive id; instances of a primitive are row-major over its rectangle.
 // ------------------------------------------------------------------------------------------------
 constexpr int kDupThreads = 256;
+constexpr int kDupChunk = 2048;
 
-__global__ void __launch_bounds__(kDupThreads) duplicate_kernel(int N, int tiles_x, const u32* __restrict__ offsets,
-                                                               const u32* __restrict__ tiles_touched,
-                                                               const int4* __restrict__ rect, const float* __restrict__ depth,
+__global__ void __launch_bounds__(kDupThreads) duplicate_kernel(int N, int tiles_x, const u32* __restrict__ order,
+                                                               const u32* __restrict__ offsets,
+                                                               const int4* __restrict__ rect,
                                                                const u32* __restrict__ num_instances, u64 capacity,
-                                                               u64* __restrict__ keys, u32* __restrict__ ids) {
-  __shared__ u32 s_incl[kDupThreads];
-  __shared__ int4 s_rect[kDupThreads];
-  __shared__ u32 s_depth[kDupThreads];
-  if ((u64)*num_instances > capacity) return;
-  const int i0 = blockIdx.x * kDupThreads;
-  const int i = i0 + threadIdx.x;
-  u32 incl = 0, tt = 0;
-  if (i < N) { incl = offsets[i]; tt = tiles_touched[i]; }
-  else if (N > 0) incl = offsets[N - 1];
-  s_incl[threadIdx.x] = incl;
-  if (tt) { s_rect[threadIdx.x] = rect[i]; s_depth[threadIdx.x] = __float_as_uint(depth[i]); }
-  __shared__ u32 s_base;
-  if (threadIdx.x == 0) s_base = incl - tt;
+                                                               u32* __restrict__ tiles_out, u32* __restrict__ ids_out) {
+  __shared__ u32 s_incl[kDupChunk];
+  __shared__ u32 s_id[kDupChunk];
+  __shared__ u32 s_lo, s_hi, s_cnt[kDupThreads / 32];
+  const u32 D = *num_instances;
+  if ((u64)D > capacity) return;
+  const u32 g0 = blockIdx.x * kDupChunk;
+  if (g0 >= D) return;
+  const u32 n = min((u32)kDupChunk, D - g0);
+  // r_lo = first rank r with offsets[r] > g0 (upper bound).  Invariant lo <= r_lo <= hi; every step probes 256
+  // evenly spaced ranks: the predicate offsets[p] <= g0 holds exactly for p < r_lo, so the true probes are a prefix
+  if (threadIdx.x == 0) { s_lo = 0; s_hi = (u32)N; }
   __syncthreads();
-  const u32 base = s_base;
-  const u32 count = s_incl[kDupThreads - 1] - base;
-  for (u32 e = threadIdx.x; e < count; e += kDupThreads) {
-    const u32 g = base + e;
-    // first p with s_incl[p] > g
-    int lo = 0, hi = kDupThreads - 1;
+  while (true) {
+    const u32 lo = s_lo, hi = s_hi;
+    if (lo >= hi) break;
+    const u32 step = (hi - lo + kDupThreads - 1) / kDupThreads;
+    const u32 p = lo + threadIdx.x * step;
+    const bool le = p < hi && __ldg(offsets + p) <= g0;
+    const u32 bal = __ballot_sync(0xffffffffu, le);
+    if ((threadIdx.x & 31) == 0) s_cnt[threadIdx.x >> 5] = __popc(bal);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      u32 c = 0;
+#pragma unroll
+      for (int w = 0; w < kDupThreads / 32; ++w) c += s_cnt[w];
+      if (c == 0) {
+        s_hi = lo;  // offsets[lo] > g0
+      } else {
+        s_lo = lo + (c - 1) * step + 1;   // probe c-1 holds
+        s_hi = min(hi, lo + c * step);    // probe c (if any) does not
+      }
+    }
+    __syncthreads();
+  }
+  const u32 r_lo = s_lo;
+  const u32 prev0 = r_lo ? __ldg(offsets + r_lo - 1) : 0u;  // instances before rank r_lo
+  // at most n ranks start inside the chunk (every rank after the first that owns an instance here)
+  for (u32 j = threadIdx.x; j < n; j += kDupThreads) {
+    const u32 r = r_lo + j;
+    s_incl[j] = r < (u32)N ? __ldg(offsets + r) : 0xffffffffu;
+    s_id[j] = r < (u32)N ? __ldg(order + r) : 0u;
+  }
+  __syncthreads();
+  for (u32 e = threadIdx.x; e < n; e += kDupThreads) {
+    const u32 g = g0 + e;
+    // first j with s_incl[j] > g
+    u32 lo = 0, hi = n - 1;
     while (lo < hi) {
-      const int mid = (lo + hi) >> 1;
+      const u32 mid = (lo + hi) >> 1;
       if (s_incl[mid] > g) hi = mid; else lo = mid + 1;
     }
-    const int4 r = s_rect[lo];
-    const u32 first = lo ? s_incl[lo - 1] : base;
+    const u32 id = s_id[lo];
+    const int4 rc = __ldg(rect + id);
+    const u32 first = lo ? s_incl[lo - 1] : prev0;
     const u32 local = g - first;
-    const u32 w = (u32)(r.z - r.x);
+    const u32 w = (u32)(rc.z - rc.x);
     const u32 row = local / w, col = local - row * w;
-    const u32 tile = (u32)(r.y + row) * (u32)tiles_x + (u32)r.x + col;
-    keys[g] = ((u64)tile << 32) | (u64)s_depth[lo];
-    ids[g] = (u32)(i0 + lo);
+    tiles_out[g] = (u32)(rc.y + row) * (u32)tiles_x + (u32)rc.x + col;
+    ids_out[g] = id;
   }
 }
 
 // ------------------------------------------------------------------------------------------------
-// K4: one LSD radix pass on the one-byte digit (key >> shift) & 255: per-block digit histogram,
-// scan of the [digit][block] table, stable scatter.
+// One LSD radix pass on the one-byte digit (key >> shift) & 255 of (u32 key, u32 value) pairs: per-block digit
+// histogram, scan of the [digit][block] table, stable scatter.  FINAL (last pass of stage B): the output is
+// the 64-bit key (key << 32) | gather[value] and the value.
 // ------------------------------------------------------------------------------------------------
 constexpr int kSortThreads = 256;
-constexpr int kSortItems = 8;
-constexpr int kSortTile = kSortThreads * kSortItems;  // 2048 pairs per block
+constexpr int kSortItems = 16;
+constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 pairs per block
 constexpr int kSortWarps = kSortThreads / 32;
 
-__global__ void __launch_bounds__(kSortThreads) sort_histogram(const u64* __restrict__ keys, const u32* __restrict__ num_instances,
+__global__ void __launch_bounds__(kSortThreads) sort_histogram(const u32* __restrict__ keys, const u32* __restrict__ count,
                                                               u32* __restrict__ table, u32 nblocks, int shift) {
-  __shared__ u32 hist[256];
-  hist[threadIdx.x] = 0;
+  __shared__ u32 hist[kSortWarps][256];
+#pragma unroll
+  for (int j = 0; j < kSortWarps; ++j) hist[j][threadIdx.x] = 0;
   __syncthreads();
-  const u32 D = *num_instances;
+  const u32 D = *count;
   const u32 start = blockIdx.x * kSortTile;
+  const int w = threadIdx.x >> 5;
   if (start < D) {
     const u32 n = min((u32)kSortTile, D - start);
-    for (u32 j = threadIdx.x; j < n; j += kSortThreads) atomicAdd(&hist[(u32)(keys[start + j] >> shift) & 255u], 1u);
+    if (n == kSortTile) {
+      const uint4* p = reinterpret_cast<const uint4*>(keys + start);
+#pragma unroll
+      for (int j = 0; j < kSortItems / 4; ++j) {
+        const uint4 k = p[j * kSortThreads + threadIdx.x];
+        atomicAdd(&hist[w][(k.x >> shift) & 255u], 1u);
+        atomicAdd(&hist[w][(k.y >> shift) & 255u], 1u);
+        atomicAdd(&hist[w][(k.z >> shift) & 255u], 1u);
+        atomicAdd(&hist[w][(k.w >> shift) & 255u], 1u);
+      }
+    } else {
+      for (u32 j = threadIdx.x; j < n; j += kSortThreads) atomicAdd(&hist[w][(keys[start + j] >> shift) & 255u], 1u);
+    }
   }
   __syncthreads();
-  table[threadIdx.x * nblocks + blockIdx.x] = hist[threadIdx.x];
+  u32 tot = 0;
+#pragma unroll
+  for (int j = 0; j < kSortWarps; ++j) tot += hist[j][threadIdx.x];
+  table[threadIdx.x * nblocks + blockIdx.x] = tot;
 }
 
-__global__ void __launch_bounds__(kSortThreads) sort_scatter(const u64* __restrict__ kin, const u32* __restrict__ vin,
-                                                            u64* __restrict__ kout, u32* __restrict__ vout,
-                                                            const u32* __restrict__ num_instances,
-                                                            const u32* __restrict__ table, u32 nblocks, int shift) {
+template <bool FINAL>
+__global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restrict__ kin, const u32* __restrict__ vin,
+                                                            u32* __restrict__ kout, u32* __restrict__ vout,
+                                                            u64* __restrict__ kout64, const u32* __restrict__ gather,
+                                                            const u32* __restrict__ count, const u32* __restrict__ table,
+                                                            u32 nblocks, int shift) {
   __shared__ u32 warp_hist[kSortWarps][256];
   __shared__ u32 local_base[256];
   __shared__ u32 global_base[256];
-  __shared__ u64 skeys[kSortTile];
+  __shared__ u32 skeys[kSortTile];
   __shared__ u32 svals[kSortTile];
-  const u32 D = *num_instances;
+  const u32 D = *count;
   const u32 start = blockIdx.x * kSortTile;
   if (start >= D) return;
   const u32 n = min((u32)kSortTile, D - start);
@@ -227,30 +306,31 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u64* __restri
   for (int j = 0; j < kSortWarps; ++j) warp_hist[j][threadIdx.x] = 0;
   __syncthreads();
 
-  u64 k[kSortItems];
-  u32 v[kSortItems], rank[kSortItems];
+  // warp w owns the contiguous run [w * 32 * kSortItems, (w+1) * 32 * kSortItems) of the block's tile, visited
+  // 32 consecutive pairs at a time: rank order = input order (stability)
+  u32 k[kSortItems], v[kSortItems], rank[kSortItems];
   const u32 lt_mask = (1u << lane) - 1u;
 #pragma unroll
   for (int r = 0; r < kSortItems; ++r) {
     const u32 idx = (u32)w * 32u * kSortItems + (u32)r * 32u + (u32)lane;
     const bool valid = idx < n;
-    k[r] = valid ? kin[start + idx] : 0;
+    k[r] = valid ? kin[start + idx] : 0xffffffffu;
     v[r] = valid ? vin[start + idx] : 0;
-    const u32 d = (u32)(k[r] >> shift) & 255u;
-    // lanes holding the same digit (valid lanes only)
-    u32 peers = __ballot_sync(0xffffffffu, valid);
+  }
 #pragma unroll
-    for (int b = 0; b < 8; ++b) {
-      const u32 bal = __ballot_sync(0xffffffffu, (d >> b) & 1u);
-      peers &= ((d >> b) & 1u) ? bal : ~bal;
-    }
+  for (int r = 0; r < kSortItems; ++r) {
+    const u32 idx = (u32)w * 32u * kSortItems + (u32)r * 32u + (u32)lane;
+    const bool valid = idx < n;
+    const u32 d = (k[r] >> shift) & 255u;
+    // lanes holding the same digit; invalid lanes get a digit value no valid lane can have
+    const u32 peers = __match_any_sync(0xffffffffu, valid ? d : 256u);
     u32 prev = 0;
     const int leader = __ffs(peers) - 1;
     if (valid && lane == leader) {
       prev = warp_hist[w][d];
       warp_hist[w][d] = prev + __popc(peers);
     }
-    prev = __shfl_sync(0xffffffffu, prev, valid ? leader : lane);
+    prev = __shfl_sync(0xffffffffu, prev, leader);
     rank[r] = prev + __popc(peers & lt_mask);
     __syncwarp();
   }
@@ -275,7 +355,7 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u64* __restri
   for (int r = 0; r < kSortItems; ++r) {
     const u32 idx = (u32)w * 32u * kSortItems + (u32)r * 32u + (u32)lane;
     if (idx < n) {
-      const u32 d = (u32)(k[r] >> shift) & 255u;
+      const u32 d = (k[r] >> shift) & 255u;
       const u32 pos = local_base[d] + warp_hist[w][d] + rank[r];
       skeys[pos] = k[r];
       svals[pos] = v[r];
@@ -283,11 +363,13 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u64* __restri
   }
   __syncthreads();
   for (u32 j = threadIdx.x; j < n; j += kSortThreads) {
-    const u64 key = skeys[j];
-    const u32 d = (u32)(key >> shift) & 255u;
+    const u32 key = skeys[j];
+    const u32 val = svals[j];
+    const u32 d = (key >> shift) & 255u;
     const u32 dst = global_base[d] + (j - local_base[d]);
-    kout[dst] = key;
-    vout[dst] = svals[j];
+    if (FINAL) kout64[dst] = ((u64)key << 32) | (u64)__ldg(gather + val);
+    else kout[dst] = key;
+    vout[dst] = val;
   }
 }
 
@@ -311,30 +393,49 @@ __global__ void clamp_count_kernel(u32* sort_count, const u32* num_instances, u6
 }
 
 inline u64 align_up(u64 x, u64 a) { return (x + a - 1) / a * a; }
+inline u32 sort_blocks(u64 n) { return (u32)((n + kSortTile - 1) / kSortTile); }
 
 struct Workspace {
   u32* scan_sums;   // scan partials (reused by every scan)
-  u32* sort_count;  // [1]
+  u32* count_a;     // [1] = N
+  u32* count_b;     // [1] = D, or 0 when D > capacity
   u32* table;       // [256][nblocks]
-  u64* keys_alt;
-  u32* ids_alt;
+  u32* pk[2];       // stage A key ping-pong [N]
+  u32* pv[2];       // stage A value ping-pong [N]; pv[0] ends up holding the depth order
+  u32* ik;          // stage B alternate keys [capacity]
+  u32* iv;          // stage B alternate values [capacity]
   u64 bytes;
 };
 
 Workspace carve(void* base, int N, u64 capacity) {
-  const u32 nblocks = (u32)((capacity + kSortTile - 1) / kSortTile);
-  const u64 table_n = (u64)256 * (nblocks ? nblocks : 1);
+  const u64 nb = (u64)(sort_blocks(capacity) > sort_blocks((u64)N) ? sort_blocks(capacity) : sort_blocks((u64)N));
+  const u64 table_n = (u64)256 * (nb ? nb : 1);
   const u64 sums_n = (u64)scan_blocks((u32)(table_n > (u64)N ? table_n : (u64)N)) + 16;
   u64 off = 0;
   Workspace w;
   char* b = (char*)base;
-  w.scan_sums = (u32*)(b + off); off = align_up(off + sums_n * 4, 256);
-  w.sort_count = (u32*)(b + off); off = align_up(off + 16, 256);
-  w.table = (u32*)(b + off); off = align_up(off + table_n * 4, 256);
-  w.keys_alt = (u64*)(b + off); off = align_up(off + capacity * 8, 256);
-  w.ids_alt = (u32*)(b + off); off = align_up(off + capacity * 4, 256);
+  auto take = [&](u64 bytes) { char* p = b + off; off = align_up(off + bytes, 256); return p; };
+  w.scan_sums = (u32*)take(sums_n * 4);
+  w.count_a = (u32*)take(16);
+  w.count_b = (u32*)take(16);
+  w.table = (u32*)take(table_n * 4);
+  for (int i = 0; i < 2; ++i) { w.pk[i] = (u32*)take((u64)N * 4); w.pv[i] = (u32*)take((u64)N * 4); }
+  w.ik = (u32*)take(capacity * 4);
+  w.iv = (u32*)take(capacity * 4);
   w.bytes = off;
   return w;
+}
+
+void radix_pass(const u32* kin, const u32* vin, u32* kout, u32* vout, u64* kout64, const u32* gather, const u32* count,
+                u32 nblocks, int shift, const Workspace& ws, cudaStream_t st) {
+  sort_histogram<<<nblocks, kSortThreads, 0, st>>>(kin, count, ws.table, nblocks, shift);
+  launched();
+  device_scan<false, false>(ws.table, nullptr, ws.table, 256u * nblocks, ws.scan_sums, nullptr, st);
+  if (kout64)
+    sort_scatter<true><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift);
+  else
+    sort_scatter<false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift);
+  launched();
 }
 
 }  // namespace
@@ -345,41 +446,53 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
                             StageTimer& tm, cudaStream_t st) {
   const Workspace ws = carve(bin.workspace, N, bin.capacity);
   const int ntiles = cam.tiles_x * cam.tiles_y;
-  // K2
-  tm.begin(GABSPLAT_STAGE_SCAN, st);
-  device_scan<true>(proj.tiles_touched, bin.offsets, (u32)N, ws.scan_sums, bin.num_instances, st);
-  tm.end(st);
-  if (N == 0 || bin.capacity == 0) {
+  if (N == 0) {
+    cudaMemsetAsync(bin.num_instances, 0, sizeof(u32), st);
     cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
     return cudaGetLastError();
   }
-  clamp_count_kernel<<<1, 1, 0, st>>>(ws.sort_count, bin.num_instances, bin.capacity);
+  // A: depth order of the primitives (digits 0-3 of the 64-bit key)
+  tm.begin(GABSPLAT_STAGE_DEPTH_SORT, st);
+  depth_keys_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, proj.tiles_touched, proj.depth, ws.pk[0], ws.pv[0], ws.count_a);
   launched();
-  // number of one-byte passes: 32 depth bits + bits of the largest tile id
+  const u32 nba = sort_blocks((u64)N);
+  for (int p = 0; p < 4; ++p)
+    radix_pass(ws.pk[p & 1], ws.pv[p & 1], ws.pk[(p & 1) ^ 1], ws.pv[(p & 1) ^ 1], nullptr, nullptr, ws.count_a, nba, 8 * p,
+               ws, st);
+  const u32* order = ws.pv[0];
+  tm.end(st);
+  // K2
+  tm.begin(GABSPLAT_STAGE_SCAN, st);
+  device_scan<true, true>(proj.tiles_touched, order, bin.offsets, (u32)N, ws.scan_sums, bin.num_instances, st);
+  tm.end(st);
+  if (bin.capacity == 0) {
+    cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
+    return cudaGetLastError();
+  }
+  clamp_count_kernel<<<1, 1, 0, st>>>(ws.count_b, bin.num_instances, bin.capacity);
+  launched();
+  // stage B passes: one per byte of the tile id.  The last pass reads the alternate buffers and writes
+  // bin.keys / bin.ids; earlier passes ping-pong between (bin.keys viewed as u32, bin.ids) and the alternates.
   int tile_bits = 0;
   while ((1 << tile_bits) < ntiles) ++tile_bits;
-  const int passes = (32 + tile_bits + 7) / 8;
-  u64* kbuf[2] = {bin.keys, ws.keys_alt};
-  u32* vbuf[2] = {bin.ids, ws.ids_alt};
-  int cur = passes & 1;  // an odd number of passes starts in the alternate buffer so the result lands in bin.keys
+  const int passes = tile_bits <= 8 ? 1 : (tile_bits + 7) / 8;
+  u32* kbuf[2] = {reinterpret_cast<u32*>(bin.keys), ws.ik};  // [1] = alternates
+  u32* vbuf[2] = {bin.ids, ws.iv};
+  int cur = (passes & 1) ? 1 : 0;  // input of pass 0, chosen so that the last pass reads the alternates
   // K3
   tm.begin(GABSPLAT_STAGE_DUPLICATE, st);
-  duplicate_kernel<<<(N + kDupThreads - 1) / kDupThreads, kDupThreads, 0, st>>>(
-      N, cam.tiles_x, bin.offsets, proj.tiles_touched, reinterpret_cast<const int4*>(proj.rect), proj.depth,
-      bin.num_instances, bin.capacity, kbuf[cur], vbuf[cur]);
+  duplicate_kernel<<<(u32)((bin.capacity + kDupChunk - 1) / kDupChunk), kDupThreads, 0, st>>>(
+      N, cam.tiles_x, order, bin.offsets, reinterpret_cast<const int4*>(proj.rect), bin.num_instances, bin.capacity,
+      kbuf[cur], vbuf[cur]);
   launched();
   tm.end(st);
-  // K4
+  // B
   tm.begin(GABSPLAT_STAGE_SORT, st);
-  const u32 nblocks = (u32)((bin.capacity + kSortTile - 1) / kSortTile);
+  const u32 nbb = sort_blocks(bin.capacity);
   for (int p = 0; p < passes; ++p) {
-    const int shift = 8 * p;
-    sort_histogram<<<nblocks, kSortThreads, 0, st>>>(kbuf[cur], ws.sort_count, ws.table, nblocks, shift);
-    launched();
-    device_scan<false>(ws.table, ws.table, 256u * nblocks, ws.scan_sums, nullptr, st);
-    sort_scatter<<<nblocks, kSortThreads, 0, st>>>(kbuf[cur], vbuf[cur], kbuf[cur ^ 1], vbuf[cur ^ 1], ws.sort_count,
-                                                   ws.table, nblocks, shift);
-    launched();
+    const bool final_pass = p == passes - 1;
+    radix_pass(kbuf[cur], vbuf[cur], kbuf[cur ^ 1], vbuf[cur ^ 1], final_pass ? bin.keys : nullptr,
+               reinterpret_cast<const u32*>(proj.depth), ws.count_b, nbb, 8 * p, ws, st);
     cur ^= 1;
   }
   tm.end(st);

@@ -43,7 +43,7 @@ def test_size_queries(lib):
     assert lib.gabsplat_packed_floats(9) == 0 and lib.gabsplat_packed_floats(-1) == 0
     a = lib.gabsplat_sort_workspace_bytes(1000, 10_000)
     b = lib.gabsplat_sort_workspace_bytes(1000, 20_000)
-    assert b > a >= 10_000 * 12
+    assert b > a >= 10_000 * 8
     assert lib.gabsplat_grad_workspace_bytes(10, 4) >= 10 * 24 * 4
     assert lib.gabsplat_grad_workspace_bytes(10, 9) == 0
 

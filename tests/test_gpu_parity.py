@@ -205,9 +205,9 @@ def test_pair_counters_and_stage_timing():
     gb.gabsplat_render_backward(c, ds, cam, proj, bins, fwd, torch.from_numpy(dL).cuda())
     recs = gb.gabsplat_timing_read(c)
     gb.gabsplat_timing_enable(c, False)
-    assert [r[0] for r in recs] == list(gb.STAGES)
+    assert [r[0] for r in recs] == list(gb.LAUNCH_ORDER)
     assert all(ms > 0 for _, ms in recs)
-    assert gb.gabsplat_kernel_launches() - l0 >= len(gb.STAGES)
+    assert gb.gabsplat_kernel_launches() - l0 >= len(gb.LAUNCH_ORDER)
     assert gb.gabsplat_timing_read(c) == []
     cnt = gb.gabsplat_count_pairs(c, ds, cam, proj, bins).cpu().numpy().astype(np.int64)
     o = orc.render_forward(scene, cam)
