@@ -101,16 +101,11 @@ __device__ Index index_track(const Camera& c, float mx, float my, float mz, cons
   return o;
 }
 
-__global__ void __launch_bounds__(256) preprocess_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= s.N) return;
+// fp64 value track of one visible primitive; everything it stores is rounded once to fp32.
+__device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camera& c, const gabsplat_projected& out,
+                                            const int i, const Index& ix) {
   const int K = s.K;
   const float mx = s.means[3 * i], my = s.means[3 * i + 1], mz = s.means[3 * i + 2];
-  // depth test first: most culled primitives are behind the camera and need nothing but the mean
-  {
-    const float tz = ffma(c.w[8], mx, ffma(c.w[9], my, ffma(c.w[10], mz, c.w[11])));
-    if (!(tz > c.z_near)) { out.tiles_touched[i] = 0; out.radius[i] = 0; return; }
-  }
   float sc[3], q[4];
 #pragma unroll
   for (int a = 0; a < 3; ++a) sc[a] = s.scales[3 * i + a];
@@ -118,11 +113,6 @@ __global__ void __launch_bounds__(256) preprocess_kernel(gabsplat_scene s, Camer
     const float4 qv = reinterpret_cast<const float4*>(s.rotations)[i];
     q[0] = qv.x; q[1] = qv.y; q[2] = qv.z; q[3] = qv.w;
   }
-  const Index ix = index_track(c, mx, my, mz, sc, q);
-  out.tiles_touched[i] = ix.tiles;
-  out.radius[i] = ix.radius;
-  if (!ix.visible) return;
-
   // ---------------- value track (fp64) ----------------
   double Wm[3][3], tau[3];
 #pragma unroll
@@ -205,7 +195,9 @@ __global__ void __launch_bounds__(256) preprocess_kernel(gabsplat_scene s, Camer
     double acc[3] = {0.5, 0.5, 0.5};
     const float4* shp = reinterpret_cast<const float4*>(s.sh + (size_t)i * 48);
     // 4 coefficients (12 floats) per 3 float4 loads
-    for (int j4 = 0; j4 < nc; j4 += 4) {
+#pragma unroll
+    for (int j4 = 0; j4 < 16; j4 += 4) {
+      if (j4 >= nc) break;
       float buf[12];
 #pragma unroll
       for (int v4 = 0; v4 < 3; ++v4) {
@@ -246,13 +238,74 @@ __global__ void __launch_bounds__(256) preprocess_kernel(gabsplat_scene s, Camer
   }
 }
 
+// One CTA of kPreThreads threads per chunk of kPreChunk consecutive primitives, in two phases:
+//  1. every thread runs the fp32 indexing track of kPreChunk / kPreThreads primitives (coalesced loads; the
+//     depth test on the mean comes first, so a primitive behind the camera costs 12 bytes) and appends the
+//     visible ones to a list in shared memory;
+//  2. the threads walk the compacted list and run the fp64 value track.  In the paper-shaped scenes only
+//     10-20 % of the primitives are visible: without the compaction the value track runs with 3-6 live lanes
+//     per warp (ncu: 4.2-9.9 thread instructions per warp instruction, profiles/r01_*).
+constexpr int kPreThreads = 256;
+constexpr int kPreChunk = 1024;
+
+__global__ void __launch_bounds__(kPreThreads, 2) preprocess_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
+  __shared__ int s_i[kPreChunk];
+  __shared__ float s_m2x[kPreChunk], s_m2y[kPreChunk], s_depth[kPreChunk];
+  __shared__ uint32_t s_xy0[kPreChunk], s_xy1[kPreChunk];
+  __shared__ int s_n;
+  if (threadIdx.x == 0) s_n = 0;
+  __syncthreads();
+  const int base = blockIdx.x * kPreChunk;
+#pragma unroll 1
+  for (int r = 0; r < kPreChunk / kPreThreads; ++r) {
+    const int i = base + r * kPreThreads + threadIdx.x;
+    bool vis = false;
+    Index ix;
+    if (i < s.N) {
+      const float mx = s.means[3 * i], my = s.means[3 * i + 1], mz = s.means[3 * i + 2];
+      const float tz = ffma(c.w[8], mx, ffma(c.w[9], my, ffma(c.w[10], mz, c.w[11])));
+      uint32_t tiles = 0;
+      int radius = 0;
+      if (tz > c.z_near) {
+        float sc[3], q[4];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) sc[a] = s.scales[3 * i + a];
+        const float4 qv = reinterpret_cast<const float4*>(s.rotations)[i];
+        q[0] = qv.x; q[1] = qv.y; q[2] = qv.z; q[3] = qv.w;
+        ix = index_track(c, mx, my, mz, sc, q);
+        vis = ix.visible;
+        tiles = ix.tiles;
+        radius = ix.radius;
+      }
+      out.tiles_touched[i] = tiles;
+      out.radius[i] = radius;
+    }
+    if (vis) {
+      const int slot = atomicAdd(&s_n, 1);
+      s_i[slot] = i;
+      s_m2x[slot] = ix.m2x; s_m2y[slot] = ix.m2y; s_depth[slot] = ix.depth;
+      s_xy0[slot] = (uint32_t)ix.x0 | ((uint32_t)ix.y0 << 16);  // tile coordinates fit 16 bits (api.cu checks)
+      s_xy1[slot] = (uint32_t)ix.x1 | ((uint32_t)ix.y1 << 16);
+    }
+  }
+  __syncthreads();
+  const int n = s_n;
+  for (int j = threadIdx.x; j < n; j += kPreThreads) {
+    Index ix;
+    ix.visible = true;
+    ix.m2x = s_m2x[j]; ix.m2y = s_m2y[j]; ix.depth = s_depth[j];
+    ix.x0 = (int)(s_xy0[j] & 0xffffu); ix.y0 = (int)(s_xy0[j] >> 16);
+    ix.x1 = (int)(s_xy1[j] & 0xffffu); ix.y1 = (int)(s_xy1[j] >> 16);
+    value_track(s, c, out, s_i[j], ix);
+  }
+}
+
 }  // namespace
 
 cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& out,
                               cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
-  const int block = 256;
-  preprocess_kernel<<<(s.N + block - 1) / block, block, 0, st>>>(s, cam, out);
+  preprocess_kernel<<<(s.N + kPreChunk - 1) / kPreChunk, kPreThreads, 0, st>>>(s, cam, out);
   launched();
   return cudaGetLastError();
 }

@@ -2,20 +2,17 @@
 // equations -- PAPER.md:48, :129; derivation in DESIGN.md "Backward", per-primitive part):
 //   conic -> U;  f2D = U^-1 T Sigma f -> (U, T, Sigma, f);  U = T Sigma T^T -> (T, Sigma);  T = J W -> J -> t;
 //   mu2D -> t;  t -> mu;  Sigma = R S S^T R^T -> (scale, quaternion);  rgb -> (SH, mu through the view direction).
-// One thread per primitive; evaluated in fp64 (HBM-bound: the arithmetic is free, see preprocess.cu).
-// Gradient arrays are zeroed first, so culled primitives cost no thread work.
+// Evaluated in fp64 (HBM-bound: the arithmetic is free, see preprocess.cu).  The kernel zeroes the gradient
+// arrays itself (coalesced, per chunk), so culled primitives cost 300 bytes of stores and no arithmetic.
 #include "common.cuh"
 #include "sh.cuh"
 
 namespace gabsplat {
 namespace {
 
-__global__ void __launch_bounds__(128) preprocess_backward_kernel(gabsplat_scene s, Camera c, const uint32_t* __restrict__ tiles_touched,
-                                                                 const uint8_t* __restrict__ rgb_clamped,
-                                                                 const float* __restrict__ grad2d, gabsplat_grads g) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= s.N) return;
-  if (tiles_touched[i] == 0) return;
+// chain rule of one visible primitive (fp64); writes its row of every gradient array
+__device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Camera& c, const uint8_t* __restrict__ rgb_clamped,
+                                             const float* __restrict__ grad2d, const gabsplat_grads& g, const int i) {
   const int K = s.K;
   const int G = grad2d_floats(K);
   const float* g2 = grad2d + (size_t)i * G;
@@ -191,17 +188,34 @@ __global__ void __launch_bounds__(128) preprocess_backward_kernel(gabsplat_scene
     const uchar4 cl = reinterpret_cast<const uchar4*>(rgb_clamped)[i];
     const double gr[3] = {cl.x ? 0.0 : (double)g2[6], cl.y ? 0.0 : (double)g2[7], cl.z ? 0.0 : (double)g2[8]};
     double gd[3] = {0, 0, 0};
-    const float* shp = s.sh + (size_t)i * 48;
-    float* dsh = g.d_sh + (size_t)i * 48;
-    for (int j = 0; j < nc; ++j) {
-      double dot = 0.0;
+    const float4* shp = reinterpret_cast<const float4*>(s.sh + (size_t)i * 48);
+    float4* dsh = reinterpret_cast<float4*>(g.d_sh + (size_t)i * 48);
+    // 4 coefficients (12 floats) per 3 vector loads / stores; rows >= nc stay zero
 #pragma unroll
-      for (int ch = 0; ch < 3; ++ch) {
-        dsh[3 * j + ch] = (float)(Y[j] * gr[ch]);
-        dot += (double)shp[3 * j + ch] * gr[ch];
+    for (int j4 = 0; j4 < 16; j4 += 4) {
+      if (j4 >= nc) break;
+      float in[12], o[12];
+#pragma unroll
+      for (int v4 = 0; v4 < 3; ++v4) {
+        const float4 x = shp[(j4 / 4) * 3 + v4];
+        in[4 * v4] = x.x; in[4 * v4 + 1] = x.y; in[4 * v4 + 2] = x.z; in[4 * v4 + 3] = x.w;
       }
 #pragma unroll
-      for (int m = 0; m < 3; ++m) gd[m] += dY[j][m] * dot;
+      for (int jj = 0; jj < 4; ++jj) {
+        const bool live = j4 + jj < nc;
+        double dot = 0.0;
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) {
+          o[3 * jj + ch] = live ? (float)(Y[j4 + jj] * gr[ch]) : 0.f;
+          dot += (double)in[3 * jj + ch] * gr[ch];
+        }
+        if (live) {
+#pragma unroll
+          for (int m = 0; m < 3; ++m) gd[m] += dY[j4 + jj][m] * dot;
+        }
+      }
+#pragma unroll
+      for (int v4 = 0; v4 < 3; ++v4) dsh[(j4 / 4) * 3 + v4] = make_float4(o[4 * v4], o[4 * v4 + 1], o[4 * v4 + 2], o[4 * v4 + 3]);
     }
     const double dg = d[0] * gd[0] + d[1] * gd[1] + d[2] * gd[2];
 #pragma unroll
@@ -214,26 +228,55 @@ __global__ void __launch_bounds__(128) preprocess_backward_kernel(gabsplat_scene
   if (g.d_mean2d_abs) { g.d_mean2d_abs[2 * i] = g2[9 + 3 * K]; g.d_mean2d_abs[2 * i + 1] = g2[10 + 3 * K]; }
 }
 
+constexpr int kBwdThreads = 128;
+constexpr int kBwdChunk = 512;
+
+// zero p[begin, end) (elements; begin is a multiple of 4 and p is 16-byte aligned), all threads of the CTA
+__device__ __forceinline__ void zero_range(float* __restrict__ p, size_t begin, size_t end) {
+  const size_t n4 = (end - begin) / 4;
+  float4* p4 = reinterpret_cast<float4*>(p + begin);
+  for (size_t j = threadIdx.x; j < n4; j += kBwdThreads) p4[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (size_t j = begin + 4 * n4 + threadIdx.x; j < end; j += kBwdThreads) p[j] = 0.f;
+}
+
+// One CTA per chunk of kBwdChunk consecutive primitives: (0) zero the chunk's slice of every gradient array
+// with coalesced 16-byte stores (most primitives are culled and get exactly zero), (1) compact the visible
+// primitives of the chunk into shared memory, (2) walk the compacted list with all lanes busy.
+__global__ void __launch_bounds__(kBwdThreads, 3) preprocess_backward_kernel(gabsplat_scene s, Camera c, const uint32_t* __restrict__ tiles_touched,
+                                                                         const uint8_t* __restrict__ rgb_clamped,
+                                                                         const float* __restrict__ grad2d, gabsplat_grads g) {
+  __shared__ int s_i[kBwdChunk];
+  __shared__ int s_n;
+  if (threadIdx.x == 0) s_n = 0;
+  const size_t b = (size_t)blockIdx.x * kBwdChunk;
+  const size_t e = min((size_t)s.N, b + kBwdChunk);
+  const size_t K = (size_t)s.K;
+  zero_range(g.d_means, 3 * b, 3 * e);
+  zero_range(g.d_scales, 3 * b, 3 * e);
+  zero_range(g.d_rotations, 4 * b, 4 * e);
+  zero_range(g.d_opacities, b, e);
+  zero_range(g.d_sh, 48 * b, 48 * e);
+  if (K) {
+    zero_range(g.d_freqs, 3 * K * b, 3 * K * e);
+    zero_range(g.d_weights, K * b, K * e);
+  }
+  if (g.d_mean2d) zero_range(g.d_mean2d, 2 * b, 2 * e);
+  if (g.d_mean2d_abs) zero_range(g.d_mean2d_abs, 2 * b, 2 * e);
+  __syncthreads();
+  for (size_t i = b + threadIdx.x; i < e; i += kBwdThreads)
+    if (tiles_touched[i] != 0) s_i[atomicAdd(&s_n, 1)] = (int)i;
+  __syncthreads();  // also orders the zero stores before the value stores of other threads
+  const int n = s_n;
+  for (int j = threadIdx.x; j < n; j += kBwdThreads) backward_one(s, c, rgb_clamped, grad2d, g, s_i[j]);
+}
+
 }  // namespace
 
 cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& proj,
                                        const float* grad2d, const gabsplat_grads& g, cudaStream_t st) {
-  const size_t N = (size_t)s.N, K = (size_t)s.K;
-  cudaMemsetAsync(g.d_means, 0, N * 3 * sizeof(float), st);
-  cudaMemsetAsync(g.d_scales, 0, N * 3 * sizeof(float), st);
-  cudaMemsetAsync(g.d_rotations, 0, N * 4 * sizeof(float), st);
-  cudaMemsetAsync(g.d_opacities, 0, N * sizeof(float), st);
-  cudaMemsetAsync(g.d_sh, 0, N * 48 * sizeof(float), st);
-  if (K) {
-    cudaMemsetAsync(g.d_freqs, 0, N * K * 3 * sizeof(float), st);
-    cudaMemsetAsync(g.d_weights, 0, N * K * sizeof(float), st);
-  }
-  if (g.d_mean2d) cudaMemsetAsync(g.d_mean2d, 0, N * 2 * sizeof(float), st);
-  if (g.d_mean2d_abs) cudaMemsetAsync(g.d_mean2d_abs, 0, N * 2 * sizeof(float), st);
   if (s.N == 0) return cudaGetLastError();
-  const int block = 128;
-  preprocess_backward_kernel<<<(s.N + block - 1) / block, block, 0, st>>>(s, cam, proj.tiles_touched, proj.rgb_clamped,
-                                                                       grad2d, g);
+  preprocess_backward_kernel<<<(s.N + kBwdChunk - 1) / kBwdChunk, kBwdThreads, 0, st>>>(s, cam, proj.tiles_touched,
+                                                                                     proj.rgb_clamped, grad2d, g);
   launched();
   return cudaGetLastError();
 }
