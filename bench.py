@@ -259,7 +259,7 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
         gb.gabsplat_preprocess(ctx, ds, cams[v], proj)
         b = gb.gabsplat_bin_sort(ctx, N, proj, cams[v], capacity=None)
         Ds.append(b.D)
-        fwd = gb.gabsplat_render_forward(ctx, ds, cams[v], proj, b)
+        fwd = gb.gabsplat_render_forward(ctx, ds, cams[v], proj, b, save_state=False)
         cnt = gb.gabsplat_count_pairs(ctx, ds, cams[v], proj, b).to(torch.int64).reshape(-1, 4).sum(0).tolist()
         stats.append({"n_visible": int((proj.tiles_touched != 0).sum().item()), "D": b.D, "examined": cnt[0],
                       "envelope": cnt[1], "blended": cnt[2], "envelope_le_last": cnt[3],
@@ -268,7 +268,7 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     del probe
     capacity = max(Ds)
     bins = gb.Binning(N, cams[0], capacity, dev)
-    fwd = gb.FwdOut(cams[0], dev)
+    fwd = gb.FwdOut(cams[0], dev, capacity if backward else None)
     grads = gb.Grads(N, K, dev, with_mean2d=False) if backward else None
 
     my_view = lambda i: (i + rank) % V
@@ -277,7 +277,9 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
         v = my_view(i)
         gb.gabsplat_preprocess(ctx, ds, cams[v], proj)
         gb.gabsplat_bin_sort(ctx, N, proj, cams[v], bin=bins, read_count=False)
-        gb.gabsplat_render_forward(ctx, ds, cams[v], proj, bins, fwd)
+        # a forward that is followed by a backward records the blend state the backward replays;
+        # a forward-only step (inference) does not
+        gb.gabsplat_render_forward(ctx, ds, cams[v], proj, bins, fwd, save_state=do_backward)
         if do_backward:
             gb.gabsplat_render_backward(ctx, ds, cams[v], proj, bins, fwd, dLs[v], grads)
 

@@ -25,6 +25,7 @@
  *   - Return value: one of the GABSPLAT_* status codes.  Nothing is printed, nothing aborts.
  *   - There is no CPU fallback: on a machine without a usable sm_100 device gabsplat_create fails.
  *   - All floating-point storage is IEEE binary32, contiguous, row-major in the index order written.
+ *   - Every device pointer must be 16-byte aligned (the kernels use 128-bit loads and stores).
  *
  * Value contract (activated inputs): scales > 0, rotations are unit quaternions (w,x,y,z)
  * and are not re-normalised, opacities in (0,1), weights omega_k in [0,1) (omega >= 0 is relied on by the
@@ -118,7 +119,17 @@ typedef struct {
   float* image;        /* [3][H][W] */
   float* final_T;      /* [H][W]    */
   uint32_t* n_contrib; /* [H][W]    */
+  /* Optional (NULL for inference): device scratch of >= gabsplat_blend_state_bytes(...) bytes in which the
+   * forward records, per half tile (one warp's 16x8 pixels), the list of primitives that were blended at one
+   * of its pixels and a 128-bit mask of those pixels.  gabsplat_render_backward replays these lists in
+   * reverse and REQUIRES them: it neither re-walks the tile lists nor re-takes any skip/stop decision. */
+  void* blend_state;
+  uint64_t blend_state_bytes;
 } gabsplat_fwd_out;
+
+/* Bytes of gabsplat_fwd_out.blend_state for an image of this size and `capacity` instance slots
+ * (worst case: every instance of a tile's list is blended in both half tiles; 40 bytes per slot). */
+uint64_t gabsplat_blend_state_bytes(int32_t width, int32_t height, uint64_t capacity);
 
 /* Gradient outputs (all required except d_mean2d / d_mean2d_abs, which may be NULL). */
 typedef struct {

@@ -50,7 +50,8 @@ class _Binning(C.Structure):
 
 
 class _FwdOut(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in ("image", "final_T", "n_contrib")]
+    _fields_ = [(n, C.c_void_p) for n in ("image", "final_T", "n_contrib", "blend_state")] + [
+        ("blend_state_bytes", C.c_uint64)]
 
 
 class _Grads(C.Structure):
@@ -79,6 +80,8 @@ def lib():
         L.gabsplat_packed_floats.restype = C.c_int32
         L.gabsplat_sort_workspace_bytes.argtypes = [C.c_int32, C.c_uint64]
         L.gabsplat_sort_workspace_bytes.restype = C.c_uint64
+        L.gabsplat_blend_state_bytes.argtypes = [C.c_int32, C.c_int32, C.c_uint64]
+        L.gabsplat_blend_state_bytes.restype = C.c_uint64
         L.gabsplat_grad_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
         L.gabsplat_grad_workspace_bytes.restype = C.c_uint64
         L.gabsplat_host_arena_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_uint64]
@@ -245,15 +248,27 @@ class Binning:
 
 
 class FwdOut:
-    def __init__(self, cam, device):
+    """capacity = the binning's instance capacity allocates the blend state the backward replays;
+    capacity=None is inference mode (gabsplat_render_backward then refuses this output)."""
+
+    def __init__(self, cam, device, capacity: int | None = None):
         H, W = cam.height, cam.width
         self.image = torch.zeros((3, H, W), dtype=torch.float32, device=device)
         self.final_T = torch.zeros((H, W), dtype=torch.float32, device=device)
         self.n_contrib = torch.zeros((H, W), dtype=torch.int32, device=device)
+        self.blend_state = None
+        self.blend_state_bytes = 0
+        if capacity is not None:
+            self.blend_state_bytes = int(lib().gabsplat_blend_state_bytes(W, H, int(capacity)))
+            self.blend_state = torch.empty((self.blend_state_bytes,), dtype=torch.uint8, device=device)
 
-    def struct(self) -> _FwdOut:
+    def struct(self, save_state: bool = True) -> _FwdOut:
         o = _FwdOut()
         o.image, o.final_T, o.n_contrib = self.image.data_ptr(), self.final_T.data_ptr(), self.n_contrib.data_ptr()
+        if save_state and self.blend_state is not None:
+            o.blend_state, o.blend_state_bytes = self.blend_state.data_ptr(), self.blend_state_bytes
+        else:
+            o.blend_state, o.blend_state_bytes = None, 0
         return o
 
 
@@ -309,9 +324,10 @@ def gabsplat_bin_sort(ctx: Context, N: int, proj: Projected, cam, bin: Binning |
 
 
 def gabsplat_render_forward(ctx: Context, scene: DeviceScene, cam, proj: Projected, bin: Binning,
-                            out: FwdOut | None = None, stream=None) -> FwdOut:
-    out = FwdOut(cam, scene.means.device) if out is None else out
-    s, c, p, b, o = scene.struct(), camera_struct(cam), proj.struct(), bin.struct(), out.struct()
+                            out: FwdOut | None = None, stream=None, save_state: bool = True) -> FwdOut:
+    """save_state=False renders without recording the blend state (inference; no backward afterwards)."""
+    out = FwdOut(cam, scene.means.device, bin.capacity if save_state else None) if out is None else out
+    s, c, p, b, o = scene.struct(), camera_struct(cam), proj.struct(), bin.struct(), out.struct(save_state)
     ctx.check(lib().gabsplat_render_forward(ctx._h, C.byref(s), C.byref(c), C.byref(p), C.byref(b), C.byref(o),
                                             _stream(stream)))
     return out

@@ -107,6 +107,11 @@ uint64_t gabsplat_sort_workspace_bytes(int32_t N, uint64_t capacity) {
   return sort_workspace_bytes(N < 0 ? 0 : N, capacity);
 }
 
+uint64_t gabsplat_blend_state_bytes(int32_t width, int32_t height, uint64_t capacity) {
+  if (width <= 0 || height <= 0) return 0;
+  return blend_state_bytes((uint64_t)((width + kTile - 1) / kTile) * ((height + kTile - 1) / kTile), capacity);
+}
+
 uint64_t gabsplat_grad_workspace_bytes(int32_t N, int32_t K) {
   if (N < 0 || K < 0 || K > kMaxK) return 0;
   return (uint64_t)N * grad2d_floats(K) * sizeof(float) + 256;
@@ -156,8 +161,17 @@ int32_t gabsplat_render_forward(gabsplat_ctx* ctx, const gabsplat_scene* scene, 
   if (!proj || (scene->N > 0 && !proj->packed)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: null packed records");
   if (!bin || !bin->tile_ranges || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: bad binning");
   if (!out || !out->image || !out->final_T || !out->n_contrib) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: null output");
+  const Camera c = make_camera(*cam);
+  const uint64_t tiles = (uint64_t)c.tiles_x * c.tiles_y;
+  BlendState save;
+  if (out->blend_state) {
+    if (out->blend_state_bytes < blend_state_bytes(tiles, bin->capacity))
+      return fail(ctx, GABSPLAT_CAPACITY, "render_forward: blend_state too small");
+    save = make_blend_state(out->blend_state, tiles, bin->capacity);
+  }
   ctx->timer.begin(GABSPLAT_STAGE_BLEND_FORWARD, (cudaStream_t)stream);
-  const cudaError_t e = launch_blend_forward(scene->K, make_camera(*cam), *proj, *bin, *out, (cudaStream_t)stream);
+  const cudaError_t e = launch_blend_forward(scene->K, c, *proj, *bin, *out, out->blend_state ? &save : nullptr,
+                                             (cudaStream_t)stream);
   ctx->timer.end((cudaStream_t)stream);
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "render_forward");
 }
@@ -172,6 +186,8 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
   if (!projected_ok(proj, scene->N, scene->K)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: null projected arrays");
   if (!bin || !bin->tile_ranges || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: bad binning");
   if (!fwd || !fwd->final_T || !fwd->n_contrib || !dL_dimage) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: null forward state");
+  if (!fwd->blend_state)
+    return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: the forward was run without blend_state (inference mode)");
   if (!grads) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: null grads");
   if (scene->N > 0 && (!grads->d_means || !grads->d_scales || !grads->d_rotations || !grads->d_opacities || !grads->d_sh ||
                        (scene->K > 0 && (!grads->d_freqs || !grads->d_weights))))
@@ -181,8 +197,13 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
   cudaStream_t st = (cudaStream_t)stream;
   const Camera c = make_camera(*cam);
   float* grad2d = reinterpret_cast<float*>(((uintptr_t)grad_workspace + 255) & ~(uintptr_t)255);
+  const uint64_t tiles = (uint64_t)c.tiles_x * c.tiles_y;
+  if (fwd->blend_state_bytes < blend_state_bytes(tiles, bin->capacity))
+    return fail(ctx, GABSPLAT_CAPACITY, "render_backward: blend_state too small");
+  const BlendState saved = make_blend_state(fwd->blend_state, tiles, bin->capacity);
   ctx->timer.begin(GABSPLAT_STAGE_BLEND_BACKWARD, st);
-  cudaError_t e = launch_blend_backward(scene->N, scene->K, grads->d_mean2d_abs != nullptr, c, *proj, *bin, *fwd, dL_dimage, grad2d, st);
+  cudaError_t e = launch_blend_backward(scene->N, scene->K, grads->d_mean2d_abs != nullptr, c, *proj, *bin, *fwd, saved,
+                                        dL_dimage, grad2d, st);
   ctx->timer.end(st);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "render_backward (blend)");
   ctx->timer.begin(GABSPLAT_STAGE_PREPROCESS_BACKWARD, st);

@@ -1,8 +1,8 @@
 // S4a / K7: the blend in reverse (gradients of sum_p <dL/dC(p), C(p)> with respect to the projected
 // quantities of every primitive, including f2D and omega; PAPER.md:48, :129 -- derivation in DESIGN.md).
-// Same CTA / pixel mapping and staging as the forward kernel (blend_common.cuh): 64 threads per tile, 4 pixels
-// per thread.  Pixels walk the tile list back to front from the tile's deepest contributor and recover the
-// transmittance in front of each primitive by division.  Per staged primitive a thread first sums the
+// Same CTA / pixel mapping as the forward kernel (blend_common.cuh): 64 threads per tile, 4 pixels per thread.
+// Each warp replays the list of blended primitives the forward saved for its half tile, back to front, and
+// recovers the transmittance in front of each primitive by division.  Per primitive a thread first sums the
 // gradient contributions of its 4 pixels in registers; the 9+3K (+2) sums are then reduced over the warp with a
 // butterfly that halves the number of live values at every exchange (one shuffle per value pair instead of
 // five per value) and leaves value i on lane idx(i), so the warp issues ONE vector of atomic adds per primitive.
@@ -61,94 +61,103 @@ __device__ __forceinline__ int reduce_index(int lane, int i) {
   return valid ? rel : -1;
 }
 
+constexpr int kReplay = 32;  // saved entries staged per warp and batch
+
 // ABS: also accumulate sum |dL/dmu2D| per pixel (AbsGS densification statistic).
+//
+// Every warp replays, back to front, the list the forward saved for its half tile (BlendState): the
+// primitives that were blended at one of the warp's 128 pixels, with the ballots of the blending lanes.  No
+// tile list is walked, no skip / stop decision is re-taken, and the two warps of a CTA never synchronise.
+// A lane recomputes G, cos, sin and alpha of its blended pixels with the forward's own functions (bit-identical
+// alpha), recovers the transmittance in front of the primitive by division, and accumulates the gradient terms.
 template <int K, bool ABS>
 __global__ void __launch_bounds__(kBlendThreads) blend_backward_kernel(Camera cam, const uint2* __restrict__ ranges,
-                                                                       const uint32_t* __restrict__ ids,
-                                                                       const float4* __restrict__ packed,
+                                                                       BlendState saved, const float4* __restrict__ packed,
                                                                        const float* __restrict__ final_T,
-                                                                       const uint32_t* __restrict__ n_contrib,
                                                                        const float* __restrict__ dL_dimage,
                                                                        float* __restrict__ grad2d) {
   constexpr int R4 = packed_floats(K) / 4;
   constexpr int TL = K > 0 ? tail_floats(K) : 1;
   constexpr int NV = 9 + 3 * K + (ABS ? 2 : 0);
   constexpr int GF = grad2d_floats(K);
-  __shared__ float4 s_rec[kBatch * R4];
-  __shared__ uint32_t s_cnt[8];
-  __shared__ uint32_t s_max[kBlendThreads / 32];
+  constexpr int kWarps = kBlendThreads / 32;
+  __shared__ float4 s_rec[kWarps][kReplay * R4];
+  __shared__ uint4 s_mask[kWarps][kReplay];
+  __shared__ uint32_t s_id[kWarps][kReplay];
   const TileGeom g = tile_geom(cam);
   const uint2 range = ranges[g.tile];
   const size_t HW = (size_t)cam.width * cam.height;
+  const int cnt = (int)saved.counts[2 * g.tile + g.warp];
+  const size_t base = 2 * (size_t)range.x + (size_t)g.warp * (range.y - range.x);
+  float4* __restrict__ rec = s_rec[g.warp];
 
   float T[kSlots], gC[kSlots][3], B[kSlots][3];
-  uint32_t last[kSlots];
-  uint32_t mx = 0;
 #pragma unroll
   for (int s = 0; s < kSlots; ++s) {
-    T[s] = 0.f; last[s] = 0;
+    T[s] = 0.f;
     gC[s][0] = gC[s][1] = gC[s][2] = 0.f;
     if (g.inside[s]) {
       const size_t pix = (size_t)g.py[s] * cam.width + g.px;
       T[s] = final_T[pix];
-      last[s] = n_contrib[pix];
       gC[s][0] = dL_dimage[pix]; gC[s][1] = dL_dimage[HW + pix]; gC[s][2] = dL_dimage[2 * HW + pix];
     }
     B[s][0] = cam.bg[0]; B[s][1] = cam.bg[1]; B[s][2] = cam.bg[2];  // colour behind the current primitive
-    mx = max(mx, last[s]);
   }
-  // the tile's deepest contributor
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) mx = max(mx, __shfl_xor_sync(kFull, mx, d));
-  if (g.lane == 0) s_max[g.warp] = mx;
-  __syncthreads();
-  uint32_t n_eff = 0;
-#pragma unroll
-  for (int w = 0; w < kBlendThreads / 32; ++w) n_eff = max(n_eff, s_max[w]);
 
   constexpr int NL = reduce_left(NV);
   int my_idx[NL];
 #pragma unroll
   for (int i = 0; i < NL; ++i) my_idx[i] = reduce_index<NV>(g.lane, i);
 
-  // batches from the back: candidate c of a batch is 1-based list position end - c
-  for (int end = (int)n_eff; end > 0; end -= kBatch) {
-    const int m = min(kBatch, end);
-    const int ns = stage_batch<K, true>(g, ids, packed, range.x, end - 1, m, s_rec, s_cnt);
-    for (int j = 0; j < ns; ++j) {
-      const float4 h0 = s_rec[j * R4], h1 = s_rec[j * R4 + 1];
-      const uint32_t pos = __float_as_uint(h1.z);
-      const float dx = __fsub_rn(g.lx, h0.x);
-      const float ux = __fmul_rn(h0.z, dx);
-      float dy[kSlots], q[kSlots], u[kSlots], v[kSlots];
-      bool pass[kSlots];
-      bool any = false;
+  // batches from the back: lane l of a batch stages saved entry end - 1 - l
+  for (int end = cnt; end > 0; end -= kReplay) {
+    const int m = min(kReplay, end);
+    uint32_t my_id = 0;
+    uint4 my_mask = make_uint4(0u, 0u, 0u, 0u);
+    if (g.lane < m) {
+      my_id = __ldg(saved.ids + base + (size_t)(end - 1 - g.lane));
+      my_mask = __ldg(saved.masks + base + (size_t)(end - 1 - g.lane));
+    }
+    s_id[g.warp][g.lane] = my_id;
+    s_mask[g.warp][g.lane] = my_mask;
 #pragma unroll
-      for (int s = 0; s < kSlots; ++s) {
-        dy[s] = __fsub_rn(g.ly[s], h0.y);
-        q[s] = envelope_q(ux, h0.w, h1.x, dy[s], u[s], v[s]);
-        pass[s] = pos <= last[s] && !(q[s] < h1.y);
-        any = any || pass[s];
+    for (int it = 0; it < R4; ++it) {
+      const int idx = it * 32 + g.lane;
+      const int r = idx / R4, part = idx - r * R4;
+      const uint32_t id_r = __shfl_sync(kFull, my_id, r);
+      if (r < m) {
+        float4 v = __ldg(packed + (size_t)id_r * R4 + part);
+        if (part == 0) {  // mean relative to the tile origin, as the forward computes it: (hi - origin) + lo
+          v.x = __fadd_rn(__fsub_rn(v.x, g.x0), v.z);
+          v.y = __fadd_rn(__fsub_rn(v.y, g.y0), v.w);
+        }
+        rec[idx] = v;
       }
-      if (!__any_sync(kFull, any)) continue;  // warp-uniform
-
-      const float4 oc = s_rec[j * R4 + 2];
+    }
+    __syncwarp();
+    for (int j = 0; j < m; ++j) {
+      const uint4 mk = s_mask[g.warp][j];
+      const float4 a = rec[j * R4], l = rec[j * R4 + 1], oc = rec[j * R4 + 2];
+      const bool hit[kSlots] = {((mk.x >> g.lane) & 1u) != 0u, ((mk.y >> g.lane) & 1u) != 0u,
+                                ((mk.z >> g.lane) & 1u) != 0u, ((mk.w >> g.lane) & 1u) != 0u};
       float tail[TL];
-      if (K > 0) load_tail<K>(s_rec + j * R4, tail);
+      if (K > 0) load_tail<K>(rec + j * R4, tail);
+      const float dx = __fsub_rn(g.lx, a.x);
+      const float ux = __fmul_rn(l.x, dx);
       float acc[NV];
 #pragma unroll
       for (int i = 0; i < NV; ++i) acc[i] = 0.f;
-      bool hit_any = false;
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) {
-        if (!pass[s]) continue;
-        const float G = __expf(q[s]);
+        if (!hit[s]) continue;
+        float u, v;
+        const float dy = __fsub_rn(g.ly[s], a.y);
+        const float q = envelope_q(ux, l.y, l.z, dy, u, v);
+        const float G = __expf(q);
         Modulation<K> e;
-        modulation<K, true>(tail, dx, dy[s], e);
+        modulation<K, true>(tail, dx, dy, e);
         const float raw = __fmul_rn(__fmul_rn(oc.x, G), e.M);
         const float alpha = fminf(kAlphaMax, raw);
-        if (alpha < kAlphaMin) continue;
-        hit_any = true;
         const float om = 1.0f - alpha;
         const float Ti = __fdividef(T[s], om);  // transmittance in front of this primitive
         T[s] = Ti;
@@ -163,17 +172,17 @@ __global__ void __launch_bounds__(kBlendThreads) blend_backward_kernel(Camera ca
           const float gM = galpha * oc.x * G;
           const float gq = galpha * raw;  // dL/dq = g_G * G
           // q = -(u^2 + v^2), u = L11 dx + L21 dy, v = L22 dy
-          float gdx = gq * (-2.0f * u[s] * h0.z);
-          float gdy = gq * (-2.0f * (u[s] * h0.w + v[s] * h1.x));
+          float gdx = gq * (-2.0f * u * l.x);
+          float gdy = gq * (-2.0f * (u * l.y + v * l.z));
           acc[2] += gq * (-0.5f * dx * dx);
-          acc[3] += gq * (-dx * dy[s]);
-          acc[4] += gq * (-0.5f * dy[s] * dy[s]);
+          acc[3] += gq * (-dx * dy);
+          acc[4] += gq * (-0.5f * dy * dy);
 #pragma unroll
           for (int k = 0; k < K; ++k) {
             acc[9 + 2 * K + k] += gM * (e.cs[k] - 1.0f);
             const float gph = -gM * tail[2 * K + k] * e.sn[k];  // dL/d(phase in radians)
             acc[9 + 2 * k] += gph * dx;
-            acc[9 + 2 * k + 1] += gph * dy[s];
+            acc[9 + 2 * k + 1] += gph * dy;
             gdx += gph * tail[2 * k];
             gdy += gph * tail[2 * k + 1];
           }
@@ -181,40 +190,40 @@ __global__ void __launch_bounds__(kBlendThreads) blend_backward_kernel(Camera ca
           if (ABS) { acc[9 + 3 * K] += fabsf(gdx); acc[10 + 3 * K] += fabsf(gdy); }
         }
       }
-      if (!__any_sync(kFull, hit_any)) continue;
       Butterfly<NV, 16>::run(acc, g.lane);
-      float* dst = grad2d + (size_t)__float_as_uint(h1.w) * GF;
+      float* dst = grad2d + (size_t)s_id[g.warp][j] * GF;
 #pragma unroll
       for (int i = 0; i < NL; ++i)
         if (my_idx[i] >= 0 && acc[i] != 0.f) atomicAdd(dst + my_idx[i], acc[i]);
     }
+    __syncwarp();
   }
 }
 
 template <int K, bool ABS>
 cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
-                     const gabsplat_fwd_out& fwd, const float* dL, float* grad2d, cudaStream_t st) {
+                     const gabsplat_fwd_out& fwd, const BlendState& saved, const float* dL, float* grad2d, cudaStream_t st) {
   const int ntiles = cam.tiles_x * cam.tiles_y;
   blend_backward_kernel<K, ABS><<<ntiles, kBlendThreads, 0, st>>>(
-      cam, reinterpret_cast<const uint2*>(bin.tile_ranges), bin.ids, reinterpret_cast<const float4*>(proj.packed),
-      fwd.final_T, fwd.n_contrib, dL, grad2d);
+      cam, reinterpret_cast<const uint2*>(bin.tile_ranges), saved, reinterpret_cast<const float4*>(proj.packed),
+      fwd.final_T, dL, grad2d);
   launched();
   return cudaGetLastError();
 }
 
 template <bool ABS>
 cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
-                     const gabsplat_fwd_out& fwd, const float* dL, float* grad2d, cudaStream_t st) {
+                     const gabsplat_fwd_out& fwd, const BlendState& saved, const float* dL, float* grad2d, cudaStream_t st) {
   switch (K) {
-    case 0: return launch_k<0, ABS>(cam, proj, bin, fwd, dL, grad2d, st);
-    case 1: return launch_k<1, ABS>(cam, proj, bin, fwd, dL, grad2d, st);
-    case 2: return launch_k<2, ABS>(cam, proj, bin, fwd, dL, grad2d, st);
-    case 3: return launch_k<3, ABS>(cam, proj, bin, fwd, dL, grad2d, st);
-    case 4: return launch_k<4, ABS>(cam, proj, bin, fwd, dL, grad2d, st);
-    case 5: return launch_k<5, ABS>(cam, proj, bin, fwd, dL, grad2d, st);
-    case 6: return launch_k<6, ABS>(cam, proj, bin, fwd, dL, grad2d, st);
-    case 7: return launch_k<7, ABS>(cam, proj, bin, fwd, dL, grad2d, st);
-    case 8: return launch_k<8, ABS>(cam, proj, bin, fwd, dL, grad2d, st);
+    case 0: return launch_k<0, ABS>(cam, proj, bin, fwd, saved, dL, grad2d, st);
+    case 1: return launch_k<1, ABS>(cam, proj, bin, fwd, saved, dL, grad2d, st);
+    case 2: return launch_k<2, ABS>(cam, proj, bin, fwd, saved, dL, grad2d, st);
+    case 3: return launch_k<3, ABS>(cam, proj, bin, fwd, saved, dL, grad2d, st);
+    case 4: return launch_k<4, ABS>(cam, proj, bin, fwd, saved, dL, grad2d, st);
+    case 5: return launch_k<5, ABS>(cam, proj, bin, fwd, saved, dL, grad2d, st);
+    case 6: return launch_k<6, ABS>(cam, proj, bin, fwd, saved, dL, grad2d, st);
+    case 7: return launch_k<7, ABS>(cam, proj, bin, fwd, saved, dL, grad2d, st);
+    case 8: return launch_k<8, ABS>(cam, proj, bin, fwd, saved, dL, grad2d, st);
   }
   return cudaErrorInvalidValue;
 }
@@ -222,11 +231,11 @@ cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, c
 }  // namespace
 
 cudaError_t launch_blend_backward(int N, int K, bool want_abs, const Camera& cam, const gabsplat_projected& proj,
-                                  const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const float* dL_dimage,
-                                  float* grad2d, cudaStream_t st) {
+                                  const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const BlendState& saved,
+                                  const float* dL_dimage, float* grad2d, cudaStream_t st) {
   cudaMemsetAsync(grad2d, 0, (size_t)N * grad2d_floats(K) * sizeof(float), st);
-  return want_abs ? dispatch<true>(K, cam, proj, bin, fwd, dL_dimage, grad2d, st)
-                  : dispatch<false>(K, cam, proj, bin, fwd, dL_dimage, grad2d, st);
+  return want_abs ? dispatch<true>(K, cam, proj, bin, fwd, saved, dL_dimage, grad2d, st)
+                  : dispatch<false>(K, cam, proj, bin, fwd, saved, dL_dimage, grad2d, st);
 }
 
 }  // namespace gabsplat

@@ -10,13 +10,15 @@ namespace {
 
 // COUNT = the instrumented variant behind gabsplat_count_pairs: same decisions; per pixel the number of list
 // entries examined / past the envelope test / blended is written to `counters` instead of the image.
-template <int K, bool COUNT>
+// SAVE = also record, per warp (half tile), the primitives blended at one of its pixels and the ballots of the
+// blending lanes (common.cuh BlendState): the backward replays exactly this list.
+template <int K, bool COUNT, bool SAVE>
 __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam, const uint2* __restrict__ ranges,
                                                                       const uint32_t* __restrict__ ids,
                                                                       const float4* __restrict__ packed,
                                                                       float* __restrict__ image, float* __restrict__ final_T,
                                                                       uint32_t* __restrict__ n_contrib,
-                                                                      uint32_t* __restrict__ counters) {
+                                                                      uint32_t* __restrict__ counters, BlendState save) {
   constexpr int R4 = packed_floats(K) / 4;
   constexpr int TL = K > 0 ? 4 * ((3 * K + 3) / 4) : 1;
   __shared__ float4 s_rec[kBatch * R4];
@@ -38,12 +40,14 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
     stop_pos[s] = 0;
   }
 
+  uint32_t n_saved = 0;                                        // warp-uniform
+  const size_t save_at = 2 * (size_t)range.x + (size_t)g.warp * n;  // this warp's slice of save.ids / save.masks
   for (int b0 = 0; b0 < n; b0 += kBatch) {
     const bool all_done = done[0] && done[1] && done[2] && done[3];
     if (__syncthreads_and(all_done)) break;
     const int m = min(kBatch, n - b0);
     const int ns = stage_batch<K, false>(g, ids, packed, range.x, b0, m, s_rec, s_cnt);
-    if (all_done) continue;
+    if (__all_sync(kFull, all_done)) continue;  // warp-uniform: the votes below need every lane
     for (int j = 0; j < ns; ++j) {
       const float4 h0 = s_rec[j * R4], h1 = s_rec[j * R4 + 1];
       const float dx = __fsub_rn(g.lx, h0.x);
@@ -59,13 +63,15 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
         pass[s] = !(q[s] < h1.y) && !done[s];  // envelope reject: o G < 1/255 and M <= 1
         any = any || pass[s];
       }
-      if (!any) continue;
+      if (!__any_sync(kFull, any)) continue;  // warp-uniform
       const float4 oc = s_rec[j * R4 + 2];
       float tail[TL];
       if (K > 0) load_tail<K>(s_rec + j * R4, tail);
       const uint32_t pos = __float_as_uint(h1.z);
+      bool blended[kSlots];
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) {
+        blended[s] = false;
         if (!pass[s]) continue;
         if (COUNT) ++n_env[s];
         const float G = __expf(q[s]);
@@ -86,10 +92,24 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
         Cb[s] = __fmaf_rn(oc.w, wgt, Cb[s]);
         T[s] = Tn;
         last[s] = pos;
+        blended[s] = true;
         if (COUNT) { ++n_blend[s]; n_env_last[s] = n_env[s]; }
+      }
+      if (SAVE) {
+        uint4 m;
+        m.x = __ballot_sync(kFull, blended[0]); m.y = __ballot_sync(kFull, blended[1]);
+        m.z = __ballot_sync(kFull, blended[2]); m.w = __ballot_sync(kFull, blended[3]);
+        if ((m.x | m.y | m.z | m.w) != 0u) {
+          if (g.lane == 0) {
+            save.ids[save_at + n_saved] = __float_as_uint(h1.w);
+            save.masks[save_at + n_saved] = m;
+          }
+          ++n_saved;
+        }
       }
     }
   }
+  if (SAVE && g.lane == 0) save.counts[2 * g.tile + g.warp] = n_saved;
   const size_t HW = (size_t)cam.width * cam.height;
 #pragma unroll
   for (int s = 0; s < kSlots; ++s) {
@@ -109,30 +129,30 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
   }
 }
 
-template <int K, bool COUNT>
+template <int K, bool COUNT, bool SAVE>
 cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, float* image,
-                     float* final_T, uint32_t* n_contrib, uint32_t* counters, cudaStream_t st) {
+                     float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save, cudaStream_t st) {
   const int ntiles = cam.tiles_x * cam.tiles_y;
-  blend_forward_kernel<K, COUNT><<<ntiles, kBlendThreads, 0, st>>>(
+  blend_forward_kernel<K, COUNT, SAVE><<<ntiles, kBlendThreads, 0, st>>>(
       cam, reinterpret_cast<const uint2*>(bin.tile_ranges), bin.ids, reinterpret_cast<const float4*>(proj.packed), image,
-      final_T, n_contrib, counters);
+      final_T, n_contrib, counters, save ? *save : BlendState{nullptr, nullptr, nullptr});
   launched();
   return cudaGetLastError();
 }
 
-template <bool COUNT>
+template <bool COUNT, bool SAVE>
 cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, float* image,
-                     float* final_T, uint32_t* n_contrib, uint32_t* counters, cudaStream_t st) {
+                     float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save, cudaStream_t st) {
   switch (K) {
-    case 0: return launch_k<0, COUNT>(cam, proj, bin, image, final_T, n_contrib, counters, st);
-    case 1: return launch_k<1, COUNT>(cam, proj, bin, image, final_T, n_contrib, counters, st);
-    case 2: return launch_k<2, COUNT>(cam, proj, bin, image, final_T, n_contrib, counters, st);
-    case 3: return launch_k<3, COUNT>(cam, proj, bin, image, final_T, n_contrib, counters, st);
-    case 4: return launch_k<4, COUNT>(cam, proj, bin, image, final_T, n_contrib, counters, st);
-    case 5: return launch_k<5, COUNT>(cam, proj, bin, image, final_T, n_contrib, counters, st);
-    case 6: return launch_k<6, COUNT>(cam, proj, bin, image, final_T, n_contrib, counters, st);
-    case 7: return launch_k<7, COUNT>(cam, proj, bin, image, final_T, n_contrib, counters, st);
-    case 8: return launch_k<8, COUNT>(cam, proj, bin, image, final_T, n_contrib, counters, st);
+    case 0: return launch_k<0, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
+    case 1: return launch_k<1, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
+    case 2: return launch_k<2, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
+    case 3: return launch_k<3, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
+    case 4: return launch_k<4, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
+    case 5: return launch_k<5, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
+    case 6: return launch_k<6, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
+    case 7: return launch_k<7, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
+    case 8: return launch_k<8, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
   }
   return cudaErrorInvalidValue;
 }
@@ -140,13 +160,15 @@ cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, c
 }  // namespace
 
 cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projected& proj,
-                                 const gabsplat_binning& bin, const gabsplat_fwd_out& out, cudaStream_t st) {
-  return dispatch<false>(K, cam, proj, bin, out.image, out.final_T, out.n_contrib, nullptr, st);
+                                 const gabsplat_binning& bin, const gabsplat_fwd_out& out, const BlendState* save,
+                                 cudaStream_t st) {
+  return save ? dispatch<false, true>(K, cam, proj, bin, out.image, out.final_T, out.n_contrib, nullptr, save, st)
+              : dispatch<false, false>(K, cam, proj, bin, out.image, out.final_T, out.n_contrib, nullptr, nullptr, st);
 }
 
 cudaError_t launch_count_pairs(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
                                uint32_t* counters, cudaStream_t st) {
-  return dispatch<true>(K, cam, proj, bin, nullptr, nullptr, nullptr, counters, st);
+  return dispatch<true, false>(K, cam, proj, bin, nullptr, nullptr, nullptr, counters, nullptr, st);
 }
 
 }  // namespace gabsplat

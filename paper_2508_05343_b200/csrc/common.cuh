@@ -34,6 +34,30 @@ __host__ __device__ constexpr int packed_floats(int K) { return 12 + tail_floats
 __host__ __device__ constexpr int grad2d_values(int K) { return 11 + 3 * K; }
 __host__ __device__ constexpr int grad2d_floats(int K) { return 4 * ((grad2d_values(K) + 3) / 4); }
 
+// ---- blend state saved by the forward for the backward (gabsplat_fwd_out.blend_state) ----------------
+// Per half tile h = 2 * tile + warp: counts[h] entries, stored at [2 * list_begin + warp * list_length, ...) of
+// ids / masks in the order they were blended (front to back): the primitive id and, for the warp's four
+// 16x2 pixel strips, the ballot of the lanes whose pixel blended the primitive.
+struct BlendState {
+  uint32_t* counts;  // [2 * tiles]
+  uint32_t* ids;     // [2 * capacity]
+  uint4* masks;      // [2 * capacity]
+};
+inline uint64_t blend_state_bytes(uint64_t tiles, uint64_t capacity) {
+  const uint64_t a = (2 * tiles * 4 + 255) & ~255ull, b = (2 * capacity * 4 + 255) & ~255ull;
+  return a + b + 2 * capacity * 16 + 256;
+}
+inline BlendState make_blend_state(void* p, uint64_t tiles, uint64_t capacity) {
+  BlendState s;
+  uintptr_t q = ((uintptr_t)p + 255) & ~(uintptr_t)255;
+  s.counts = reinterpret_cast<uint32_t*>(q);
+  q += (2 * tiles * 4 + 255) & ~255ull;
+  s.ids = reinterpret_cast<uint32_t*>(q);
+  q += (2 * capacity * 4 + 255) & ~255ull;
+  s.masks = reinterpret_cast<uint4*>(q);
+  return s;
+}
+
 struct Camera {  // device copy of gabsplat_camera plus derived integers
   int width, height, tiles_x, tiles_y;
   float fx, fy, cx, cy;
@@ -99,12 +123,13 @@ cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const 
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
                             StageTimer& tm, cudaStream_t st);
 cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projected& proj,
-                                 const gabsplat_binning& bin, const gabsplat_fwd_out& out, cudaStream_t st);
+                                 const gabsplat_binning& bin, const gabsplat_fwd_out& out, const BlendState* save,
+                                 cudaStream_t st);
 cudaError_t launch_count_pairs(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
                                uint32_t* counters, cudaStream_t st);
 cudaError_t launch_blend_backward(int N, int K, bool want_abs, const Camera& cam, const gabsplat_projected& proj,
-                                  const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const float* dL_dimage,
-                                  float* grad2d, cudaStream_t st);
+                                  const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const BlendState& saved,
+                                  const float* dL_dimage, float* grad2d, cudaStream_t st);
 cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& proj,
                                        const float* grad2d, const gabsplat_grads& g, cudaStream_t st);
 

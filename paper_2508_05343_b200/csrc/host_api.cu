@@ -63,6 +63,8 @@ Layout carve(void* base, int N, int K, int width, int height, uint64_t capacity)
   l.fwd.image = a.take<float>(3 * hw);
   l.fwd.final_T = a.take<float>(hw);
   l.fwd.n_contrib = a.take<uint32_t>(hw);
+  l.fwd.blend_state_bytes = blend_state_bytes(tiles, capacity);
+  l.fwd.blend_state = a.take<char>(l.fwd.blend_state_bytes);
   l.dL = a.take<float>(3 * hw);
   l.grads.d_means = a.take<float>(n * 3);
   l.grads.d_scales = a.take<float>(n * 3);
@@ -117,6 +119,7 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* sh, const 
   uint64_t D = 0;
   rc = gabsplat_bin_sort(ctx, sh->N, &l.proj, cam, &l.bin, &D, stream);
   if (rc != GABSPLAT_OK) return rc;
+  if (!dL_dimage_host) l.fwd.blend_state = nullptr;  // inference: nothing to replay
   rc = gabsplat_render_forward(ctx, &l.scene, cam, &l.proj, &l.bin, &l.fwd, stream);
   if (rc != GABSPLAT_OK) return rc;
   GS_D2H(image_host, l.fwd.image, 3 * hw);

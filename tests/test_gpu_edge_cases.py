@@ -134,3 +134,28 @@ def test_render_host_matches_device_path():
     assert np.array_equal(img.numpy(), ref["image"])
     for n in names:
         assert np.allclose(grads[n].numpy(), ref[n], rtol=1e-4, atol=1e-6 * np.abs(ref[n]).max())
+
+
+def test_inference_forward_has_no_blend_state():
+    """A forward run without blend_state (inference) gives the same image bit for bit, and the backward refuses
+    it with INVALID_ARG instead of silently re-deciding anything."""
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny")
+    cam = scenes.make_cameras("tiny")[0]
+    dL = torch.from_numpy(scenes.make_image_grad("tiny", 0, cam)).cuda()
+    ds = gb.upload_scene(scene)
+    proj = gb.gabsplat_preprocess(ctx, ds, cam)
+    bins = gb.gabsplat_bin_sort(ctx, ds.N, proj, cam)
+    train = gb.gabsplat_render_forward(ctx, ds, cam, proj, bins)
+    infer = gb.gabsplat_render_forward(ctx, ds, cam, proj, bins, save_state=False)
+    torch.cuda.synchronize()
+    assert torch.equal(train.image, infer.image) and torch.equal(train.n_contrib, infer.n_contrib)
+    with pytest.raises(gb.GabsplatError) as e:
+        gb.gabsplat_render_backward(ctx, ds, cam, proj, bins, infer, dL)
+    assert e.value.code == gb.INVALID_ARG
+    # the saved lists: per half tile at most the tile's list length, ids inside the tile's list
+    tiles = cam.tiles_x * cam.tiles_y
+    counts = train.blend_state[:].view(torch.int32)[:2 * tiles].cpu().numpy().reshape(tiles, 2)
+    ranges = bins.tile_ranges.cpu().numpy().view(np.uint32).reshape(tiles, 2)
+    assert np.all(counts <= (ranges[:, 1] - ranges[:, 0])[:, None])
+    assert counts.sum() > 0
