@@ -105,6 +105,8 @@ typedef struct {
   uint64_t* keys;             /* [capacity]  sorted on return: (tile_id << 32) | bits(depth)         */
   uint32_t* ids;              /* [capacity]  primitive index of each instance, same order            */
   uint32_t* tile_ranges;      /* [tiles_y*tiles_x][2]  [start,end) into keys/ids; (0,0) if empty     */
+  uint32_t* tile_order;       /* [tiles_y*tiles_x]  the tiles by descending list length: the order in
+                                 which the forward blend launches its CTAs (longest first)            */
   uint64_t capacity;
   uint32_t* num_instances;    /* [1]  device: D = total instance count                               */
   void* workspace;            /* device scratch, >= gabsplat_sort_workspace_bytes(N, capacity) bytes */

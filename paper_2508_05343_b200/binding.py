@@ -45,7 +45,7 @@ class _Projected(C.Structure):
 
 class _Binning(C.Structure):
     _fields_ = [("offsets", C.c_void_p), ("keys", C.c_void_p), ("ids", C.c_void_p), ("tile_ranges", C.c_void_p),
-                ("capacity", C.c_uint64), ("num_instances", C.c_void_p), ("workspace", C.c_void_p),
+                ("tile_order", C.c_void_p), ("capacity", C.c_uint64), ("num_instances", C.c_void_p), ("workspace", C.c_void_p),
                 ("workspace_bytes", C.c_uint64)]
 
 
@@ -231,6 +231,7 @@ class Binning:
         self.keys = z((max(self.capacity, 1),), torch.int64)
         self.ids = z((max(self.capacity, 1),), torch.int32)
         self.tile_ranges = z((self.n_tiles, 2), torch.int32)
+        self.tile_order = z((self.n_tiles,), torch.int32)
         self.num_instances = z((4,), torch.int32)
         self.workspace_bytes = int(lib().gabsplat_sort_workspace_bytes(N, self.capacity))
         self.workspace = z((self.workspace_bytes + 256,), torch.uint8)
@@ -240,6 +241,7 @@ class Binning:
         b = _Binning()
         b.offsets, b.keys, b.ids = self.offsets.data_ptr(), self.keys.data_ptr(), self.ids.data_ptr()
         b.tile_ranges = self.tile_ranges.data_ptr()
+        b.tile_order = self.tile_order.data_ptr()
         b.capacity = self.capacity
         b.num_instances = self.num_instances.data_ptr()
         b.workspace = (self.workspace.data_ptr() + 255) // 256 * 256

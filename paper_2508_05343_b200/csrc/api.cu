@@ -55,7 +55,7 @@ bool projected_ok(const gabsplat_projected* p, int N, int K) {
 }
 
 bool binning_ok(const gabsplat_binning* b, int N) {
-  if (!b || !b->tile_ranges || !b->num_instances) return false;
+  if (!b || !b->tile_ranges || !b->tile_order || !b->num_instances) return false;
   if (N > 0 && !b->offsets) return false;
   if (b->capacity > 0 && (!b->keys || !b->ids)) return false;
   if (b->capacity >= (1ull << 32)) return false;
@@ -159,7 +159,7 @@ int32_t gabsplat_render_forward(gabsplat_ctx* ctx, const gabsplat_scene* scene, 
   if (!scene || scene->K < 0 || scene->K > kMaxK || scene->N < 0) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: bad scene");
   if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: bad camera");
   if (!proj || (scene->N > 0 && !proj->packed)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: null packed records");
-  if (!bin || !bin->tile_ranges || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: bad binning");
+  if (!bin || !bin->tile_ranges || !bin->tile_order || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: bad binning");
   if (!out || !out->image || !out->final_T || !out->n_contrib) return fail(ctx, GABSPLAT_INVALID_ARG, "render_forward: null output");
   const Camera c = make_camera(*cam);
   const uint64_t tiles = (uint64_t)c.tiles_x * c.tiles_y;
@@ -246,7 +246,7 @@ int32_t gabsplat_count_pairs(gabsplat_ctx* ctx, const gabsplat_scene* scene, con
   if (!scene || scene->K < 0 || scene->K > kMaxK || scene->N < 0) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: bad scene");
   if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: bad camera");
   if (!proj || (scene->N > 0 && !proj->packed)) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: null packed records");
-  if (!bin || !bin->tile_ranges || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: bad binning");
+  if (!bin || !bin->tile_ranges || !bin->tile_order || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: bad binning");
   if (!counters) return fail(ctx, GABSPLAT_INVALID_ARG, "count_pairs: null output");
   const cudaError_t e = launch_count_pairs(scene->K, make_camera(*cam), *proj, *bin, counters, (cudaStream_t)stream);
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "count_pairs");

@@ -323,7 +323,20 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
     const bool valid = idx < n;
     const u32 d = (k[r] >> shift) & 255u;
     // lanes holding the same digit; invalid lanes get a digit value no valid lane can have
+#ifdef GS_SORT_MATCH_ANY
     const u32 peers = __match_any_sync(0xffffffffu, valid ? d : 256u);
+#else
+    // lanes holding the same digit: one vote per digit bit (MATCH.ANY is far slower than 8 VOTEs on sm_100a:
+    // ncu showed 60 % of the kernel's stalls waiting on it)
+    u32 peers = __ballot_sync(0xffffffffu, valid);
+    if (!valid) peers = ~peers;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+      const bool bit = (d >> b) & 1u;
+      const u32 bal = __ballot_sync(0xffffffffu, bit);
+      peers &= bit ? bal : ~bal;
+    }
+#endif
     u32 prev = 0;
     const int leader = __ffs(peers) - 1;
     if (valid && lane == leader) {
@@ -387,6 +400,43 @@ __global__ void __launch_bounds__(256) tile_ranges_kernel(const u64* __restrict_
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Launch order of the blend CTAs: the tiles by descending work (longest processing time first), so that the
+// last wave of CTAs is made of the shortest lists (ncu: 9-12 % of the SM cycles of both blend kernels were
+// idle in the tail with tiles launched in raster order).  One CTA: max, 256-bucket counting sort by
+// work / max; the order inside a bucket is immaterial.
+// ------------------------------------------------------------------------------------------------
+template <bool SUM>
+__global__ void __launch_bounds__(1024) tile_order_kernel(const uint2* __restrict__ pairs, u32 ntiles, u32* __restrict__ order) {
+  __shared__ u32 s_max, s_hist[256], s_base[256];
+  if (threadIdx.x == 0) s_max = 0;
+  if (threadIdx.x < 256) s_hist[threadIdx.x] = 0;
+  __syncthreads();
+  u32 mx = 0;
+  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) {
+    const uint2 p = pairs[t];
+    mx = max(mx, SUM ? p.x + p.y : p.y - p.x);
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+  if ((threadIdx.x & 31) == 0) atomicMax(&s_max, mx);
+  __syncthreads();
+  const float scale = 255.0f / (float)max(s_max, 1u);
+  auto bucket = [&](const uint2 p) { return 255u - min(255u, (u32)((float)(SUM ? p.x + p.y : p.y - p.x) * scale)); };
+  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) atomicAdd(&s_hist[bucket(pairs[t])], 1u);
+  __syncthreads();
+  if (threadIdx.x < 32) {  // exclusive scan of 256 counts by one warp, 8 per lane
+    u32 c[8], tot = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { c[j] = s_hist[threadIdx.x * 8 + j]; tot += c[j]; }
+    u32 run = warp_inclusive_scan(tot, threadIdx.x) - tot;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { s_base[threadIdx.x * 8 + j] = run; run += c[j]; }
+  }
+  __syncthreads();
+  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) order[atomicAdd(&s_base[bucket(pairs[t])], 1u)] = t;
+}
+
 __global__ void clamp_count_kernel(u32* sort_count, const u32* num_instances, u64 capacity) {
   // the sort kernels see 0 instances when the caller's buffers are too small
   *sort_count = (u64)*num_instances > capacity ? 0u : *num_instances;
@@ -440,6 +490,14 @@ void radix_pass(const u32* kin, const u32* vin, u32* kout, u32* vout, u64* kout6
 
 }  // namespace
 
+cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint32_t* order, cudaStream_t st) {
+  if (ntiles <= 0) return cudaSuccess;
+  if (sum) tile_order_kernel<true><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
+  else tile_order_kernel<false><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
+  launched();
+  return cudaGetLastError();
+}
+
 uint64_t sort_workspace_bytes(int N, uint64_t capacity) { return carve(nullptr, N, capacity).bytes; }
 
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
@@ -449,7 +507,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   if (N == 0) {
     cudaMemsetAsync(bin.num_instances, 0, sizeof(u32), st);
     cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
-    return cudaGetLastError();
+    return launch_tile_order(bin.tile_ranges, false, ntiles, bin.tile_order, st);
   }
   // A: depth order of the primitives (digits 0-3 of the 64-bit key)
   tm.begin(GABSPLAT_STAGE_DEPTH_SORT, st);
@@ -467,7 +525,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   tm.end(st);
   if (bin.capacity == 0) {
     cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
-    return cudaGetLastError();
+    return launch_tile_order(bin.tile_ranges, false, ntiles, bin.tile_order, st);
   }
   clamp_count_kernel<<<1, 1, 0, st>>>(ws.count_b, bin.num_instances, bin.capacity);
   launched();
@@ -502,8 +560,9 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   tile_ranges_kernel<<<148 * 8, 256, 0, st>>>(bin.keys, bin.num_instances, bin.capacity,
                                               reinterpret_cast<uint2*>(bin.tile_ranges));
   launched();
+  const cudaError_t eo = launch_tile_order(bin.tile_ranges, false, ntiles, bin.tile_order, st);
   tm.end(st);
-  return cudaGetLastError();
+  return eo != cudaSuccess ? eo : cudaGetLastError();
 }
 
 }  // namespace gabsplat

@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(kBlendThreads) blend_backward_kernel(Camera ca
   __shared__ float4 s_rec[kWarps][kReplay * R4];
   __shared__ uint4 s_mask[kWarps][kReplay];
   __shared__ uint32_t s_id[kWarps][kReplay];
-  const TileGeom g = tile_geom(cam);
+  const TileGeom g = tile_geom(cam, saved.order);
   const uint2 range = ranges[g.tile];
   const size_t HW = (size_t)cam.width * cam.height;
   const int cnt = (int)saved.counts[2 * g.tile + g.warp];
@@ -234,6 +234,9 @@ cudaError_t launch_blend_backward(int N, int K, bool want_abs, const Camera& cam
                                   const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const BlendState& saved,
                                   const float* dL_dimage, float* grad2d, cudaStream_t st) {
   cudaMemsetAsync(grad2d, 0, (size_t)N * grad2d_floats(K) * sizeof(float), st);
+  // launch order: half-tile pairs with the longest saved lists first
+  const cudaError_t eo = launch_tile_order(saved.counts, true, cam.tiles_x * cam.tiles_y, saved.order, st);
+  if (eo != cudaSuccess) return eo;
   return want_abs ? dispatch<true>(K, cam, proj, bin, fwd, saved, dL_dimage, grad2d, st)
                   : dispatch<false>(K, cam, proj, bin, fwd, saved, dL_dimage, grad2d, st);
 }

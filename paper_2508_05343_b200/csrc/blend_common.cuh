@@ -42,9 +42,10 @@ struct TileGeom {
   float x0, y0;         // tile origin in pixels
 };
 
-__device__ __forceinline__ TileGeom tile_geom(const Camera& cam) {
+// CTA b works on tile order[b]: the tiles by descending work (binning.cu tile_order_kernel)
+__device__ __forceinline__ TileGeom tile_geom(const Camera& cam, const uint32_t* __restrict__ order) {
   TileGeom g;
-  g.tile = blockIdx.x;
+  g.tile = (int)__ldg(order + blockIdx.x);
   g.tx = g.tile % cam.tiles_x;
   g.ty = g.tile / cam.tiles_x;
   g.warp = threadIdx.x >> 5;

@@ -13,7 +13,8 @@ namespace {
 // SAVE = also record, per warp (half tile), the primitives blended at one of its pixels and the ballots of the
 // blending lanes (common.cuh BlendState): the backward replays exactly this list.
 template <int K, bool COUNT, bool SAVE>
-__global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam, const uint2* __restrict__ ranges,
+__global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam, const uint32_t* __restrict__ order,
+                                                                      const uint2* __restrict__ ranges,
                                                                       const uint32_t* __restrict__ ids,
                                                                       const float4* __restrict__ packed,
                                                                       float* __restrict__ image, float* __restrict__ final_T,
@@ -23,7 +24,7 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
   constexpr int TL = K > 0 ? 4 * ((3 * K + 3) / 4) : 1;
   __shared__ float4 s_rec[kBatch * R4];
   __shared__ uint32_t s_cnt[8];
-  const TileGeom g = tile_geom(cam);
+  const TileGeom g = tile_geom(cam, order);
   const uint2 range = ranges[g.tile];
   const int n = (int)(range.y - range.x);
 
@@ -134,7 +135,7 @@ cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const ga
                      float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save, cudaStream_t st) {
   const int ntiles = cam.tiles_x * cam.tiles_y;
   blend_forward_kernel<K, COUNT, SAVE><<<ntiles, kBlendThreads, 0, st>>>(
-      cam, reinterpret_cast<const uint2*>(bin.tile_ranges), bin.ids, reinterpret_cast<const float4*>(proj.packed), image,
+      cam, bin.tile_order, reinterpret_cast<const uint2*>(bin.tile_ranges), bin.ids, reinterpret_cast<const float4*>(proj.packed), image,
       final_T, n_contrib, counters, save ? *save : BlendState{nullptr, nullptr, nullptr});
   launched();
   return cudaGetLastError();

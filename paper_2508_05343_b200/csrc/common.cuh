@@ -40,18 +40,21 @@ __host__ __device__ constexpr int grad2d_floats(int K) { return 4 * ((grad2d_val
 // 16x2 pixel strips, the ballot of the lanes whose pixel blended the primitive.
 struct BlendState {
   uint32_t* counts;  // [2 * tiles]
+  uint32_t* order;   // [tiles]  tiles by descending counts (launch order of the backward CTAs)
   uint32_t* ids;     // [2 * capacity]
   uint4* masks;      // [2 * capacity]
 };
 inline uint64_t blend_state_bytes(uint64_t tiles, uint64_t capacity) {
-  const uint64_t a = (2 * tiles * 4 + 255) & ~255ull, b = (2 * capacity * 4 + 255) & ~255ull;
-  return a + b + 2 * capacity * 16 + 256;
+  const uint64_t a = (2 * tiles * 4 + 255) & ~255ull, o = (tiles * 4 + 255) & ~255ull, b = (2 * capacity * 4 + 255) & ~255ull;
+  return a + o + b + 2 * capacity * 16 + 256;
 }
 inline BlendState make_blend_state(void* p, uint64_t tiles, uint64_t capacity) {
   BlendState s;
   uintptr_t q = ((uintptr_t)p + 255) & ~(uintptr_t)255;
   s.counts = reinterpret_cast<uint32_t*>(q);
   q += (2 * tiles * 4 + 255) & ~255ull;
+  s.order = reinterpret_cast<uint32_t*>(q);
+  q += (tiles * 4 + 255) & ~255ull;
   s.ids = reinterpret_cast<uint32_t*>(q);
   q += (2 * capacity * 4 + 255) & ~255ull;
   s.masks = reinterpret_cast<uint4*>(q);
@@ -132,6 +135,9 @@ cudaError_t launch_blend_backward(int N, int K, bool want_abs, const Camera& cam
                                   const float* dL_dimage, float* grad2d, cudaStream_t st);
 cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& proj,
                                        const float* grad2d, const gabsplat_grads& g, cudaStream_t st);
+
+// order[] = the tiles by descending work, work(t) = pairs[t].y - pairs[t].x (sum == false) or pairs[t].x + pairs[t].y
+cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint32_t* order, cudaStream_t st);
 
 uint64_t sort_workspace_bytes(int N, uint64_t capacity);
 

@@ -56,6 +56,7 @@ Layout carve(void* base, int N, int K, int width, int height, uint64_t capacity)
   l.bin.keys = a.take<uint64_t>(capacity);
   l.bin.ids = a.take<uint32_t>(capacity);
   l.bin.tile_ranges = a.take<uint32_t>(tiles * 2);
+  l.bin.tile_order = a.take<uint32_t>(tiles);
   l.bin.capacity = capacity;
   l.bin.num_instances = a.take<uint32_t>(4);
   l.bin.workspace_bytes = sort_workspace_bytes(N, capacity);
