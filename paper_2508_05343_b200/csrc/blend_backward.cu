@@ -71,7 +71,7 @@ constexpr int kReplay = 32;  // saved entries staged per warp and batch
 // A lane recomputes G, cos, sin and alpha of its blended pixels with the forward's own functions (bit-identical
 // alpha), recovers the transmittance in front of the primitive by division, and accumulates the gradient terms.
 template <int K, bool ABS>
-__global__ void __launch_bounds__(kBlendThreads) blend_backward_kernel(Camera cam, const uint2* __restrict__ ranges,
+__global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera cam, const uint2* __restrict__ ranges,
                                                                        BlendState saved, const float4* __restrict__ packed,
                                                                        const float* __restrict__ final_T,
                                                                        const float* __restrict__ dL_dimage,
