@@ -190,14 +190,23 @@ def stage_work(K, N, stats, tiles, passes) -> dict:
     w = {}
     w["preprocess"] = ("hbm", N * 16 + n_vis * (par - 12 + 49 + 8 * K - 4))
     w["scan"] = ("hbm", 8 * N)
-    # S2 as built: the LSD sort of the 64-bit keys is split into the 4 depth digits, sorted on
-    # the N primitives (read 4 B for the histogram, then 8 B in + 8 B out per pass), and the tile digits, sorted
-    # on the D instances (4 B histogram read; 8 B in + 8 B out per pass, the last pass 8 B in + 4 B depth gather
-    # + 12 B out); the duplication writes 8 B per instance
+    # S2 as built: the 4 depth digits are sorted on the N primitives (read 4 B for the histogram,
+    # then 8 B in + 8 B out per one-byte pass); the tile digits either in one counting pass (below) or, for
+    # images of more than 26000 tiles, in one-byte passes on the D duplicated instances
     w["depth_sort"] = ("hbm", N * (4 + 4 * 16))
-    w["duplicate"] = ("hbm", 8 * N + 20 * n_vis + 8 * D)
-    w["sort"] = ("hbm", D * (4 + (passes - 1) * 16 + 24))
-    w["ranges"] = ("hbm", 8 * D + 8 * tiles)
+    if tiles <= 26000:
+        # counting pass on the tile id: C = 592 chunks of the depth-ordered primitives;
+        # "duplicate" = chunk bounds + per-(tile, chunk) counts (rect + order of every visible primitive read,
+        # the table written); "ranges" = prefix of the table over the chunks (read + written) and of the totals
+        # over the tiles; "sort" = placement: every instance written ONCE (8 B key + 4 B id), table read
+        C = 592
+        w["duplicate"] = ("hbm", 20 * n_vis + 4 * tiles * C)
+        w["ranges"] = ("hbm", 8 * tiles * C + 24 * tiles)
+        w["sort"] = ("hbm", 12 * D + 28 * n_vis + 4 * tiles * C + 8 * tiles)
+    else:
+        w["duplicate"] = ("hbm", 8 * N + 20 * n_vis + 8 * D)
+        w["sort"] = ("hbm", D * (4 + (passes - 1) * 16 + 24))
+        w["ranges"] = ("hbm", 8 * D + 8 * tiles)
     w["preprocess_backward"] = ("hbm", n_vis * (par + (9 + 3 * K) * 4) + N * par)
     # blend: FP32-pipe lane-instructions and MUFU lane-ops
     f_fp32 = 9 * E + (4 * K + 10) * P

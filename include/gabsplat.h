@@ -109,11 +109,11 @@ typedef struct {
                                  which the forward blend launches its CTAs (longest first)            */
   uint64_t capacity;
   uint32_t* num_instances;    /* [1]  device: D = total instance count                               */
-  void* workspace;            /* device scratch, >= gabsplat_sort_workspace_bytes(N, capacity) bytes */
+  void* workspace;            /* device scratch, >= gabsplat_sort_workspace_bytes(N, capacity, W, H) bytes */
   uint64_t workspace_bytes;
 } gabsplat_binning;
 
-uint64_t gabsplat_sort_workspace_bytes(int32_t N, uint64_t capacity);
+uint64_t gabsplat_sort_workspace_bytes(int32_t N, uint64_t capacity, int32_t width, int32_t height);
 
 /* Forward outputs.  n_contrib[p] = 1-based position, within the tile list of pixel p, of the last
  * primitive that was blended at p (0 = none); its id is ids[tile_ranges[tile][0] + n_contrib - 1]. */

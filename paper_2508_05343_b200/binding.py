@@ -78,7 +78,7 @@ def lib():
         L.gabsplat_last_error.restype = C.c_char_p
         L.gabsplat_packed_floats.argtypes = [C.c_int32]
         L.gabsplat_packed_floats.restype = C.c_int32
-        L.gabsplat_sort_workspace_bytes.argtypes = [C.c_int32, C.c_uint64]
+        L.gabsplat_sort_workspace_bytes.argtypes = [C.c_int32, C.c_uint64, C.c_int32, C.c_int32]
         L.gabsplat_sort_workspace_bytes.restype = C.c_uint64
         L.gabsplat_blend_state_bytes.argtypes = [C.c_int32, C.c_int32, C.c_uint64]
         L.gabsplat_blend_state_bytes.restype = C.c_uint64
@@ -233,7 +233,7 @@ class Binning:
         self.tile_ranges = z((self.n_tiles, 2), torch.int32)
         self.tile_order = z((self.n_tiles,), torch.int32)
         self.num_instances = z((4,), torch.int32)
-        self.workspace_bytes = int(lib().gabsplat_sort_workspace_bytes(N, self.capacity))
+        self.workspace_bytes = int(lib().gabsplat_sort_workspace_bytes(N, self.capacity, cam.width, cam.height))
         self.workspace = z((self.workspace_bytes + 256,), torch.uint8)
         self.D = None  # host copy of the instance count when the call read it back
 
@@ -372,7 +372,9 @@ def gabsplat_render_host(ctx: Context, scene, cam, capacity: int, image_host: to
 
 STAGES = ("preprocess", "scan", "duplicate", "sort", "ranges", "blend_forward", "blend_backward",
           "preprocess_backward", "depth_sort")          # indexed by GABSPLAT_STAGE_*
-LAUNCH_ORDER = ("preprocess", "depth_sort", "scan", "duplicate", "sort", "ranges", "blend_forward", "blend_backward",
+# stage records of one forward + backward pass, in launch order (images of at most 26000 tiles: the tile ranges
+# are known before the instances are placed; larger images run "duplicate", "sort", "ranges")
+LAUNCH_ORDER = ("preprocess", "depth_sort", "scan", "duplicate", "ranges", "sort", "blend_forward", "blend_backward",
                 "preprocess_backward")
 
 

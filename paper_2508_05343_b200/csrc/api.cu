@@ -103,8 +103,9 @@ const char* gabsplat_last_error(const gabsplat_ctx* ctx) { return ctx ? ctx->err
 
 int32_t gabsplat_packed_floats(int32_t K) { return (K < 0 || K > kMaxK) ? 0 : packed_floats(K); }
 
-uint64_t gabsplat_sort_workspace_bytes(int32_t N, uint64_t capacity) {
-  return sort_workspace_bytes(N < 0 ? 0 : N, capacity);
+uint64_t gabsplat_sort_workspace_bytes(int32_t N, uint64_t capacity, int32_t width, int32_t height) {
+  if (width <= 0 || height <= 0) return 0;
+  return sort_workspace_bytes(N < 0 ? 0 : N, capacity, ((width + kTile - 1) / kTile) * ((height + kTile - 1) / kTile));
 }
 
 uint64_t gabsplat_blend_state_bytes(int32_t width, int32_t height, uint64_t capacity) {
@@ -136,7 +137,8 @@ int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected
   if (!proj || (N > 0 && (!proj->tiles_touched || !proj->rect || !proj->depth)))
     return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: null projected arrays");
   if (!binning_ok(bin, N)) return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: bad binning buffers");
-  if (!bin->workspace || bin->workspace_bytes < sort_workspace_bytes(N, bin->capacity))
+  if (!bin->workspace ||
+      bin->workspace_bytes < gabsplat_sort_workspace_bytes(N, bin->capacity, cam->width, cam->height))
     return fail(ctx, GABSPLAT_CAPACITY, "bin_sort: workspace too small");
   cudaStream_t st = (cudaStream_t)stream;
   cudaError_t e = launch_bin_sort(N, *proj, make_camera(*cam), *bin, ctx->timer, st);

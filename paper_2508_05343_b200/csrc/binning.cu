@@ -158,11 +158,15 @@ void device_scan(const u32* in, const u32* idx, u32* out, u32 n, u32* sums, u32*
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __restrict__ tiles_touched,
                                                          const float* __restrict__ depth, u32* __restrict__ keys,
-                                                         u32* __restrict__ vals, u32* __restrict__ count) {
+                                                         u32* __restrict__ vals, u32* __restrict__ count,
+                                                         u32* __restrict__ n_vis) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i == 0) *count = (u32)N;
+  const bool vis = i < N && tiles_touched[i] != 0;
+  const u32 bal = __ballot_sync(0xffffffffu, vis);
+  if ((threadIdx.x & 31) == 0 && bal) atomicAdd(n_vis, (u32)__popc(bal));  // *n_vis zeroed by the launcher
   if (i >= N) return;
-  keys[i] = tiles_touched[i] ? __float_as_uint(depth[i]) : 0xffffffffu;
+  keys[i] = vis ? __float_as_uint(depth[i]) : 0xffffffffu;
   vals[i] = (u32)i;
 }
 
@@ -442,6 +446,235 @@ __global__ void clamp_count_kernel(u32* sort_count, const u32* num_instances, u6
   *sort_count = (u64)*num_instances > capacity ? 0u : *num_instances;
 }
 
+// ------------------------------------------------------------------------------------------------
+// B': the tile digit in ONE stable counting-sort pass.  The depth-ordered primitive sequence is cut into
+// kChunks chunks of equal estimated cost; because a primitive covers a tile at most once, the per-(chunk, tile)
+// histogram is simply the number of the chunk's primitives whose rectangle contains the tile:
+//   tile_count_kernel   table[tile][chunk] = that number                       (shared-memory histogram per CTA)
+//   tile_scan_kernel    table[tile][.] -> exclusive prefix over the chunks; totals[tile]
+//   tile_ranges_scan    exclusive prefix of the totals over the tiles -> tile_ranges (+ launch order of the blend)
+//   tile_place_kernel   every CTA re-walks its chunk in depth order, kStep primitives at a time, and writes
+//                       (tile | depth, id) at  ranges[tile].x + table[tile][chunk] + (rank inside the chunk)
+// The rank inside a step is the number of lower-ranked primitives of the step that cover the same tile: the
+// step's primitives OR their bit into mask[tile] (shared memory), then every instance counts the bits below
+// its own.  Result: exactly the order of a stable sort by tile of the depth-ordered instance sequence, i.e.
+// what the one-byte LSD passes on the tile digits produce (kept below as the path for images with more tiles
+// than fit in shared memory), at a fraction of the traffic: the instances are written once and never read.
+// ------------------------------------------------------------------------------------------------
+constexpr int kChunks = 592;       // 4 per SM
+constexpr int kPlaceThreads = 256;
+constexpr int kStep = 32;          // primitives per step (one mask bit each)
+constexpr u32 kCostPerPrimitive = 16;  // chunk cost = instances + 16 * primitives
+constexpr int kMaxTilesCounting = 26000;  // 2 * 4 B * tiles (and 4 B * (tiles_x+1)(tiles_y+1)) of shared memory must fit in 227 KB
+
+// boundary c of the chunking: the number of ranks r < n_vis with offsets[r] + kCost * (r + 1) <= c * total / kChunks
+__global__ void __launch_bounds__(256) chunk_bounds_kernel(const u32* __restrict__ offsets, const u32* __restrict__ n_vis_p,
+                                                           u32* __restrict__ bounds) {
+  __shared__ u32 s_lo, s_hi, s_cnt[8];
+  const u32 n_vis = *n_vis_p;
+  const u32 c = blockIdx.x;
+  if (n_vis == 0) { if (threadIdx.x == 0) bounds[c] = 0; return; }
+  const u64 total = (u64)__ldg(offsets + n_vis - 1) + (u64)kCostPerPrimitive * n_vis;
+  const u64 target = total * c / kChunks;
+  if (threadIdx.x == 0) { s_lo = 0; s_hi = n_vis; }
+  __syncthreads();
+  while (true) {
+    const u32 lo = s_lo, hi = s_hi;
+    if (lo >= hi) break;
+    const u32 step = (hi - lo + 255) / 256;
+    const u32 p = lo + threadIdx.x * step;
+    const bool le = p < hi && (u64)__ldg(offsets + p) + (u64)kCostPerPrimitive * (p + 1) <= target;
+    const u32 bal = __ballot_sync(0xffffffffu, le);
+    if ((threadIdx.x & 31) == 0) s_cnt[threadIdx.x >> 5] = __popc(bal);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      u32 k = 0;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) k += s_cnt[w];
+      if (k == 0) s_hi = lo;
+      else { s_lo = lo + (k - 1) * step + 1; s_hi = min(hi, lo + k * step); }
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) bounds[c] = s_lo;
+}
+
+// record r of the depth-ordered visible primitives: (id, bits(depth), x0 | y0 << 16, x1 | y1 << 16): what the two
+// walks below read, coalesced, instead of chasing order -> rect / depth per primitive
+__global__ void __launch_bounds__(256) visible_records_kernel(const u32* __restrict__ order, const int4* __restrict__ rect,
+                                                              const float* __restrict__ depth, const u32* __restrict__ n_vis_p,
+                                                              uint4* __restrict__ recs) {
+  const u32 n_vis = *n_vis_p;
+  for (u32 r = blockIdx.x * blockDim.x + threadIdx.x; r < n_vis; r += gridDim.x * blockDim.x) {
+    const u32 id = __ldg(order + r);
+    const int4 rc = __ldg(rect + id);
+    recs[r] = make_uint4(id, __float_as_uint(__ldg(depth + id)), (u32)rc.x | ((u32)rc.y << 16), (u32)rc.z | ((u32)rc.w << 16));
+  }
+}
+
+// walks the tiles of one rectangle with the lanes of a warp: f(tile) for tile number lane, lane + 32, ...
+template <typename F>
+__device__ __forceinline__ void for_rect_tiles(u32 xy0, u32 xy1, int tiles_x, int lane, F f) {
+  const int x0 = (int)(xy0 & 0xffffu), y0 = (int)(xy0 >> 16);
+  const int w = (int)(xy1 & 0xffffu) - x0, n = w * ((int)(xy1 >> 16) - y0);
+  // floor(a / w) for 0 <= a <= 32 without an integer division: (a + 0.5) / w is at least 0.5 / w away from every
+  // integer, far more than the error of the approximate quotient
+  const float fw = (float)w;
+  int row = __float2int_rz(__fdividef((float)lane + 0.5f, fw)), col = lane - row * w;
+  const int drow = __float2int_rz(__fdividef(32.5f, fw)), dcol = 32 - drow * w;
+  for (int e = lane; e < n; e += 32) {
+    f((u32)((y0 + row) * tiles_x + x0 + col));
+    row += drow; col += dcol;
+    if (col >= w) { col -= w; ++row; }
+  }
+}
+
+// table[tile][chunk] = number of the chunk's primitives whose rectangle contains the tile, by a 2D difference
+// array in shared memory: four corner updates per primitive, then prefix sums along x and along y.
+__global__ void __launch_bounds__(kPlaceThreads) tile_count_kernel(int tiles_x, int tiles_y, const uint4* __restrict__ recs,
+                                                                   const u32* __restrict__ bounds, u32* __restrict__ table) {
+  extern __shared__ int s_d[];  // [(tiles_y + 1)][(tiles_x + 1)]
+  const int sx = tiles_x + 1, sy = tiles_y + 1;
+  for (int t = threadIdx.x; t < sx * sy; t += kPlaceThreads) s_d[t] = 0;
+  __syncthreads();
+  const u32 b0 = bounds[blockIdx.x], b1 = bounds[blockIdx.x + 1];
+  for (u32 r = b0 + threadIdx.x; r < b1; r += kPlaceThreads) {
+    const uint4 rc = __ldg(recs + r);
+    const int x0 = (int)(rc.z & 0xffffu), y0 = (int)(rc.z >> 16), x1 = (int)(rc.w & 0xffffu), y1 = (int)(rc.w >> 16);
+    atomicAdd(&s_d[y0 * sx + x0], 1);
+    atomicAdd(&s_d[y0 * sx + x1], -1);
+    atomicAdd(&s_d[y1 * sx + x0], -1);
+    atomicAdd(&s_d[y1 * sx + x1], 1);
+  }
+  __syncthreads();
+  for (int y = threadIdx.x; y < sy; y += kPlaceThreads) {
+    int run = 0;
+    for (int x = 0; x < sx; ++x) { run += s_d[y * sx + x]; s_d[y * sx + x] = run; }
+  }
+  __syncthreads();
+  for (int x = threadIdx.x; x < sx; x += kPlaceThreads) {
+    int run = 0;
+    for (int y = 0; y < sy; ++y) { run += s_d[y * sx + x]; s_d[y * sx + x] = run; }
+  }
+  __syncthreads();
+  for (int t = threadIdx.x; t < tiles_x * tiles_y; t += kPlaceThreads) {
+    const int y = t / tiles_x, x = t - y * tiles_x;
+    table[(size_t)t * kChunks + blockIdx.x] = (u32)s_d[y * sx + x];
+  }
+}
+
+// a warp per tile: exclusive prefix of table[tile][0..kChunks) in place, total to totals[tile]
+__global__ void __launch_bounds__(256) tile_scan_kernel(int ntiles, u32* __restrict__ table, u32* __restrict__ totals) {
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (t >= ntiles) return;
+  u32* row = table + (size_t)t * kChunks;
+  u32 carry = 0;
+  for (int c0 = 0; c0 < kChunks; c0 += 32) {
+    const int c = c0 + lane;
+    const u32 v = c < kChunks ? row[c] : 0u;
+    const u32 inc = warp_inclusive_scan(v, lane);
+    if (c < kChunks) row[c] = carry + inc - v;
+    carry += __shfl_sync(0xffffffffu, inc, 31);
+  }
+  if (lane == 0) totals[t] = carry;
+}
+
+// one CTA: tile_ranges[t] = [start, start + totals[t]) by an exclusive prefix over the tiles ((0,0) for an empty
+// tile and for every tile when the instances do not fit the caller's buffers)
+__global__ void __launch_bounds__(1024) tile_ranges_scan_kernel(int ntiles, const u32* __restrict__ totals,
+                                                               const u32* __restrict__ num_instances, u64 capacity,
+                                                               uint2* __restrict__ ranges) {
+  __shared__ u32 s_warp[32], s_carry;
+  const bool fits = (u64)*num_instances <= capacity;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (threadIdx.x == 0) s_carry = 0;
+  __syncthreads();
+  for (int base = 0; base < ntiles; base += 1024) {
+    const int t = base + threadIdx.x;
+    const u32 v = t < ntiles ? totals[t] : 0u;
+    const u32 inc = warp_inclusive_scan(v, lane);
+    if (lane == 31) s_warp[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+      const u32 x = s_warp[lane];
+      const u32 xi = warp_inclusive_scan(x, lane);
+      s_warp[lane] = xi - x;
+    }
+    __syncthreads();
+    const u32 start = s_carry + s_warp[w] + inc - v;
+    if (t < ntiles) ranges[t] = (fits && v) ? make_uint2(start, start + v) : make_uint2(0u, 0u);
+    __syncthreads();
+    if (threadIdx.x == 1023) s_carry = start + v;
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(kPlaceThreads) tile_place_kernel(int ntiles, int tiles_x, const uint4* __restrict__ recs,
+                                                                   const u32* __restrict__ bounds, const u32* __restrict__ table,
+                                                                   const uint2* __restrict__ ranges,
+                                                                   const u32* __restrict__ num_instances, u64 capacity,
+                                                                   u32* __restrict__ ids) {
+  extern __shared__ u32 s_mem[];
+  u32* s_pos = s_mem;            // [ntiles] next free slot of the tile for this chunk
+  u32* s_mask = s_mem + ntiles;  // [ntiles] bit w set: primitive w of the current step covers the tile
+  __shared__ uint4 s_rec[2][kStep];
+  if ((u64)*num_instances > capacity) return;
+  for (int t = threadIdx.x; t < ntiles; t += kPlaceThreads) {
+    s_pos[t] = ranges[t].x + table[(size_t)t * kChunks + blockIdx.x];
+    s_mask[t] = 0;
+  }
+  const u32 b0 = bounds[blockIdx.x], b1 = bounds[blockIdx.x + 1];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int kWarps = kPlaceThreads / 32;
+  if (threadIdx.x < kStep && b0 + threadIdx.x < b1) s_rec[0][threadIdx.x] = __ldg(recs + b0 + threadIdx.x);
+  int buf = 0;
+  for (u32 r0 = b0; r0 < b1; r0 += kStep, buf ^= 1) {
+    // prefetch the next step's records while this one runs
+    uint4 next = make_uint4(0u, 0u, 0u, 0u);
+    const bool pre = threadIdx.x < kStep && r0 + kStep + threadIdx.x < b1;
+    if (pre) next = __ldg(recs + r0 + kStep + threadIdx.x);
+    __syncthreads();  // s_rec[buf] visible; first step: s_pos / s_mask initialised; phase 3 of the previous step done
+    const int m = (int)min((u32)kStep, b1 - r0);
+    // phase 1: every primitive of the step marks the tiles it covers (a warp per primitive, lanes over tiles)
+    for (int w = warp; w < m; w += kWarps) {
+      const uint4 rc = s_rec[buf][w];
+      for_rect_tiles(rc.z, rc.w, tiles_x, lane, [&](u32 t) { atomicOr(&s_mask[t], 1u << w); });
+    }
+    __syncthreads();
+    // phase 2: slot = tile cursor + number of lower-ranked primitives of the step on the same tile
+    for (int w = warp; w < m; w += kWarps) {
+      const uint4 rc = s_rec[buf][w];
+      const u32 below = (1u << w) - 1u;
+      for_rect_tiles(rc.z, rc.w, tiles_x, lane, [&](u32 t) {
+        ids[s_pos[t] + __popc(s_mask[t] & below)] = rc.x;
+      });
+    }
+    __syncthreads();
+    // phase 3: the highest-ranked primitive of the step on a tile advances the cursor and clears the mask
+    for (int w = warp; w < m; w += kWarps) {
+      const uint4 rc = s_rec[buf][w];
+      for_rect_tiles(rc.z, rc.w, tiles_x, lane, [&](u32 t) {
+        const u32 mk = s_mask[t];
+        if ((mk >> w) == 1u) { s_pos[t] += __popc(mk); s_mask[t] = 0; }
+      });
+    }
+    if (pre) s_rec[buf ^ 1][threadIdx.x] = next;
+  }
+}
+
+// keys[i] = (tile << 32) | bits(depth[ids[i]]) for the sorted instances: a warp per tile, coalesced.  (The blend
+// kernels never read the keys; they are the inspectable statement of the order.)
+__global__ void __launch_bounds__(256) tile_keys_kernel(int ntiles, const uint2* __restrict__ ranges, const u32* __restrict__ ids,
+                                                        const float* __restrict__ depth, u64* __restrict__ keys) {
+  const int lane = threadIdx.x & 31;
+  const int t = blockIdx.x * 8 + (threadIdx.x >> 5);
+  if (t >= ntiles) return;
+  const uint2 rg = ranges[t];
+  for (u32 i = rg.x + lane; i < rg.y; i += 32)
+    keys[i] = ((u64)(u32)t << 32) | (u64)__float_as_uint(__ldg(depth + ids[i]));
+}
+
 inline u64 align_up(u64 x, u64 a) { return (x + a - 1) / a * a; }
 inline u32 sort_blocks(u64 n) { return (u32)((n + kSortTile - 1) / kSortTile); }
 
@@ -452,12 +685,19 @@ struct Workspace {
   u32* table;       // [256][nblocks]
   u32* pk[2];       // stage A key ping-pong [N]
   u32* pv[2];       // stage A value ping-pong [N]; pv[0] ends up holding the depth order
-  u32* ik;          // stage B alternate keys [capacity]
-  u32* iv;          // stage B alternate values [capacity]
+  u32* ik;          // stage B (radix path) alternate keys [capacity]
+  u32* iv;          // stage B (radix path) alternate values [capacity]
+  u32* n_vis;       // [1] number of visible primitives
+  u32* bounds;      // [kChunks + 1] chunk boundaries (ranks in depth order)
+  u32* totals;      // [ntiles] instances per tile
+  uint4* recs;      // [N] records of the visible primitives in depth order
+  u32* chunk_table; // [ntiles][kChunks] per-(tile, chunk) counts, then exclusive prefixes over the chunks
   u64 bytes;
 };
 
-Workspace carve(void* base, int N, u64 capacity) {
+inline bool counting_path(int ntiles) { return ntiles <= kMaxTilesCounting; }
+
+Workspace carve(void* base, int N, u64 capacity, int ntiles) {
   const u64 nb = (u64)(sort_blocks(capacity) > sort_blocks((u64)N) ? sort_blocks(capacity) : sort_blocks((u64)N));
   const u64 table_n = (u64)256 * (nb ? nb : 1);
   const u64 sums_n = (u64)scan_blocks((u32)(table_n > (u64)N ? table_n : (u64)N)) + 16;
@@ -470,8 +710,19 @@ Workspace carve(void* base, int N, u64 capacity) {
   w.count_b = (u32*)take(16);
   w.table = (u32*)take(table_n * 4);
   for (int i = 0; i < 2; ++i) { w.pk[i] = (u32*)take((u64)N * 4); w.pv[i] = (u32*)take((u64)N * 4); }
-  w.ik = (u32*)take(capacity * 4);
-  w.iv = (u32*)take(capacity * 4);
+  w.n_vis = (u32*)take(16);
+  w.bounds = (u32*)take((kChunks + 1) * 4);
+  if (counting_path(ntiles)) {
+    w.ik = w.iv = nullptr;
+    w.totals = (u32*)take((u64)ntiles * 4);
+    w.recs = (uint4*)take((u64)N * 16);
+    w.chunk_table = (u32*)take((u64)ntiles * kChunks * 4);
+  } else {
+    w.totals = w.chunk_table = nullptr;
+    w.recs = nullptr;
+    w.ik = (u32*)take(capacity * 4);
+    w.iv = (u32*)take(capacity * 4);
+  }
   w.bytes = off;
   return w;
 }
@@ -498,12 +749,12 @@ cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint3
   return cudaGetLastError();
 }
 
-uint64_t sort_workspace_bytes(int N, uint64_t capacity) { return carve(nullptr, N, capacity).bytes; }
+uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles) { return carve(nullptr, N, capacity, ntiles).bytes; }
 
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
                             StageTimer& tm, cudaStream_t st) {
-  const Workspace ws = carve(bin.workspace, N, bin.capacity);
   const int ntiles = cam.tiles_x * cam.tiles_y;
+  const Workspace ws = carve(bin.workspace, N, bin.capacity, ntiles);
   if (N == 0) {
     cudaMemsetAsync(bin.num_instances, 0, sizeof(u32), st);
     cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
@@ -511,7 +762,9 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   }
   // A: depth order of the primitives (digits 0-3 of the 64-bit key)
   tm.begin(GABSPLAT_STAGE_DEPTH_SORT, st);
-  depth_keys_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, proj.tiles_touched, proj.depth, ws.pk[0], ws.pv[0], ws.count_a);
+  cudaMemsetAsync(ws.n_vis, 0, sizeof(u32), st);
+  depth_keys_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, proj.tiles_touched, proj.depth, ws.pk[0], ws.pv[0], ws.count_a,
+                                                     ws.n_vis);
   launched();
   const u32 nba = sort_blocks((u64)N);
   for (int p = 0; p < 4; ++p)
@@ -527,6 +780,39 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
     cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
     return launch_tile_order(bin.tile_ranges, false, ntiles, bin.tile_order, st);
   }
+  if (counting_path(ntiles)) {
+    // B': one counting-sort pass on the whole tile id (see the kernels above)
+    const size_t smem_count = (size_t)(cam.tiles_x + 1) * (cam.tiles_y + 1) * sizeof(int);
+    const size_t smem_place = 2 * (size_t)ntiles * sizeof(u32);
+    if (smem_place > 48 * 1024 || smem_count > 48 * 1024) {
+      cudaFuncSetAttribute(tile_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_count);
+      cudaFuncSetAttribute(tile_place_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_place);
+    }
+    const int4* rect = reinterpret_cast<const int4*>(proj.rect);
+    uint2* ranges = reinterpret_cast<uint2*>(bin.tile_ranges);
+    tm.begin(GABSPLAT_STAGE_DUPLICATE, st);
+    chunk_bounds_kernel<<<kChunks + 1, 256, 0, st>>>(bin.offsets, ws.n_vis, ws.bounds);
+    visible_records_kernel<<<148 * 4, 256, 0, st>>>(order, rect, proj.depth, ws.n_vis, ws.recs);
+    tile_count_kernel<<<kChunks, kPlaceThreads, smem_count, st>>>(cam.tiles_x, cam.tiles_y, ws.recs, ws.bounds, ws.chunk_table);
+    launched(3);
+    tm.end(st);
+    tm.begin(GABSPLAT_STAGE_RANGES, st);
+    tile_scan_kernel<<<(ntiles + 7) / 8, 256, 0, st>>>(ntiles, ws.chunk_table, ws.totals);
+    tile_ranges_scan_kernel<<<1, 1024, 0, st>>>(ntiles, ws.totals, bin.num_instances, bin.capacity, ranges);
+    launched(2);
+    const cudaError_t eo = launch_tile_order(bin.tile_ranges, false, ntiles, bin.tile_order, st);
+    tm.end(st);
+    if (eo != cudaSuccess) return eo;
+    tm.begin(GABSPLAT_STAGE_SORT, st);
+    tile_place_kernel<<<kChunks, kPlaceThreads, smem_place, st>>>(ntiles, cam.tiles_x, ws.recs, ws.bounds, ws.chunk_table,
+                                                                 ranges, bin.num_instances, bin.capacity, bin.ids);
+    tile_keys_kernel<<<(ntiles + 7) / 8, 256, 0, st>>>(ntiles, ranges, bin.ids, proj.depth, bin.keys);
+    launched(2);
+    tm.end(st);
+    return cudaGetLastError();
+  }
+  // images with more tiles than the counting pass can histogram in shared memory: one-byte LSD passes on the
+  // tile id over the duplicated instances
   clamp_count_kernel<<<1, 1, 0, st>>>(ws.count_b, bin.num_instances, bin.capacity);
   launched();
   // stage B passes: one per byte of the tile id.  The last pass reads the alternate buffers and writes

@@ -139,6 +139,6 @@ cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& ca
 // order[] = the tiles by descending work, work(t) = pairs[t].y - pairs[t].x (sum == false) or pairs[t].x + pairs[t].y
 cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint32_t* order, cudaStream_t st);
 
-uint64_t sort_workspace_bytes(int N, uint64_t capacity);
+uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles);
 
 }  // namespace gabsplat

@@ -59,7 +59,7 @@ Layout carve(void* base, int N, int K, int width, int height, uint64_t capacity)
   l.bin.tile_order = a.take<uint32_t>(tiles);
   l.bin.capacity = capacity;
   l.bin.num_instances = a.take<uint32_t>(4);
-  l.bin.workspace_bytes = sort_workspace_bytes(N, capacity);
+  l.bin.workspace_bytes = sort_workspace_bytes(N, capacity, (int)tiles);
   l.bin.workspace = a.take<char>(l.bin.workspace_bytes);
   l.fwd.image = a.take<float>(3 * hw);
   l.fwd.final_T = a.take<float>(hw);

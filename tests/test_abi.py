@@ -37,12 +37,12 @@ def test_every_declared_symbol_is_exported(lib):
 def test_size_queries(lib):
     lib.gabsplat_packed_floats.restype = C.c_int32
     lib.gabsplat_sort_workspace_bytes.restype = C.c_uint64
-    lib.gabsplat_sort_workspace_bytes.argtypes = [C.c_int32, C.c_uint64]
+    lib.gabsplat_sort_workspace_bytes.argtypes = [C.c_int32, C.c_uint64, C.c_int32, C.c_int32]
     lib.gabsplat_grad_workspace_bytes.restype = C.c_uint64
     assert [lib.gabsplat_packed_floats(k) for k in (0, 1, 2, 4, 8)] == [12, 16, 20, 24, 36]
     assert lib.gabsplat_packed_floats(9) == 0 and lib.gabsplat_packed_floats(-1) == 0
-    a = lib.gabsplat_sort_workspace_bytes(1000, 10_000)
-    b = lib.gabsplat_sort_workspace_bytes(1000, 20_000)
+    a = lib.gabsplat_sort_workspace_bytes(1000, 10_000, 8000, 4000)
+    b = lib.gabsplat_sort_workspace_bytes(1000, 20_000, 8000, 4000)
     assert b > a >= 10_000 * 8
     assert lib.gabsplat_grad_workspace_bytes(10, 4) >= 10 * 24 * 4
     assert lib.gabsplat_grad_workspace_bytes(10, 9) == 0

@@ -218,3 +218,21 @@ def test_pair_counters_and_stage_timing():
     # the envelope test is a threshold on exp(): equal up to borderline pairs
     assert abs(int(cnt[..., 1].sum()) - int(oc[..., 1].sum())) <= 1e-3 * oc[..., 1].sum()
     assert np.all(cnt[..., 3] <= cnt[..., 1]) and np.all(cnt[..., 2] <= cnt[..., 3])
+
+
+def test_many_tiles_radix_path():
+    """An image with more tiles (28 000) than the counting pass can histogram in shared memory takes the
+    one-byte LSD passes on the tile digits over the duplicated instances: same bit-exact keys, ids, ranges."""
+    orc = _oracle()
+    scene = scenes.make_scene("tiny", N=3000)
+    base = scenes.make_cameras("tiny")[0]
+    cam = scenes.make_camera(3200, 2240, 3750.0, base.world_to_cam, base.bg)
+    assert cam.tiles_x * cam.tiles_y > 26000
+    g = _gpu(scene, cam)
+    check_projection(g, orc.project(scene, cam), scene.K)
+    check_binning(g, orc.bin_sort(scene, cam))
+    px = np.stack([np.arange(100, 3100, 30), np.arange(100, 2100, 20)], axis=1).astype(np.int32)
+    r = orc.render_pixels(scene, cam, px)
+    dec = np.minimum(r["margin"][:, 0], r["margin"][:, 1]) > DELTA
+    err = np.abs(g["image"][:, px[:, 1], px[:, 0]].T.astype(np.float64) - r["colour"]).max(axis=1)
+    assert err[dec].max() <= IMG_TOL
