@@ -512,17 +512,17 @@ __global__ void __launch_bounds__(256) visible_records_kernel(const u32* __restr
   }
 }
 
-// walks the tiles of one rectangle with the lanes of a warp: f(tile) for tile number lane, lane + 32, ...
+// walks the tiles of one rectangle: f(tile) for tile number start, start + stride, ... (row-major in the rectangle)
 template <typename F>
-__device__ __forceinline__ void for_rect_tiles(u32 xy0, u32 xy1, int tiles_x, int lane, F f) {
+__device__ __forceinline__ void for_rect_tiles(u32 xy0, u32 xy1, int tiles_x, int start, int stride, F f) {
   const int x0 = (int)(xy0 & 0xffffu), y0 = (int)(xy0 >> 16);
   const int w = (int)(xy1 & 0xffffu) - x0, n = w * ((int)(xy1 >> 16) - y0);
-  // floor(a / w) for 0 <= a <= 32 without an integer division: (a + 0.5) / w is at least 0.5 / w away from every
-  // integer, far more than the error of the approximate quotient
+  // floor(a / w) for 0 <= a <= 256 without an integer division: (a + 0.5) / w is at least 0.5 / w away from
+  // every integer, far more than the error of the approximate quotient
   const float fw = (float)w;
-  int row = __float2int_rz(__fdividef((float)lane + 0.5f, fw)), col = lane - row * w;
-  const int drow = __float2int_rz(__fdividef(32.5f, fw)), dcol = 32 - drow * w;
-  for (int e = lane; e < n; e += 32) {
+  int row = __float2int_rz(__fdividef((float)start + 0.5f, fw)), col = start - row * w;
+  const int drow = __float2int_rz(__fdividef((float)stride + 0.5f, fw)), dcol = stride - drow * w;
+  for (int e = start; e < n; e += stride) {
     f((u32)((y0 + row) * tiles_x + x0 + col));
     row += drow; col += dcol;
     if (col >= w) { col -= w; ++row; }
@@ -610,6 +610,20 @@ __global__ void __launch_bounds__(1024) tile_ranges_scan_kernel(int ntiles, cons
   }
 }
 
+constexpr int kFlat = 8;  // instances a thread keeps in registers during a step
+constexpr u32 kStepInstances = kFlat * kPlaceThreads;
+
+__device__ __forceinline__ u32 rect_tiles(const uint4& rc) {
+  return ((rc.w & 0xffffu) - (rc.z & 0xffffu)) * ((rc.w >> 16) - (rc.z >> 16));
+}
+
+// A step is the longest run of consecutive primitives (at most kStep) whose rectangles hold at most
+// kStepInstances tiles together, and at least one primitive.
+//  * one primitive: its tiles are all different, so the whole CTA appends its id to their lists directly;
+//  * several: instance e of the step belongs to thread e % 256, which locates it once (binary search in the
+//    prefix of the tile counts, then row / column inside the rectangle) and keeps (tile | w << 16) in registers
+//    through the three phases: mark (OR bit w into mask[tile]), place (cursor + bits below w), close (the
+//    highest bit advances the cursor and clears the mask).
 __global__ void __launch_bounds__(kPlaceThreads) tile_place_kernel(int ntiles, int tiles_x, const uint4* __restrict__ recs,
                                                                    const u32* __restrict__ bounds, const u32* __restrict__ table,
                                                                    const uint2* __restrict__ ranges,
@@ -619,6 +633,8 @@ __global__ void __launch_bounds__(kPlaceThreads) tile_place_kernel(int ntiles, i
   u32* s_pos = s_mem;            // [ntiles] next free slot of the tile for this chunk
   u32* s_mask = s_mem + ntiles;  // [ntiles] bit w set: primitive w of the current step covers the tile
   __shared__ uint4 s_rec[2][kStep];
+  __shared__ u32 s_pre[2][kStep + 1];  // exclusive prefix of the tile counts of the step's primitives
+  __shared__ int s_m[2];               // primitives in the step
   if ((u64)*num_instances > capacity) return;
   for (int t = threadIdx.x; t < ntiles; t += kPlaceThreads) {
     s_pos[t] = ranges[t].x + table[(size_t)t * kChunks + blockIdx.x];
@@ -626,40 +642,67 @@ __global__ void __launch_bounds__(kPlaceThreads) tile_place_kernel(int ntiles, i
   }
   const u32 b0 = bounds[blockIdx.x], b1 = bounds[blockIdx.x + 1];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  constexpr int kWarps = kPlaceThreads / 32;
-  if (threadIdx.x < kStep && b0 + threadIdx.x < b1) s_rec[0][threadIdx.x] = __ldg(recs + b0 + threadIdx.x);
+  // warp 0 stages the step that starts at rank r
+  auto stage = [&](int buf, u32 r) {
+    const bool have = r + lane < b1;
+    const uint4 rc = have ? __ldg(recs + r + lane) : make_uint4(0u, 0u, 0u, 0u);
+    const u32 n = have ? rect_tiles(rc) : 0u;
+    const u32 inc = warp_inclusive_scan(n, lane);
+    const int m = max(1, __popc(__ballot_sync(0xffffffffu, have && inc <= kStepInstances)));
+    s_rec[buf][lane] = rc;
+    s_pre[buf][lane + 1] = lane < m ? inc : 0xffffffffu;  // the binary search never steps past primitive m - 1
+    if (lane == 0) { s_pre[buf][0] = 0; s_m[buf] = m; }
+  };
+  if (warp == 0 && b0 < b1) stage(0, b0);
   int buf = 0;
-  for (u32 r0 = b0; r0 < b1; r0 += kStep, buf ^= 1) {
-    // prefetch the next step's records while this one runs
-    uint4 next = make_uint4(0u, 0u, 0u, 0u);
-    const bool pre = threadIdx.x < kStep && r0 + kStep + threadIdx.x < b1;
-    if (pre) next = __ldg(recs + r0 + kStep + threadIdx.x);
-    __syncthreads();  // s_rec[buf] visible; first step: s_pos / s_mask initialised; phase 3 of the previous step done
-    const int m = (int)min((u32)kStep, b1 - r0);
-    // phase 1: every primitive of the step marks the tiles it covers (a warp per primitive, lanes over tiles)
-    for (int w = warp; w < m; w += kWarps) {
-      const uint4 rc = s_rec[buf][w];
-      for_rect_tiles(rc.z, rc.w, tiles_x, lane, [&](u32 t) { atomicOr(&s_mask[t], 1u << w); });
+  u32 r0 = b0;
+  while (r0 < b1) {
+    __syncthreads();  // stage(buf) visible; first step: s_pos / s_mask initialised; previous step finished
+    const int m = s_m[buf];
+    const u32 total = s_pre[buf][m];
+    if (warp == 0 && r0 + m < b1) stage(buf ^ 1, r0 + m);  // overlaps the global load with this step
+    if (m == 1) {
+      const uint4 rc = s_rec[buf][0];
+      for_rect_tiles(rc.z, rc.w, tiles_x, (int)threadIdx.x, kPlaceThreads, [&](u32 t) { ids[s_pos[t]++] = rc.x; });
+    } else {
+      u32 tw[kFlat];
+#pragma unroll
+      for (int i = 0; i < kFlat; ++i) {
+        const u32 e = (u32)i * kPlaceThreads + threadIdx.x;
+        tw[i] = 0xffffffffu;
+        if (e < total) {
+          u32 w = 0;
+#pragma unroll
+          for (int b = kStep / 2; b > 0; b >>= 1) if (s_pre[buf][w + b] <= e) w += b;
+          const uint4 rc = s_rec[buf][w];
+          const u32 x0 = rc.z & 0xffffu, y0 = rc.z >> 16, wd = (rc.w & 0xffffu) - x0;
+          const u32 local = e - s_pre[buf][w];
+          const u32 row = (u32)__float2int_rz(__fdividef((float)local + 0.5f, (float)wd));  // local < 2048: exact
+          const u32 t = (y0 + row) * (u32)tiles_x + x0 + (local - row * wd);
+          tw[i] = t | (w << 16);
+          atomicOr(&s_mask[t], 1u << w);
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < kFlat; ++i) {
+        if (tw[i] != 0xffffffffu) {
+          const u32 t = tw[i] & 0xffffu, w = tw[i] >> 16;
+          ids[s_pos[t] + __popc(s_mask[t] & ((1u << w) - 1u))] = s_rec[buf][w].x;
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < kFlat; ++i) {
+        if (tw[i] != 0xffffffffu) {
+          const u32 t = tw[i] & 0xffffu, w = tw[i] >> 16;
+          const u32 mk = s_mask[t];
+          if ((mk >> w) == 1u) { s_pos[t] += __popc(mk); s_mask[t] = 0; }
+        }
+      }
     }
-    __syncthreads();
-    // phase 2: slot = tile cursor + number of lower-ranked primitives of the step on the same tile
-    for (int w = warp; w < m; w += kWarps) {
-      const uint4 rc = s_rec[buf][w];
-      const u32 below = (1u << w) - 1u;
-      for_rect_tiles(rc.z, rc.w, tiles_x, lane, [&](u32 t) {
-        ids[s_pos[t] + __popc(s_mask[t] & below)] = rc.x;
-      });
-    }
-    __syncthreads();
-    // phase 3: the highest-ranked primitive of the step on a tile advances the cursor and clears the mask
-    for (int w = warp; w < m; w += kWarps) {
-      const uint4 rc = s_rec[buf][w];
-      for_rect_tiles(rc.z, rc.w, tiles_x, lane, [&](u32 t) {
-        const u32 mk = s_mask[t];
-        if ((mk >> w) == 1u) { s_pos[t] += __popc(mk); s_mask[t] = 0; }
-      });
-    }
-    if (pre) s_rec[buf ^ 1][threadIdx.x] = next;
+    r0 += m;
+    buf ^= 1;
   }
 }
 
@@ -667,12 +710,18 @@ __global__ void __launch_bounds__(kPlaceThreads) tile_place_kernel(int ntiles, i
 // kernels never read the keys; they are the inspectable statement of the order.)
 __global__ void __launch_bounds__(256) tile_keys_kernel(int ntiles, const uint2* __restrict__ ranges, const u32* __restrict__ ids,
                                                         const float* __restrict__ depth, u64* __restrict__ keys) {
-  const int lane = threadIdx.x & 31;
-  const int t = blockIdx.x * 8 + (threadIdx.x >> 5);
+  // half a CTA (128 threads) per tile, two instances per thread and iteration in flight
+  const int t = blockIdx.x * 2 + (threadIdx.x >> 7);
   if (t >= ntiles) return;
   const uint2 rg = ranges[t];
-  for (u32 i = rg.x + lane; i < rg.y; i += 32)
-    keys[i] = ((u64)(u32)t << 32) | (u64)__float_as_uint(__ldg(depth + ids[i]));
+  const u64 hi = (u64)(u32)t << 32;
+  for (u32 i = rg.x + (threadIdx.x & 127); i < rg.y; i += 256) {
+    const u32 j = i + 128;
+    const u32 a = ids[i], b = j < rg.y ? ids[j] : 0u;
+    const u32 da = __float_as_uint(__ldg(depth + a)), db = __float_as_uint(__ldg(depth + b));
+    keys[i] = hi | (u64)da;
+    if (j < rg.y) keys[j] = hi | (u64)db;
+  }
 }
 
 inline u64 align_up(u64 x, u64 a) { return (x + a - 1) / a * a; }
@@ -806,7 +855,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
     tm.begin(GABSPLAT_STAGE_SORT, st);
     tile_place_kernel<<<kChunks, kPlaceThreads, smem_place, st>>>(ntiles, cam.tiles_x, ws.recs, ws.bounds, ws.chunk_table,
                                                                  ranges, bin.num_instances, bin.capacity, bin.ids);
-    tile_keys_kernel<<<(ntiles + 7) / 8, 256, 0, st>>>(ntiles, ranges, bin.ids, proj.depth, bin.keys);
+    tile_keys_kernel<<<(ntiles + 1) / 2, 256, 0, st>>>(ntiles, ranges, bin.ids, proj.depth, bin.keys);
     launched(2);
     tm.end(st);
     return cudaGetLastError();
