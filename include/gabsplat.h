@@ -102,7 +102,9 @@ int32_t gabsplat_packed_floats(int32_t K);
 /* Tile binning state.  capacity = number of (key,id) slots the caller allocated. */
 typedef struct {
   uint32_t* offsets;          /* [N]  inclusive prefix sum of tiles_touched taken in depth order     */
-  uint64_t* keys;             /* [capacity]  sorted on return: (tile_id << 32) | bits(depth)         */
+  uint64_t* keys;             /* [capacity]  sorted on return: (tile_id << 32) | bits(depth).  No later stage
+                                 reads the keys: for images of at most 26000 tiles the pointer may be NULL
+                                 and the keys are then not materialised                                */
   uint32_t* ids;              /* [capacity]  primitive index of each instance, same order            */
   uint32_t* tile_ranges;      /* [tiles_y*tiles_x][2]  [start,end) into keys/ids; (0,0) if empty     */
   uint32_t* tile_order;       /* [tiles_y*tiles_x]  the tiles by descending list length: the order in

@@ -223,12 +223,12 @@ class Projected:
 class Binning:
     """Device buffers of gabsplat_binning for N primitives and `capacity` instances."""
 
-    def __init__(self, N: int, cam, capacity: int, device):
+    def __init__(self, N: int, cam, capacity: int, device, with_keys: bool = True):
         z = lambda shape, dt: torch.zeros(shape, dtype=dt, device=device)
         self.N, self.capacity = N, int(capacity)
         self.n_tiles = ((cam.width + TILE - 1) // TILE) * ((cam.height + TILE - 1) // TILE)
         self.offsets = z((max(N, 1),), torch.int32)
-        self.keys = z((max(self.capacity, 1),), torch.int64)
+        self.keys = z((max(self.capacity, 1),), torch.int64) if with_keys else None
         self.ids = z((max(self.capacity, 1),), torch.int32)
         self.tile_ranges = z((self.n_tiles, 2), torch.int32)
         self.tile_order = z((self.n_tiles,), torch.int32)
@@ -239,7 +239,8 @@ class Binning:
 
     def struct(self) -> _Binning:
         b = _Binning()
-        b.offsets, b.keys, b.ids = self.offsets.data_ptr(), self.keys.data_ptr(), self.ids.data_ptr()
+        b.offsets, b.ids = self.offsets.data_ptr(), self.ids.data_ptr()
+        b.keys = self.keys.data_ptr() if self.keys is not None else None
         b.tile_ranges = self.tile_ranges.data_ptr()
         b.tile_order = self.tile_order.data_ptr()
         b.capacity = self.capacity

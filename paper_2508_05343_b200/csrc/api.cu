@@ -57,7 +57,7 @@ bool projected_ok(const gabsplat_projected* p, int N, int K) {
 bool binning_ok(const gabsplat_binning* b, int N) {
   if (!b || !b->tile_ranges || !b->tile_order || !b->num_instances) return false;
   if (N > 0 && !b->offsets) return false;
-  if (b->capacity > 0 && (!b->keys || !b->ids)) return false;
+  if (b->capacity > 0 && !b->ids) return false;
   if (b->capacity >= (1ull << 32)) return false;
   return true;
 }
@@ -137,6 +137,8 @@ int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected
   if (!proj || (N > 0 && (!proj->tiles_touched || !proj->rect || !proj->depth)))
     return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: null projected arrays");
   if (!binning_ok(bin, N)) return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: bad binning buffers");
+  if (bin->capacity > 0 && !bin->keys && !keys_optional(((cam->width + kTile - 1) / kTile) * ((cam->height + kTile - 1) / kTile)))
+    return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: images of more than 26000 tiles need the key buffer");
   if (!bin->workspace ||
       bin->workspace_bytes < gabsplat_sort_workspace_bytes(N, bin->capacity, cam->width, cam->height))
     return fail(ctx, GABSPLAT_CAPACITY, "bin_sort: workspace too small");

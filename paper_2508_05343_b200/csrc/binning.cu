@@ -798,6 +798,8 @@ cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint3
   return cudaGetLastError();
 }
 
+bool keys_optional(int ntiles) { return counting_path(ntiles); }
+
 uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles) { return carve(nullptr, N, capacity, ntiles).bytes; }
 
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
@@ -855,8 +857,11 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
     tm.begin(GABSPLAT_STAGE_SORT, st);
     tile_place_kernel<<<kChunks, kPlaceThreads, smem_place, st>>>(ntiles, cam.tiles_x, ws.recs, ws.bounds, ws.chunk_table,
                                                                  ranges, bin.num_instances, bin.capacity, bin.ids);
-    tile_keys_kernel<<<(ntiles + 1) / 2, 256, 0, st>>>(ntiles, ranges, bin.ids, proj.depth, bin.keys);
-    launched(2);
+    launched();
+    if (bin.keys) {
+      tile_keys_kernel<<<(ntiles + 1) / 2, 256, 0, st>>>(ntiles, ranges, bin.ids, proj.depth, bin.keys);
+      launched();
+    }
     tm.end(st);
     return cudaGetLastError();
   }

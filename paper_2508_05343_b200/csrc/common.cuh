@@ -140,5 +140,6 @@ cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& ca
 cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint32_t* order, cudaStream_t st);
 
 uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles);
+bool keys_optional(int ntiles);  // true when the binning never reads gabsplat_binning.keys itself
 
 }  // namespace gabsplat
