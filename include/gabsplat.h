@@ -49,6 +49,7 @@ extern "C" {
 
 #define GABSPLAT_MAX_K 8
 #define GABSPLAT_TILE 16       /* tiles are 16x16 pixels */
+#define GABSPLAT_CHUNK 1024    /* primitives per CTA of the projection kernel */
 #define GABSPLAT_SH_COEFFS 16  /* storage stride of SH coefficients per primitive (degree 3) */
 
 typedef struct gabsplat_ctx gabsplat_ctx;
@@ -94,6 +95,8 @@ typedef struct {
   uint32_t* tiles_touched; /* [N]     number of tiles in the primitive's rectangle                */
   int32_t* rect;           /* [N][4]  xmin,ymin,xmax,ymax in tiles, max exclusive                  */
   float* packed;           /* [N][gabsplat_packed_floats(K)]  gather record, 16-byte aligned       */
+  uint32_t* chunk_visible; /* [ceil(N / GABSPLAT_CHUNK)]  visible primitives per chunk of consecutive
+                              primitives (what the binning needs to compact them in index order)   */
 } gabsplat_projected;
 
 /* Number of floats per primitive in gabsplat_projected.packed (a multiple of 4). */
@@ -101,7 +104,8 @@ int32_t gabsplat_packed_floats(int32_t K);
 
 /* Tile binning state.  capacity = number of (key,id) slots the caller allocated. */
 typedef struct {
-  uint32_t* offsets;          /* [N]  inclusive prefix sum of tiles_touched taken in depth order     */
+  uint32_t* offsets;          /* [N]  inclusive prefix sum of tiles_touched over the visible primitives in
+                                 depth order (one entry per visible primitive; the rest is not written) */
   uint64_t* keys;             /* [capacity]  sorted on return: (tile_id << 32) | bits(depth).  No later stage
                                  reads the keys: for images of at most 26000 tiles the pointer may be NULL
                                  and the keys are then not materialised                                */

@@ -18,6 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgabsplat.so")
 
 OK, INVALID_ARG, CAPACITY, CUDA_ERROR, UNSUPPORTED = 0, 1, 2, 3, 4
+CHUNK = 1024   # GABSPLAT_CHUNK
 TILE = 16
 
 
@@ -40,7 +41,7 @@ class _Scene(C.Structure):
 
 class _Projected(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("mean2d", "depth", "radius", "conic_opacity", "rgb", "rgb_clamped",
-                                          "freq2d", "tiles_touched", "rect", "packed")]
+                                          "freq2d", "tiles_touched", "rect", "packed", "chunk_visible")]
 
 
 class _Binning(C.Structure):
@@ -211,6 +212,7 @@ class Projected:
         self.tiles_touched = z((N,), torch.int32)  # uint32 on the device; torch has no uint32 arithmetic
         self.rect = z((N, 4), torch.int32)
         self.packed = z((N, lib().gabsplat_packed_floats(K)), torch.float32)
+        self.chunk_visible = z(((N + CHUNK - 1) // CHUNK + 1,), torch.int32)
 
     def struct(self) -> _Projected:
         p = _Projected()

@@ -51,7 +51,7 @@ bool projected_ok(const gabsplat_projected* p, int N, int K) {
   if (!p) return false;
   if (N == 0) return true;
   return p->mean2d && p->depth && p->radius && p->conic_opacity && p->rgb && p->rgb_clamped &&
-         (K == 0 || p->freq2d) && p->tiles_touched && p->rect && p->packed;
+         (K == 0 || p->freq2d) && p->tiles_touched && p->rect && p->packed && p->chunk_visible;
 }
 
 bool binning_ok(const gabsplat_binning* b, int N) {
@@ -134,7 +134,7 @@ int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected
                           gabsplat_binning* bin, uint64_t* num_instances_host, void* stream) {
   if (!ctx) return GABSPLAT_INVALID_ARG;
   if (N < 0 || !camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: bad N or camera");
-  if (!proj || (N > 0 && (!proj->tiles_touched || !proj->rect || !proj->depth)))
+  if (!proj || (N > 0 && (!proj->tiles_touched || !proj->rect || !proj->depth || !proj->chunk_visible)))
     return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: null projected arrays");
   if (!binning_ok(bin, N)) return fail(ctx, GABSPLAT_INVALID_ARG, "bin_sort: bad binning buffers");
   if (bin->capacity > 0 && !bin->keys && !keys_optional(((cam->width + kTile - 1) / kTile) * ((cam->height + kTile - 1) / kTile)))

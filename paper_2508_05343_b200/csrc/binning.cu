@@ -3,8 +3,8 @@
 // ties by primitive index -- exactly what a stable LSD radix sort of the keys on one-byte digits gives -- plus
 // the [start,end) range of every tile.  The LSD passes are split around the duplication step so that the four
 // depth digits are sorted on the N primitives, not on the D >> N instances:
-//   A   keys = bits(depth) (culled primitives: 0xffffffff), 4 stable one-byte passes over the N primitives
-//       -> `order`: primitives front to back, ties by index
+//   A   (bits(depth), index) of the n_vis visible primitives, compacted in index order; 4 stable one-byte
+//       passes over them -> `order`: visible primitives front to back, ties by index
 //   K2  inclusive prefix sum of tiles_touched taken in that order               -> offsets, D
 //   K3  one (tile,id) per (primitive, tile of its rectangle), emitted in depth order, row-major over the rectangle
 //   B   ceil(tile_bits / 8) stable one-byte passes on the tile id over the D instances; the last pass writes the
@@ -83,7 +83,8 @@ __device__ __forceinline__ void scan_load(const u32* __restrict__ in, const u32*
 
 template <bool GATHER>
 __global__ void __launch_bounds__(kScanThreads) scan_block_sums(const u32* __restrict__ in, const u32* __restrict__ idx, u32 n,
-                                                                 u32* __restrict__ sums) {
+                                                                 const u32* __restrict__ n_dev, u32* __restrict__ sums) {
+  if (n_dev) n = min(n, *n_dev);  // the element count lives on the device (n is its host-side bound)
   const u32 base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
   u32 v[kScanItems];
   scan_load<GATHER>(in, idx, base, n, v);
@@ -111,7 +112,9 @@ __global__ void __launch_bounds__(kScanThreads) scan_of_sums(u32* __restrict__ s
 
 template <bool INCLUSIVE, bool GATHER>
 __global__ void __launch_bounds__(kScanThreads) scan_apply(const u32* __restrict__ in, const u32* __restrict__ idx, u32 n,
-                                                            const u32* __restrict__ sums, u32* __restrict__ out) {
+                                                            const u32* __restrict__ n_dev, const u32* __restrict__ sums,
+                                                            u32* __restrict__ out) {
+  if (n_dev) n = min(n, *n_dev);
   const u32 base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
   u32 v[kScanItems];
   scan_load<GATHER>(in, idx, base, n, v);
@@ -140,34 +143,65 @@ inline u32 scan_blocks(u32 n) { return (n + kScanTile - 1) / kScanTile; }
 
 // sums must hold scan_blocks(n) u32.  in/out/idx must be 16-byte aligned.  in == out is allowed (not with GATHER).
 template <bool INCLUSIVE, bool GATHER>
-void device_scan(const u32* in, const u32* idx, u32* out, u32 n, u32* sums, u32* total_out, cudaStream_t st) {
+void device_scan(const u32* in, const u32* idx, u32* out, u32 n, const u32* n_dev, u32* sums, u32* total_out, cudaStream_t st) {
   const u32 nb = scan_blocks(n);
   if (nb == 0) {
     scan_of_sums<<<1, kScanThreads, 0, st>>>(sums, 0, total_out);
     launched();
     return;
   }
-  scan_block_sums<GATHER><<<nb, kScanThreads, 0, st>>>(in, idx, n, sums);
+  scan_block_sums<GATHER><<<nb, kScanThreads, 0, st>>>(in, idx, n, n_dev, sums);
   scan_of_sums<<<1, kScanThreads, 0, st>>>(sums, nb, total_out);
-  scan_apply<INCLUSIVE, GATHER><<<nb, kScanThreads, 0, st>>>(in, idx, n, sums, out);
+  scan_apply<INCLUSIVE, GATHER><<<nb, kScanThreads, 0, st>>>(in, idx, n, n_dev, sums, out);
   launched(3);
 }
 
 // ------------------------------------------------------------------------------------------------
 // A: depth keys of the primitives.  Culled primitives (tiles_touched == 0) sort to the end.
 // ------------------------------------------------------------------------------------------------
+// One CTA per GABSPLAT_CHUNK consecutive primitives (the chunks of the projection kernel, which left the
+// number of visible primitives of every chunk in chunk_visible): the visible primitives are compacted in
+// index order -- (bits(depth), index) pairs at [sum of the earlier chunks' counts, ...) -- so that the depth
+// passes sort n_vis pairs, not N.
 __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __restrict__ tiles_touched,
-                                                         const float* __restrict__ depth, u32* __restrict__ keys,
-                                                         u32* __restrict__ vals, u32* __restrict__ count,
-                                                         u32* __restrict__ n_vis) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i == 0) *count = (u32)N;
-  const bool vis = i < N && tiles_touched[i] != 0;
-  const u32 bal = __ballot_sync(0xffffffffu, vis);
-  if ((threadIdx.x & 31) == 0 && bal) atomicAdd(n_vis, (u32)__popc(bal));  // *n_vis zeroed by the launcher
-  if (i >= N) return;
-  keys[i] = vis ? __float_as_uint(depth[i]) : 0xffffffffu;
-  vals[i] = (u32)i;
+                                                         const float* __restrict__ depth, const u32* __restrict__ chunk_visible,
+                                                         u32* __restrict__ keys, u32* __restrict__ vals, u32* __restrict__ n_vis) {
+  __shared__ u32 s_part[8], s_off;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  u32 acc = 0;
+  for (u32 c = threadIdx.x; c < blockIdx.x; c += 256) acc += __ldg(chunk_visible + c);
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+  if (lane == 0) s_part[w] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    u32 t = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) t += s_part[j];
+    s_off = t;
+  }
+  __syncthreads();
+  u32 run = s_off;
+  const int base = blockIdx.x * GABSPLAT_CHUNK;
+#pragma unroll 1
+  for (int r = 0; r < GABSPLAT_CHUNK / 256; ++r) {
+    const int i = base + r * 256 + (int)threadIdx.x;
+    const bool vis = i < N && tiles_touched[i] != 0;
+    const u32 bal = __ballot_sync(0xffffffffu, vis);
+    __syncthreads();  // s_part of the previous round consumed
+    if (lane == 0) s_part[w] = (u32)__popc(bal);
+    __syncthreads();
+    u32 before = 0, total = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { const u32 c = s_part[j]; before += j < w ? c : 0u; total += c; }
+    if (vis) {
+      const u32 pos = run + before + (u32)__popc(bal & ((1u << lane) - 1u));
+      keys[pos] = __float_as_uint(depth[i]);
+      vals[pos] = (u32)i;
+    }
+    run += total;
+  }
+  if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *n_vis = run;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -181,7 +215,7 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __res
 constexpr int kDupThreads = 256;
 constexpr int kDupChunk = 2048;
 
-__global__ void __launch_bounds__(kDupThreads) duplicate_kernel(int N, int tiles_x, const u32* __restrict__ order,
+__global__ void __launch_bounds__(kDupThreads) duplicate_kernel(const u32* __restrict__ n_vis_p, int tiles_x, const u32* __restrict__ order,
                                                                const u32* __restrict__ offsets,
                                                                const int4* __restrict__ rect,
                                                                const u32* __restrict__ num_instances, u64 capacity,
@@ -191,6 +225,7 @@ __global__ void __launch_bounds__(kDupThreads) duplicate_kernel(int N, int tiles
   __shared__ u32 s_lo, s_hi, s_cnt[kDupThreads / 32];
   const u32 D = *num_instances;
   if ((u64)D > capacity) return;
+  const int N = (int)*n_vis_p;  // ranks of the depth order (visible primitives only)
   const u32 g0 = blockIdx.x * kDupChunk;
   if (g0 >= D) return;
   const u32 n = min((u32)kDupChunk, D - g0);
@@ -258,6 +293,8 @@ constexpr int kSortItems = 16;
 constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 pairs per block
 constexpr int kSortWarps = kSortThreads / 32;
 
+// BLOCK_MAJOR: table[block][digit] (read back by sort_scatter<., true>); else table[digit][block] (scanned in place)
+template <bool BLOCK_MAJOR>
 __global__ void __launch_bounds__(kSortThreads) sort_histogram(const u32* __restrict__ keys, const u32* __restrict__ count,
                                                               u32* __restrict__ table, u32 nblocks, int shift) {
   __shared__ u32 hist[kSortWarps][256];
@@ -287,10 +324,14 @@ __global__ void __launch_bounds__(kSortThreads) sort_histogram(const u32* __rest
   u32 tot = 0;
 #pragma unroll
   for (int j = 0; j < kSortWarps; ++j) tot += hist[j][threadIdx.x];
-  table[threadIdx.x * nblocks + blockIdx.x] = tot;
+  if (BLOCK_MAJOR) table[blockIdx.x * 256u + threadIdx.x] = tot;
+  else table[threadIdx.x * nblocks + blockIdx.x] = tot;
 }
 
-template <bool FINAL>
+// SELF: the table holds raw per-block counts, block-major; every CTA sums the columns of the blocks before it
+// and the digit totals itself (a few dozen blocks when the pairs are the visible primitives): two launches per
+// pass instead of five.  Otherwise the table holds the exclusive scan of the digit-major counts.
+template <bool FINAL, bool SELF>
 __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restrict__ kin, const u32* __restrict__ vin,
                                                             u32* __restrict__ kout, u32* __restrict__ vout,
                                                             u64* __restrict__ kout64, const u32* __restrict__ gather,
@@ -365,7 +406,19 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
     u32 total;
     const u32 ex = block_exclusive_scan(tot, &total);
     local_base[d] = ex;
-    global_base[d] = table[(u32)d * nblocks + blockIdx.x];
+    if (SELF) {
+      const u32 nact = (D + kSortTile - 1) / kSortTile;
+      u32 below = 0, all = 0;
+      for (u32 bb = 0; bb < nact; ++bb) {
+        const u32 c = __ldg(table + bb * 256u + (u32)d);
+        all += c;
+        below += bb < blockIdx.x ? c : 0u;
+      }
+      u32 gtotal;
+      global_base[d] = block_exclusive_scan(all, &gtotal) + below;
+    } else {
+      global_base[d] = table[(u32)d * nblocks + blockIdx.x];
+    }
   }
   __syncthreads();
 #pragma unroll
@@ -778,14 +831,22 @@ Workspace carve(void* base, int N, u64 capacity, int ntiles) {
 
 void radix_pass(const u32* kin, const u32* vin, u32* kout, u32* vout, u64* kout64, const u32* gather, const u32* count,
                 u32 nblocks, int shift, const Workspace& ws, cudaStream_t st) {
-  sort_histogram<<<nblocks, kSortThreads, 0, st>>>(kin, count, ws.table, nblocks, shift);
+  sort_histogram<false><<<nblocks, kSortThreads, 0, st>>>(kin, count, ws.table, nblocks, shift);
   launched();
-  device_scan<false, false>(ws.table, nullptr, ws.table, 256u * nblocks, ws.scan_sums, nullptr, st);
+  device_scan<false, false>(ws.table, nullptr, ws.table, 256u * nblocks, nullptr, ws.scan_sums, nullptr, st);
   if (kout64)
-    sort_scatter<true><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift);
+    sort_scatter<true, false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift);
   else
-    sort_scatter<false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift);
+    sort_scatter<false, false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift);
   launched();
+}
+
+// a pass over the visible primitives: histogram + self-scanning scatter
+void radix_pass_small(const u32* kin, const u32* vin, u32* kout, u32* vout, const u32* count, u32 nblocks, int shift,
+                      const Workspace& ws, cudaStream_t st) {
+  sort_histogram<true><<<nblocks, kSortThreads, 0, st>>>(kin, count, ws.table, nblocks, shift);
+  sort_scatter<false, true><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, nullptr, nullptr, count, ws.table, nblocks, shift);
+  launched(2);
 }
 
 }  // namespace
@@ -813,19 +874,17 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   }
   // A: depth order of the primitives (digits 0-3 of the 64-bit key)
   tm.begin(GABSPLAT_STAGE_DEPTH_SORT, st);
-  cudaMemsetAsync(ws.n_vis, 0, sizeof(u32), st);
-  depth_keys_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, proj.tiles_touched, proj.depth, ws.pk[0], ws.pv[0], ws.count_a,
-                                                     ws.n_vis);
+  depth_keys_kernel<<<(N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK, 256, 0, st>>>(N, proj.tiles_touched, proj.depth,
+                                                                            proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis);
   launched();
   const u32 nba = sort_blocks((u64)N);
   for (int p = 0; p < 4; ++p)
-    radix_pass(ws.pk[p & 1], ws.pv[p & 1], ws.pk[(p & 1) ^ 1], ws.pv[(p & 1) ^ 1], nullptr, nullptr, ws.count_a, nba, 8 * p,
-               ws, st);
+    radix_pass_small(ws.pk[p & 1], ws.pv[p & 1], ws.pk[(p & 1) ^ 1], ws.pv[(p & 1) ^ 1], ws.n_vis, nba, 8 * p, ws, st);
   const u32* order = ws.pv[0];
   tm.end(st);
-  // K2
+  // K2 (over the n_vis ranks)
   tm.begin(GABSPLAT_STAGE_SCAN, st);
-  device_scan<true, true>(proj.tiles_touched, order, bin.offsets, (u32)N, ws.scan_sums, bin.num_instances, st);
+  device_scan<true, true>(proj.tiles_touched, order, bin.offsets, (u32)N, ws.n_vis, ws.scan_sums, bin.num_instances, st);
   tm.end(st);
   if (bin.capacity == 0) {
     cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
@@ -880,7 +939,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   // K3
   tm.begin(GABSPLAT_STAGE_DUPLICATE, st);
   duplicate_kernel<<<(u32)((bin.capacity + kDupChunk - 1) / kDupChunk), kDupThreads, 0, st>>>(
-      N, cam.tiles_x, order, bin.offsets, reinterpret_cast<const int4*>(proj.rect), bin.num_instances, bin.capacity,
+      ws.n_vis, cam.tiles_x, order, bin.offsets, reinterpret_cast<const int4*>(proj.rect), bin.num_instances, bin.capacity,
       kbuf[cur], vbuf[cur]);
   launched();
   tm.end(st);

@@ -246,7 +246,7 @@ __device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camer
 //     10-20 % of the primitives are visible: without the compaction the value track runs with 3-6 live lanes
 //     per warp (ncu: 4.2-9.9 thread instructions per warp instruction, profiles/r01_*).
 constexpr int kPreThreads = 256;
-constexpr int kPreChunk = 1024;
+constexpr int kPreChunk = GABSPLAT_CHUNK;
 
 __global__ void __launch_bounds__(kPreThreads, 2) preprocess_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
   __shared__ int s_i[kPreChunk];
@@ -290,6 +290,7 @@ __global__ void __launch_bounds__(kPreThreads, 2) preprocess_kernel(gabsplat_sce
   }
   __syncthreads();
   const int n = s_n;
+  if (threadIdx.x == 0) out.chunk_visible[blockIdx.x] = (uint32_t)n;
   for (int j = threadIdx.x; j < n; j += kPreThreads) {
     Index ix;
     ix.visible = true;

@@ -52,7 +52,7 @@ def test_struct_sizes_match_header():
     from paper_2508_05343_b200 import binding as gb
     assert C.sizeof(gb._Camera) == 4 * (2 + 4 + 12 + 1 + 3)
     assert C.sizeof(gb._Scene) == 16 + 7 * 8
-    assert C.sizeof(gb._Projected) == 10 * 8
+    assert C.sizeof(gb._Projected) == 11 * 8
     assert C.sizeof(gb._Binning) == 9 * 8
     assert C.sizeof(gb._FwdOut) == 5 * 8
     assert C.sizeof(gb._Grads) == 9 * 8

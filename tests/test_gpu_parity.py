@@ -116,7 +116,8 @@ def test_zero_weights_equals_gaussian():
     assert np.array_equal(g4["image"], g0["image"])
     assert np.array_equal(g4["n_contrib"], g0["n_contrib"])
     for n in ("d_means", "d_scales", "d_rotations", "d_opacities", "d_sh"):
-        assert np.allclose(g4[n], g0[n], rtol=1e-5, atol=1e-7 * np.abs(g0[n]).max())
+        # equal up to the order of the fp32 atomic accumulation (different launch orders, different kernels)
+        assert np.allclose(g4[n], g0[n], rtol=1e-4, atol=2e-6 * np.abs(g0[n]).max())
     assert np.all(g4["d_freqs"] == 0)
     check_forward(g4, orc.render_forward(s4, cam))
 
