@@ -237,3 +237,13 @@ def test_many_tiles_radix_path():
     dec = np.minimum(r["margin"][:, 0], r["margin"][:, 1]) > DELTA
     err = np.abs(g["image"][:, px[:, 1], px[:, 0]].T.astype(np.float64) - r["colour"]).max(axis=1)
     assert err[dec].max() <= IMG_TOL
+
+
+def test_banded_placement(monkeypatch):
+    """Large instance counts are placed band by band of tile rows (binning.cu tile_place_kernel); forced here on
+    a small case: 3 bands must give the same bit-exact lists as one."""
+    orc = _oracle()
+    scene, cam = _ragged_case("unbounded", 40000, 203, 131, 180.0)
+    monkeypatch.setenv("GABSPLAT_PLACE_BANDS", "3")
+    g = _gpu(scene, cam)
+    check_binning(g, orc.bin_sort(scene, cam))
