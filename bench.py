@@ -169,6 +169,26 @@ def run_reference(args, name, scene, cams, rank) -> dict:
     }
 
 
+def view_of_step(step: int, rank: int, n_views: int) -> int:
+    """Replicas only: rank r renders view (step + r) mod n_views of the replicated scene."""
+    return (step + rank) % n_views
+
+
+def job_value(pixels_per_view: int, world: int, ms_per_step_max_over_ranks: float) -> float:
+    """Whole-job Mpix/s: every rank renders one view per step; the step time is the max over ranks."""
+    return world * pixels_per_view / 1e6 / (ms_per_step_max_over_ranks / 1e3)
+
+
+def max_over_ranks(ms: float, dist, device=None) -> float:
+    """The slowest rank's time (all_reduce MAX); identity without a process group."""
+    if dist is None:
+        return ms
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def workload_config(args, name, scene, cam) -> dict:
     return {"workload": "%s: N=%d primitives, K=%d, SH degree 3, %dx%d, 8 seeded views, %s" % (
                 name, scene.N, scene.K, cam.width, cam.height,
@@ -211,8 +231,11 @@ def stage_work(K, N, stats, tiles, passes) -> dict:
     # blend: FP32-pipe lane-instructions and MUFU lane-ops
     f_fp32 = 9 * E + (4 * K + 10) * P
     f_mufu = (1 + K) * P
-    b_fp32 = 9 * Eb + (4 * K + 10) * Pb + (10 * K + 45) * B
-    b_mufu = (1 + K) * Pb + K * B
+    # backward as built: the forward has recorded which (pixel, primitive) pairs were blended, so the method's
+    # work is per BLENDED pair only: envelope (9) + Gabor recompute (4K+10, 1+K MUFU) + gradient terms
+    # (10K+45, K MUFU for the sines).  (A backward that re-walks the lists would add 9 * walked + (4K+10) * Pb.)
+    b_fp32 = (9 + 4 * K + 10 + 10 * K + 45) * B
+    b_mufu = (1 + 2 * K) * B
     w["blend_forward"] = ("alu", f_fp32, f_mufu)
     w["blend_backward"] = ("alu", b_fp32, b_mufu)
     return w
@@ -282,7 +305,7 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     fwd = gb.FwdOut(cams[0], dev, capacity if backward else None)
     grads = gb.Grads(N, K, dev, with_mean2d=False) if backward else None
 
-    my_view = lambda i: (i + rank) % V
+    my_view = lambda i: view_of_step(i, rank, V)
 
     def step(i, do_backward, bins=bins):
         v = my_view(i)
@@ -317,10 +340,7 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
         launches = gb.gabsplat_kernel_launches() - l0
         recs = gb.gabsplat_timing_read(ctx) if with_stage_timing else []
         gb.gabsplat_timing_enable(ctx, False)
-        if dist is not None:
-            t = torch.tensor([ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(ms, dist, dev)
         return ms, launches, recs
 
     sampler = ClockSampler(local_rank)
@@ -336,7 +356,7 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     keys_total_ms, _, _ = timed(args.steps, backward, False, bins_k)
     del bins_k
     ms_per_step = total_ms / args.steps
-    value = world * H * W / 1e6 / (ms_per_step / 1e3)
+    value = job_value(H * W, world, ms_per_step)
 
     # per-stage means over the timed region; the views of the timed steps weight the numerators
     stage_ms = {}
