@@ -152,7 +152,9 @@ typedef struct {
   float* d_mean2d_abs; /* [N][2] optional: sum over pixels of |per-pixel dL/dmu2D| (AbsGS variant, :224) */
 } gabsplat_grads;
 
-/* Bytes of device scratch gabsplat_render_backward needs for N primitives with K components. */
+/* Bytes of device scratch gabsplat_render_backward needs for N primitives with K components.  The scratch must
+ * be ALL ZERO when gabsplat_render_backward is called; the call returns it all zero again (it clears exactly the
+ * records it wrote), so the caller zeroes it once, after allocating it. */
 uint64_t gabsplat_grad_workspace_bytes(int32_t N, int32_t K);
 
 /* S1.  Writes every array of `out` for all N primitives. */
@@ -176,7 +178,9 @@ int32_t gabsplat_render_forward(gabsplat_ctx* ctx, const gabsplat_scene* scene, 
                                 const gabsplat_projected* proj, const gabsplat_binning* bin, gabsplat_fwd_out* out,
                                 void* stream);
 
-/* S4a + S4b.  dL_dimage is [3][H][W] on the device. */
+/* S4a + S4b.  dL_dimage is [3][H][W] on the device.  `bin` must be exactly what gabsplat_bin_sort returned for this
+ * view, workspace included (the projection backward walks the list of visible primitives it holds); `fwd` must
+ * carry the blend state. */
 int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
                                  const gabsplat_projected* proj, const gabsplat_binning* bin,
                                  const gabsplat_fwd_out* fwd, const float* dL_dimage, gabsplat_grads* grads,
@@ -187,7 +191,8 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
  * device->host copies of the image / gradients inside the call; synchronises.  All pointers in
  * `scene_host` and `grads_host` are HOST pointers here; grads_host may be NULL when dL_dimage_host is.
  * Device memory is taken from `device_arena` (device pointer, arena_bytes long; query the size with
- * gabsplat_host_arena_bytes). */
+ * gabsplat_host_arena_bytes; zero it once after allocating it -- it holds the gradient scratch, see
+ * gabsplat_grad_workspace_bytes). */
 uint64_t gabsplat_host_arena_bytes(int32_t N, int32_t K, int32_t width, int32_t height, uint64_t capacity);
 int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* scene_host, const gabsplat_camera* cam,
                              uint64_t capacity, float* image_host, const float* dL_dimage_host,

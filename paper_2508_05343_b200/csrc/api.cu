@@ -9,6 +9,8 @@
 struct gabsplat_ctx {
   int device;
   uint64_t* pinned_count;  // 8-byte pinned readback slot for D
+  cudaStream_t side;       // side stream: the zeroing of the gradient arrays overlaps the blend backward
+  cudaEvent_t ev_fork, ev_join;
   gabsplat::StageTimer timer;
   char error[256];
 };
@@ -87,6 +89,13 @@ int32_t gabsplat_create(gabsplat_ctx** out, int32_t device) {
     delete ctx;
     return GABSPLAT_CUDA;
   }
+  ctx->side = nullptr; ctx->ev_fork = ctx->ev_join = nullptr;
+  if (cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+    gabsplat_destroy(ctx);
+    return GABSPLAT_CUDA;
+  }
   cudaDeviceSynchronize();
   *out = ctx;
   return GABSPLAT_OK;
@@ -95,6 +104,9 @@ int32_t gabsplat_create(gabsplat_ctx** out, int32_t device) {
 void gabsplat_destroy(gabsplat_ctx* ctx) {
   if (!ctx) return;
   if (ctx->pinned_count) cudaFreeHost(ctx->pinned_count);
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+  if (ctx->side) cudaStreamDestroy(ctx->side);
   ctx->timer.destroy();
   delete ctx;
 }
@@ -192,6 +204,9 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
   if (!fwd || !fwd->final_T || !fwd->n_contrib || !dL_dimage) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: null forward state");
   if (!fwd->blend_state)
     return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: the forward was run without blend_state (inference mode)");
+  if (scene->N > 0 && (!bin->workspace ||
+                       bin->workspace_bytes < gabsplat_sort_workspace_bytes(scene->N, bin->capacity, cam->width, cam->height)))
+    return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: bin.workspace must still hold what gabsplat_bin_sort left in it");
   if (!grads) return fail(ctx, GABSPLAT_INVALID_ARG, "render_backward: null grads");
   if (scene->N > 0 && (!grads->d_means || !grads->d_scales || !grads->d_rotations || !grads->d_opacities || !grads->d_sh ||
                        (scene->K > 0 && (!grads->d_freqs || !grads->d_weights))))
@@ -205,13 +220,22 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
   if (fwd->blend_state_bytes < blend_state_bytes(tiles, bin->capacity))
     return fail(ctx, GABSPLAT_CAPACITY, "render_backward: blend_state too small");
   const BlendState saved = make_blend_state(fwd->blend_state, tiles, bin->capacity);
+  // fork: zero the gradient arrays on the side stream (store-only, HBM bound) while the blend backward
+  // (ALU bound) runs on the caller's stream; join before the projection backward writes the visible rows
+  cudaError_t e = cudaEventRecord(ctx->ev_fork, st);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0);
+  if (e == cudaSuccess) e = launch_grad_zero(*scene, *grads, ctx->side);
+  if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_join, ctx->side);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "render_backward (gradient zeroing)");
   ctx->timer.begin(GABSPLAT_STAGE_BLEND_BACKWARD, st);
-  cudaError_t e = launch_blend_backward(scene->N, scene->K, grads->d_mean2d_abs != nullptr, c, *proj, *bin, *fwd, saved,
+  e = launch_blend_backward(scene->N, scene->K, grads->d_mean2d_abs != nullptr, c, *proj, *bin, *fwd, saved,
                                         dL_dimage, grad2d, st);
   ctx->timer.end(st);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "render_backward (blend)");
+  e = cudaStreamWaitEvent(st, ctx->ev_join, 0);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "render_backward (join)");
   ctx->timer.begin(GABSPLAT_STAGE_PREPROCESS_BACKWARD, st);
-  e = launch_preprocess_backward(*scene, c, *proj, grad2d, *grads, st);
+  e = launch_preprocess_backward(*scene, c, *proj, *bin, grad2d, *grads, st);
   ctx->timer.end(st);
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "render_backward (projection)");
 }

@@ -910,6 +910,12 @@ cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint3
 
 bool keys_optional(int ntiles) { return counting_path(ntiles); }
 
+void binning_visible_list(const gabsplat_binning& bin, int N, int ntiles, const uint32_t** order, const uint32_t** n_vis) {
+  const Workspace ws = carve(bin.workspace, N, bin.capacity, ntiles);
+  *order = ws.pv[0];  // four passes: the depth order ends in the buffer it started in
+  *n_vis = ws.n_vis;
+}
+
 uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles) { return carve(nullptr, N, capacity, ntiles).bytes; }
 
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,

@@ -233,7 +233,8 @@ cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, c
 cudaError_t launch_blend_backward(int N, int K, bool want_abs, const Camera& cam, const gabsplat_projected& proj,
                                   const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const BlendState& saved,
                                   const float* dL_dimage, float* grad2d, cudaStream_t st) {
-  cudaMemsetAsync(grad2d, 0, (size_t)N * grad2d_floats(K) * sizeof(float), st);
+  // grad2d is all zero on entry: the caller zeroes the workspace once, the projection backward clears the rows it read
+  (void)N;
   // launch order: half-tile pairs with the longest saved lists first
   const cudaError_t eo = launch_tile_order(saved.counts, true, cam.tiles_x * cam.tiles_y, saved.order, st);
   if (eo != cudaSuccess) return eo;

@@ -133,8 +133,11 @@ cudaError_t launch_count_pairs(int K, const Camera& cam, const gabsplat_projecte
 cudaError_t launch_blend_backward(int N, int K, bool want_abs, const Camera& cam, const gabsplat_projected& proj,
                                   const gabsplat_binning& bin, const gabsplat_fwd_out& fwd, const BlendState& saved,
                                   const float* dL_dimage, float* grad2d, cudaStream_t st);
+cudaError_t launch_grad_zero(const gabsplat_scene& s, const gabsplat_grads& g, cudaStream_t st);
 cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& proj,
-                                       const float* grad2d, const gabsplat_grads& g, cudaStream_t st);
+                                       const gabsplat_binning& bin, float* grad2d, const gabsplat_grads& g, cudaStream_t st);
+// the depth-ordered ids of the visible primitives and their number, as gabsplat_bin_sort left them in bin.workspace
+void binning_visible_list(const gabsplat_binning& bin, int N, int ntiles, const uint32_t** order, const uint32_t** n_vis);
 
 // order[] = the tiles by descending work, work(t) = pairs[t].y - pairs[t].x (sum == false) or pairs[t].x + pairs[t].y
 cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint32_t* order, cudaStream_t st);

@@ -3,7 +3,7 @@
 //   conic -> U;  f2D = U^-1 T Sigma f -> (U, T, Sigma, f);  U = T Sigma T^T -> (T, Sigma);  T = J W -> J -> t;
 //   mu2D -> t;  t -> mu;  Sigma = R S S^T R^T -> (scale, quaternion);  rgb -> (SH, mu through the view direction).
 // Evaluated in fp64 (HBM-bound: the arithmetic is free, see preprocess.cu).  The kernel zeroes the gradient
-// arrays itself (coalesced, per chunk), so culled primitives cost 300 bytes of stores and no arithmetic.
+// arrays are zeroed by a separate store-only kernel that overlaps the blend backward on a side stream.
 #include "common.cuh"
 #include "sh.cuh"
 
@@ -12,7 +12,7 @@ namespace {
 
 // chain rule of one visible primitive (fp64); writes its row of every gradient array
 __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Camera& c, const uint8_t* __restrict__ rgb_clamped,
-                                             const float* __restrict__ grad2d, const gabsplat_grads& g, const int i) {
+                                             float* grad2d, const gabsplat_grads& g, const int i) {
   const int K = s.K;
   const int G = grad2d_floats(K);
   const float* g2 = grad2d + (size_t)i * G;
@@ -226,57 +226,65 @@ __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Came
   g.d_opacities[i] = g2[5];
   if (g.d_mean2d) { g.d_mean2d[2 * i] = g2[0]; g.d_mean2d[2 * i + 1] = g2[1]; }
   if (g.d_mean2d_abs) { g.d_mean2d_abs[2 * i] = g2[9 + 3 * K]; g.d_mean2d_abs[2 * i + 1] = g2[10 + 3 * K]; }
+  // clear the primitive's 2D gradient record: the workspace is all zero again when the call returns (only visible
+  // primitives ever have a non-zero record), so no 96 B x N memset is needed before the next blend backward
+  float4* row = reinterpret_cast<float4*>(grad2d + (size_t)i * G);
+  for (int q = 0; q < G / 4; ++q) row[q] = make_float4(0.f, 0.f, 0.f, 0.f);
 }
 
 constexpr int kBwdThreads = 128;
-constexpr int kBwdChunk = 512;
 
-// zero p[begin, end) (elements; begin is a multiple of 4 and p is 16-byte aligned), all threads of the CTA
-__device__ __forceinline__ void zero_range(float* __restrict__ p, size_t begin, size_t end) {
-  const size_t n4 = (end - begin) / 4;
-  float4* p4 = reinterpret_cast<float4*>(p + begin);
-  for (size_t j = threadIdx.x; j < n4; j += kBwdThreads) p4[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-  for (size_t j = begin + 4 * n4 + threadIdx.x; j < end; j += kBwdThreads) p[j] = 0.f;
+// One thread per VISIBLE primitive: rank r of the binning's depth-ordered list (any order would do; the list is
+// there, compact, and keeps every lane of every live warp busy -- 10-20 % of the primitives are visible).  The
+// gradient arrays were zeroed by grad_zero_kernel (side stream, concurrently with the blend backward); rows of
+// culled primitives stay zero.
+__global__ void __launch_bounds__(kBwdThreads, 3) preprocess_backward_kernel(gabsplat_scene s, Camera c, const uint32_t* __restrict__ order,
+                                                                         const uint32_t* __restrict__ n_vis,
+                                                                         const uint8_t* __restrict__ rgb_clamped,
+                                                                         float* grad2d, gabsplat_grads g) {
+  const uint32_t r = blockIdx.x * kBwdThreads + threadIdx.x;
+  if (r >= *n_vis) return;
+  backward_one(s, c, rgb_clamped, grad2d, g, (int)order[r]);
 }
 
-// One CTA per chunk of kBwdChunk consecutive primitives: (0) zero the chunk's slice of every gradient array
-// with coalesced 16-byte stores (most primitives are culled and get exactly zero), (1) compact the visible
-// primitives of the chunk into shared memory, (2) walk the compacted list with all lanes busy.
-__global__ void __launch_bounds__(kBwdThreads, 3) preprocess_backward_kernel(gabsplat_scene s, Camera c, const uint32_t* __restrict__ tiles_touched,
-                                                                         const uint8_t* __restrict__ rgb_clamped,
-                                                                         const float* __restrict__ grad2d, gabsplat_grads g) {
-  __shared__ int s_i[kBwdChunk];
-  __shared__ int s_n;
-  if (threadIdx.x == 0) s_n = 0;
-  const size_t b = (size_t)blockIdx.x * kBwdChunk;
-  const size_t e = min((size_t)s.N, b + kBwdChunk);
-  const size_t K = (size_t)s.K;
-  zero_range(g.d_means, 3 * b, 3 * e);
-  zero_range(g.d_scales, 3 * b, 3 * e);
-  zero_range(g.d_rotations, 4 * b, 4 * e);
-  zero_range(g.d_opacities, b, e);
-  zero_range(g.d_sh, 48 * b, 48 * e);
-  if (K) {
-    zero_range(g.d_freqs, 3 * K * b, 3 * K * e);
-    zero_range(g.d_weights, K * b, K * e);
-  }
-  if (g.d_mean2d) zero_range(g.d_mean2d, 2 * b, 2 * e);
-  if (g.d_mean2d_abs) zero_range(g.d_mean2d_abs, 2 * b, 2 * e);
-  __syncthreads();
-  for (size_t i = b + threadIdx.x; i < e; i += kBwdThreads)
-    if (tiles_touched[i] != 0) s_i[atomicAdd(&s_n, 1)] = (int)i;
-  __syncthreads();  // also orders the zero stores before the value stores of other threads
-  const int n = s_n;
-  for (int j = threadIdx.x; j < n; j += kBwdThreads) backward_one(s, c, rgb_clamped, grad2d, g, s_i[j]);
+// Zeroes every gradient array (coalesced 16-byte stores, grid-stride): 300 B per primitive of pure HBM writes,
+// launched on a side stream so that it overlaps the ALU-bound blend backward.
+__global__ void __launch_bounds__(256) grad_zero_kernel(int N, int K, gabsplat_grads g) {
+  const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+  auto fill = [&](float* p, size_t n) {  // p is 16-byte aligned; n floats
+    if (!p) return;
+    float4* p4 = reinterpret_cast<float4*>(p);
+    const size_t n4 = n / 4, stride = (size_t)gridDim.x * blockDim.x, t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (size_t j = t; j < n4; j += stride) p4[j] = z;
+    for (size_t j = 4 * n4 + t; j < n; j += stride) p[j] = 0.f;
+  };
+  const size_t n = (size_t)N, k = (size_t)K;
+  fill(g.d_sh, 48 * n);
+  fill(g.d_means, 3 * n);
+  fill(g.d_scales, 3 * n);
+  fill(g.d_rotations, 4 * n);
+  fill(g.d_opacities, n);
+  if (K) { fill(g.d_freqs, 3 * k * n); fill(g.d_weights, k * n); }
+  fill(g.d_mean2d, 2 * n);
+  fill(g.d_mean2d_abs, 2 * n);
 }
 
 }  // namespace
 
+cudaError_t launch_grad_zero(const gabsplat_scene& s, const gabsplat_grads& g, cudaStream_t st) {
+  if (s.N == 0) return cudaSuccess;
+  grad_zero_kernel<<<148 * 8, 256, 0, st>>>(s.N, s.K, g);
+  launched();
+  return cudaGetLastError();
+}
+
 cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& proj,
-                                       const float* grad2d, const gabsplat_grads& g, cudaStream_t st) {
+                                       const gabsplat_binning& bin, float* grad2d, const gabsplat_grads& g, cudaStream_t st) {
   if (s.N == 0) return cudaGetLastError();
-  preprocess_backward_kernel<<<(s.N + kBwdChunk - 1) / kBwdChunk, kBwdThreads, 0, st>>>(s, cam, proj.tiles_touched,
-                                                                                     proj.rgb_clamped, grad2d, g);
+  const uint32_t *order, *n_vis;
+  binning_visible_list(bin, s.N, cam.tiles_x * cam.tiles_y, &order, &n_vis);
+  preprocess_backward_kernel<<<(s.N + kBwdThreads - 1) / kBwdThreads, kBwdThreads, 0, st>>>(s, cam, order, n_vis,
+                                                                                       proj.rgb_clamped, grad2d, g);
   launched();
   return cudaGetLastError();
 }

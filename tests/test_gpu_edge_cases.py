@@ -159,3 +159,26 @@ def test_inference_forward_has_no_blend_state():
     ranges = bins.tile_ranges.cpu().numpy().view(np.uint32).reshape(tiles, 2)
     assert np.all(counts <= (ranges[:, 1] - ranges[:, 0])[:, None])
     assert counts.sum() > 0
+
+
+def test_backward_leaves_its_workspace_zero():
+    """gabsplat_render_backward needs an all-zero gradient scratch and returns it all zero: two backward calls
+    through the same Grads object give the same gradients (up to the order of the fp32 atomics)."""
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny")
+    cam = scenes.make_cameras("tiny")[0]
+    dL = torch.from_numpy(scenes.make_image_grad("tiny", 0, cam)).cuda()
+    ds = gb.upload_scene(scene)
+    proj = gb.gabsplat_preprocess(ctx, ds, cam)
+    bins = gb.gabsplat_bin_sort(ctx, ds.N, proj, cam)
+    fwd = gb.gabsplat_render_forward(ctx, ds, cam, proj, bins)
+    g = gb.gabsplat_render_backward(ctx, ds, cam, proj, bins, fwd, dL)
+    torch.cuda.synchronize()
+    assert int(g.workspace.count_nonzero().item()) == 0
+    first = {n: getattr(g, n).clone() for n in ("d_means", "d_sh", "d_freqs", "d_weights", "d_opacities")}
+    g.d_means.fill_(123.0)                      # outputs are fully overwritten
+    gb.gabsplat_render_backward(ctx, ds, cam, proj, bins, fwd, dL, g)
+    torch.cuda.synchronize()
+    assert int(g.workspace.count_nonzero().item()) == 0
+    for n, ref in first.items():
+        assert torch.allclose(getattr(g, n), ref, rtol=1e-4, atol=2e-6 * float(ref.abs().max()))
