@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
         float u, v;
         const float dy = __fsub_rn(g.ly[s], a.y);
         const float q = envelope_q(ux, l.y, l.z, dy, u, v);
-        const float G = __expf(q);
+        const float G = envelope_exp2(q);
         Modulation<K> e;
         modulation<K, true>(tail, dx, dy, e);
         const float raw = __fmul_rn(__fmul_rn(oc.x, G), e.M);
@@ -171,9 +171,9 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
           acc[5] += galpha * G * e.M;
           const float gM = galpha * oc.x * G;
           const float gq = galpha * raw;  // dL/dq = g_G * G
-          // q = -(u^2 + v^2), u = L11 dx + L21 dy, v = L22 dy
-          float gdx = gq * (-2.0f * u * l.x);
-          float gdy = gq * (-2.0f * (u * l.y + v * l.z));
+          // G = 2^q, q = -(u^2 + v^2), u = L11 dx + L21 dy, v = L22 dy:  dL/dq = gq ln 2
+          float gdx = gq * (-1.3862943611198906f * u * l.x);
+          float gdy = gq * (-1.3862943611198906f * (u * l.y + v * l.z));
           acc[2] += gq * (-0.5f * dx * dx);
           acc[3] += gq * (-dx * dy);
           acc[4] += gq * (-0.5f * dy * dy);

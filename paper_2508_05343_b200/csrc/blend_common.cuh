@@ -160,12 +160,19 @@ __device__ __forceinline__ int stage_batch(const TileGeom& g, const uint32_t* __
 
 // ---- one primitive at one pixel ---------------------------------------------------------------------
 
-// Quadratic form of the envelope from the packed Cholesky factor: q = -(u^2 + v^2) <= 0  (Eq.3 :101);
+// Quadratic form of the envelope from the packed Cholesky factor, in base 2: G = 2^q, q = -(u^2 + v^2) <= 0  (Eq.3 :101);
 // ux = L11 * dx is shared by the 4 slots of a thread.
 __device__ __forceinline__ float envelope_q(float ux, float L21, float L22, float dy, float& u, float& v) {
   u = __fmaf_rn(L21, dy, ux);
   v = __fmul_rn(L22, dy);
   return -__fmaf_rn(u, u, __fmul_rn(v, v));
+}
+
+// G = 2^q for the base-2 exponent of the packed record (q in [-8, 0]: never denormal)
+__device__ __forceinline__ float envelope_exp2(float q) {
+  float g;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(g) : "f"(q));
+  return g;
 }
 
 template <int K>

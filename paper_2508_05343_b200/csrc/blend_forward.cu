@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
         blended[s] = false;
         if (!pass[s]) continue;
         if (COUNT) ++n_env[s];
-        const float G = __expf(q[s]);
+        const float G = envelope_exp2(q[s]);
         Modulation<K> e;
         modulation<K, false>(tail, dx, dy[s], e);
         const float raw = __fmul_rn(__fmul_rn(oc.x, G), e.M);

@@ -20,8 +20,8 @@ constexpr int kMaxK = GABSPLAT_MAX_K;
 
 // ---- packed gather record (gabsplat_projected.packed), floats -----------------------------------
 //  [0..3]   mean2d hi.x, hi.y (fp32 mean, the indexing value), lo.x, lo.y (fp64 residual)
-//  [4..7]   L11, L21, L22 (sqrt(1/2) * Cholesky factor of the conic: q = -(u^2 + v^2), u = L11 dx + L21 dy,
-//           v = L22 dy), qmin = -ln(255 o) - margin   (envelope reject: skip when q < qmin)
+//  [4..7]   L11, L21, L22 (sqrt(log2(e)/2) * Cholesky factor of the conic: G = 2^q, q = -(u^2 + v^2),
+//           u = L11 dx + L21 dy, v = L22 dy), qmin = (-ln(255 o) - margin) log2(e)   (envelope reject: skip when q < qmin)
 //  [8..11]  opacity, r, g, b
 //  [12..]   tail: 2 pi f2D (x,y) * K (radians per pixel), then omega * K; padded to a multiple of 4 floats
 __host__ __device__ constexpr int tail_floats(int K) { return 4 * ((3 * K + 3) / 4); }

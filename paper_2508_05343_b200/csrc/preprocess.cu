@@ -175,10 +175,12 @@ __device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camer
   {
     // conic = l l^T (Cholesky); q = -1/2 d^T conic d = -(u^2 + v^2) with L = l / sqrt(2)
     const double l11 = sqrt(ca), l21 = cb / l11, l22 = sqrt(fmax(cc - l21 * l21, 0.0));
-    const double rs = 0.70710678118654752440;
+    // ... and in base 2: G = 2^q with q = -(u^2 + v^2), L = l * sqrt(log2(e) / 2), so that the blend kernels feed q
+    // straight to ex2 (no multiply by log2 e, no denormal guard: q >= qmin >= -8)
+    const double rs = 0.84932180028801904272;  // sqrt(0.5 * log2(e))
     // envelope reject threshold: o G < 1/255  <=>  q < -ln(255 o); a little slack keeps the exact alpha test
     // the one that decides borderline pairs
-    const float qmin = (float)(-log(255.0 * (double)opac) - 1e-4);
+    const float qmin = (float)((-log(255.0 * (double)opac) - 1e-4) * 1.4426950408889634074);  // in log2 units
     reinterpret_cast<float4*>(rec)[1] = make_float4((float)(l11 * rs), (float)(l21 * rs), (float)(l22 * rs), qmin);
   }
   // colour: max(0, 0.5 + sum_j Y_j(dir) sh_j), dir from the camera centre to the mean (reading C22)
