@@ -144,6 +144,8 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
       if (K > 0) load_tail<K>(rec + j * R4, tail);
       const float dx = __fsub_rn(g.lx, a.x);
       const float ux = __fmul_rn(l.x, dx);
+      ModulationEntry<K> me;
+      modulation_entry<K>(tail, dx, me);
       float acc[NV];
 #pragma unroll
       for (int i = 0; i < NV; ++i) acc[i] = 0.f;
@@ -155,7 +157,7 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
         const float q = envelope_q(ux, l.y, l.z, dy, u, v);
         const float G = envelope_exp2(q);
         Modulation<K> e;
-        modulation<K, true>(tail, dx, dy, e);
+        modulation<K, true>(tail, me, dy, e);
         const float raw = __fmul_rn(__fmul_rn(oc.x, G), e.M);
         const float alpha = fminf(kAlphaMax, raw);
         const float om = 1.0f - alpha;

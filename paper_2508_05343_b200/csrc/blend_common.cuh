@@ -181,18 +181,36 @@ struct Modulation {
   float cs[K > 0 ? K : 1], sn[K > 0 ? K : 1];
 };
 
-// M = (1 - sum w) + sum w cos(2 pi f2D . d) = 1 + sum w (cos - 1)   (Eq.12 bracket).  tail = staged
-// (2 pi f2D, omega); the phase is in radians and goes to the MUFU unit directly (its own range reduction
-// works in turns: measured error 1.2e-7 |phase|).
-template <int K, bool WANT_SIN>
-__device__ __forceinline__ void modulation(const float* __restrict__ tail, float dx, float dy, Modulation<K>& e) {
-  float M = 1.0f;
+// Per-entry part of the modulation, shared by the 4 pixels of a thread (same column): base = 1 - sum w, and the
+// x part of every phase.
+template <int K>
+struct ModulationEntry {
+  float base;
+  float phx[K > 0 ? K : 1];
+};
+template <int K>
+__device__ __forceinline__ void modulation_entry(const float* __restrict__ tail, float dx, ModulationEntry<K>& m) {
+  float b = 1.0f;
 #pragma unroll
   for (int k = 0; k < K; ++k) {
-    const float ph = __fmaf_rn(tail[2 * k + 1], dy, __fmul_rn(tail[2 * k], dx));
+    b = __fsub_rn(b, tail[2 * K + k]);
+    m.phx[k] = __fmul_rn(tail[2 * k], dx);
+  }
+  m.base = b;
+}
+
+// M = (1 - sum w) + sum w cos(2 pi f2D . d)   (Eq.12 bracket).  tail = staged (2 pi f2D, omega); the phase is in
+// radians and goes to the MUFU unit directly (its own range reduction works in turns: measured error
+// 1.2e-7 |phase|).
+template <int K, bool WANT_SIN>
+__device__ __forceinline__ void modulation(const float* __restrict__ tail, const ModulationEntry<K>& m, float dy, Modulation<K>& e) {
+  float M = m.base;
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+    const float ph = __fmaf_rn(tail[2 * k + 1], dy, m.phx[k]);
     e.cs[k] = __cosf(ph);
     if (WANT_SIN) e.sn[k] = __sinf(ph);
-    M = __fmaf_rn(tail[2 * K + k], __fsub_rn(e.cs[k], 1.0f), M);
+    M = __fmaf_rn(tail[2 * K + k], e.cs[k], M);
   }
   e.M = M;
 }

@@ -69,6 +69,8 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
       float tail[TL];
       if (K > 0) load_tail<K>(s_rec + j * R4, tail);
       const uint32_t pos = __float_as_uint(h1.z);
+      ModulationEntry<K> me;
+      modulation_entry<K>(tail, dx, me);
       bool blended[kSlots];
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) {
@@ -77,7 +79,7 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
         if (COUNT) ++n_env[s];
         const float G = envelope_exp2(q[s]);
         Modulation<K> e;
-        modulation<K, false>(tail, dx, dy[s], e);
+        modulation<K, false>(tail, me, dy[s], e);
         const float raw = __fmul_rn(__fmul_rn(oc.x, G), e.M);
         const float alpha = fminf(kAlphaMax, raw);
         if (alpha < kAlphaMin) continue;
