@@ -149,6 +149,11 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
       float acc[NV];
 #pragma unroll
       for (int i = 0; i < NV; ++i) acc[i] = 0.f;
+      // sums over the thread's pixels of terms whose common factors (dx, L, 2 pi f2D) are applied once, below
+      float Sq = 0.f, Sqy = 0.f, Sqyy = 0.f, Squ = 0.f, Sqv = 0.f;
+      float Sg[K > 0 ? K : 1], Sgy[K > 0 ? K : 1];
+#pragma unroll
+      for (int k = 0; k < K; ++k) Sg[k] = Sgy[k] = 0.f;
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) {
         if (!hit[s]) continue;
@@ -165,32 +170,51 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
         T[s] = Ti;
         const float aT = alpha * Ti;
         acc[6] += aT * gC[s][0]; acc[7] += aT * gC[s][1]; acc[8] += aT * gC[s][2];
-        const float galpha = Ti * (gC[s][0] * (oc.y - B[s][0]) + gC[s][1] * (oc.z - B[s][1]) + gC[s][2] * (oc.w - B[s][2]));
-        B[s][0] = alpha * oc.y + om * B[s][0];
-        B[s][1] = alpha * oc.z + om * B[s][1];
-        B[s][2] = alpha * oc.w + om * B[s][2];
+        const float d0 = oc.y - B[s][0], d1 = oc.z - B[s][1], d2 = oc.w - B[s][2];  // colour minus what is behind
+        const float galpha = Ti * (gC[s][0] * d0 + gC[s][1] * d1 + gC[s][2] * d2);
+        B[s][0] = fmaf(alpha, d0, B[s][0]);  // = alpha c + (1 - alpha) B
+        B[s][1] = fmaf(alpha, d1, B[s][1]);
+        B[s][2] = fmaf(alpha, d2, B[s][2]);
         if (!(raw > kAlphaMax)) {  // the clamp min(0.99, .) has zero derivative when active
-          acc[5] += galpha * G * e.M;
-          const float gM = galpha * oc.x * G;
-          const float gq = galpha * raw;  // dL/dq = g_G * G
-          // G = 2^q, q = -(u^2 + v^2), u = L11 dx + L21 dy, v = L22 dy:  dL/dq = gq ln 2
-          float gdx = gq * (-1.3862943611198906f * u * l.x);
-          float gdy = gq * (-1.3862943611198906f * (u * l.y + v * l.z));
-          acc[2] += gq * (-0.5f * dx * dx);
-          acc[3] += gq * (-dx * dy);
-          acc[4] += gq * (-0.5f * dy * dy);
+          const float gG = galpha * G;
+          acc[5] += gG * e.M;
+          const float ngM = -(gG * oc.x);   // -dL/dM
+          const float gq = galpha * raw;    // dL/d(ln G)
+          const float gqy = gq * dy;
+          Sq += gq; Sqy += gqy; Sqyy += gqy * dy;
+          Squ += gq * u; Sqv += gq * v;
+          float pdx = 0.f, pdy = 0.f;       // per-pixel d/d(dx), d/d(dy) through the phases (AbsGS only)
 #pragma unroll
           for (int k = 0; k < K; ++k) {
-            acc[9 + 2 * K + k] += gM * (e.cs[k] - 1.0f);
-            const float gph = -gM * tail[2 * K + k] * e.sn[k];  // dL/d(phase in radians)
-            acc[9 + 2 * k] += gph * dx;
-            acc[9 + 2 * k + 1] += gph * dy;
-            gdx += gph * tail[2 * k];
-            gdy += gph * tail[2 * k + 1];
+            acc[9 + 2 * K + k] -= ngM * (e.cs[k] - 1.0f);
+            const float gph = ngM * tail[2 * K + k] * e.sn[k];  // dL/d(phase in radians)
+            Sg[k] += gph;
+            Sgy[k] += gph * dy;
+            if (ABS) { pdx += gph * tail[2 * k]; pdy += gph * tail[2 * k + 1]; }
           }
-          acc[0] -= gdx; acc[1] -= gdy;
-          if (ABS) { acc[9 + 3 * K] += fabsf(gdx); acc[10 + 3 * K] += fabsf(gdy); }
+          if (ABS) {
+            // G = 2^q, q = -(u^2 + v^2), u = L11 dx + L21 dy, v = L22 dy:  dL/dq = gq ln 2
+            acc[9 + 3 * K] += fabsf(pdx + gq * (-1.3862943611198906f * u * l.x));
+            acc[10 + 3 * K] += fabsf(pdy + gq * (-1.3862943611198906f * (u * l.y + v * l.z)));
+          }
         }
+      }
+      {
+        // conic (a, b, c): dL/dq (-dx^2 / 2, -dx dy, -dy^2 / 2)
+        acc[2] = -0.5f * dx * dx * Sq;
+        acc[3] = -dx * Sqy;
+        acc[4] = -0.5f * Sqyy;
+        // mean: d = p - mu2D, so dL/dmu2D = -dL/dd;  dL/dd = dL/dq ln 2 (-2 u L11, -2 (u L21 + v L22)) + sum_k gph_k 2 pi f2D_k
+        float gdx = -1.3862943611198906f * l.x * Squ;
+        float gdy = -1.3862943611198906f * (l.y * Squ + l.z * Sqv);
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+          gdx += Sg[k] * tail[2 * k];
+          gdy += Sg[k] * tail[2 * k + 1];
+          acc[9 + 2 * k] = Sg[k] * dx;
+          acc[9 + 2 * k + 1] = Sgy[k];
+        }
+        acc[0] = -gdx; acc[1] = -gdy;
       }
       Butterfly<NV, 16>::run(acc, g.lane);
       float* dst = grad2d + (size_t)s_id[g.warp][j] * GF;
