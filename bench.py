@@ -429,6 +429,24 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
                "d2h_bytes_per_step": 3 * H * W * 4 + (par_bytes if backward else 0),
                "api": "gabsplat_render_host (pinned host buffers in, image + gradients out)"}
 
+    # SURVEY 8(f) f2, beside the step (not part of it): Eq.14 loss forward + backward on a rendered-size image
+    loss_ms = None
+    if rank == 0:
+        img = torch.rand((3, H, W), dtype=torch.float32, device=dev)
+        tgt = torch.rand((3, H, W), dtype=torch.float32, device=dev)
+        ws = torch.empty((int(gb.lib().gabsplat_loss_workspace_bytes(W, H)),), dtype=torch.uint8, device=dev)
+        for _ in range(3):
+            gb.gabsplat_loss(ctx, img, tgt, 0.2, workspace=ws)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(20):
+            gb.gabsplat_loss(ctx, img, tgt, 0.2, workspace=ws)
+        e1.record()
+        torch.cuda.synchronize()
+        loss_ms = e0.elapsed_time(e1) / 20
+        del img, tgt, ws
+
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
@@ -443,6 +461,7 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
         "fwd_ms_per_frame": fwd_ms / args.steps, "fwd_bwd_ms_per_view": ms_per_step if backward else None,
         "fwd_mpix_per_s": world * H * W / 1e6 / (fwd_ms / args.steps / 1e3),
         "ms_per_step_with_keys": keys_total_ms / args.steps,
+        "loss_fwd_bwd_ms": loss_ms,
         "keys": "the sorted 64-bit (tile|depth) keys are an inspectable by-product that no stage reads; the timed "
                 "step does not materialise them, ms_per_step_with_keys is the same step with them written",
         "roofline": roofline, "roofline_per_stage": per_stage,

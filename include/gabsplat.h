@@ -186,6 +186,16 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
                                  const gabsplat_fwd_out* fwd, const float* dL_dimage, gabsplat_grads* grads,
                                  void* grad_workspace, uint64_t grad_workspace_bytes, void* stream);
 
+/* The training loss of PAPER.md:171 Eq.14 on the device:
+ *     L = (1 - lambda) mean|image - target| + lambda (1 - mean SSIM(image, target)),
+ * SSIM per channel with the 11x11 Gaussian window (sigma 1.5, normalised, zero padding) and C1 = 0.01^2, C2 = 0.03^2
+ * of the 3DGS loss the paper adopts.  image, target: [3][H][W] device.  loss_out: device [3] = (L, mean L1, mean SSIM).
+ * dL_dimage (may be NULL: forward only): [3][H][W] device, fully overwritten -- the dL_dimage argument of
+ * gabsplat_render_backward.  Deterministic (fixed-order reductions).  lambda in [0,1]. */
+uint64_t gabsplat_loss_workspace_bytes(int32_t width, int32_t height);
+int32_t gabsplat_loss(gabsplat_ctx* ctx, int32_t width, int32_t height, const float* image, const float* target, float lambda,
+                      float* loss_out, float* dL_dimage, void* workspace, uint64_t workspace_bytes, void* stream);
+
 /* Convenience for callers with HOST buffers (bench.py's end-to-end leg): one forward (and, if
  * dL_dimage_host != NULL, backward) pass with host->device copies of the scene / image gradient and
  * device->host copies of the image / gradients inside the call; synchronises.  All pointers in

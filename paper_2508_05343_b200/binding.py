@@ -98,6 +98,10 @@ def lib():
                                                C.c_uint64, P]
         L.gabsplat_render_host.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.c_uint64, P, P,
                                            C.POINTER(_Grads), P, C.c_uint64, P]
+        L.gabsplat_loss_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
+        L.gabsplat_loss_workspace_bytes.restype = C.c_uint64
+        L.gabsplat_loss.argtypes = [P, C.c_int32, C.c_int32, P, P, C.c_float, P, P, P, C.c_uint64, P]
+        L.gabsplat_loss.restype = C.c_int32
         L.gabsplat_kernel_launches.argtypes = []
         L.gabsplat_kernel_launches.restype = C.c_uint64
         L.gabsplat_timing_enable.argtypes = [P, C.c_int32]
@@ -379,6 +383,22 @@ STAGES = ("preprocess", "scan", "duplicate", "sort", "ranges", "blend_forward", 
 # are known before the instances are placed; larger images run "duplicate", "sort", "ranges")
 LAUNCH_ORDER = ("preprocess", "depth_sort", "scan", "duplicate", "ranges", "sort", "blend_forward", "blend_backward",
                 "preprocess_backward")
+
+
+def gabsplat_loss(ctx: Context, image: torch.Tensor, target: torch.Tensor, lam: float = 0.2, want_grad: bool = True,
+                  workspace: torch.Tensor | None = None, stream=None):
+    """Eq.14 on the device: returns (loss_out [3] = (L, L1, mean SSIM) device tensor, dL_dimage or None)."""
+    assert image.dtype == torch.float32 and target.dtype == torch.float32 and image.shape == target.shape
+    assert image.is_contiguous() and target.is_contiguous() and image.dim() == 3 and image.shape[0] == 3
+    H, W = int(image.shape[1]), int(image.shape[2])
+    nbytes = int(lib().gabsplat_loss_workspace_bytes(W, H))
+    if workspace is None:
+        workspace = torch.empty((nbytes,), dtype=torch.uint8, device=image.device)
+    out = torch.zeros((3,), dtype=torch.float32, device=image.device)
+    grad = torch.empty_like(image) if want_grad else None
+    ctx.check(lib().gabsplat_loss(ctx._h, W, H, _ptr(image), _ptr(target), float(lam), _ptr(out),
+                                  _ptr(grad) if want_grad else None, _ptr(workspace), workspace.numel(), _stream(stream)))
+    return out, grad
 
 
 def gabsplat_kernel_launches() -> int:

@@ -240,6 +240,21 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "render_backward (projection)");
 }
 
+uint64_t gabsplat_loss_workspace_bytes(int32_t width, int32_t height) {
+  return (width <= 0 || height <= 0) ? 0 : loss_workspace_bytes(width, height);
+}
+
+int32_t gabsplat_loss(gabsplat_ctx* ctx, int32_t width, int32_t height, const float* image, const float* target, float lambda,
+                      float* loss_out, float* dL_dimage, void* workspace, uint64_t workspace_bytes, void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  if (width <= 0 || height <= 0 || !image || !target || !loss_out || !(lambda >= 0.f && lambda <= 1.f))
+    return fail(ctx, GABSPLAT_INVALID_ARG, "loss: bad size, lambda or null pointer");
+  if (!workspace || workspace_bytes < loss_workspace_bytes(width, height))
+    return fail(ctx, GABSPLAT_CAPACITY, "loss: workspace too small");
+  const cudaError_t e = launch_loss(width, height, image, target, lambda, loss_out, dL_dimage, workspace, (cudaStream_t)stream);
+  return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "loss");
+}
+
 uint64_t gabsplat_kernel_launches(void) { return g_kernel_launches; }
 
 int32_t gabsplat_timing_enable(gabsplat_ctx* ctx, int32_t on) {

@@ -142,6 +142,10 @@ void binning_visible_list(const gabsplat_binning& bin, int N, int ntiles, const 
 // order[] = the tiles by descending work, work(t) = pairs[t].y - pairs[t].x (sum == false) or pairs[t].x + pairs[t].y
 cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint32_t* order, cudaStream_t st);
 
+uint64_t loss_workspace_bytes(int W, int H);
+cudaError_t launch_loss(int W, int H, const float* image, const float* target, float lambda, float* loss_out,
+                        float* dL_dimage, void* workspace, cudaStream_t st);
+
 uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles);
 bool keys_optional(int ntiles);  // true when the binning never reads gabsplat_binning.keys itself
 
