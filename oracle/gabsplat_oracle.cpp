@@ -771,6 +771,32 @@ void orc_render_forward(SCENE_ARGS, const double* cam, int literal, double* imag
         }
 }
 
+// Auxiliary renders (the paper's frequency-map diagnostic): the same compositing
+// (Eq.12-13, same lists, same alpha rules) with the colour of primitive i replaced by
+//   ( sum_k omega_k |f2D_k|  [cycles per pixel],   t_z  [camera depth],   1 )
+// over a zero background: channel 0 is the blended frequency map, channel 1 the blended depth, channel 2 the
+// accumulated alpha (= 1 - final T).
+void orc_render_aux(SCENE_ARGS, const double* cam, double* image, double* final_T) {
+    const Scene s = make_scene(SCENE_PASS);
+    Cam c = load_cam(cam);
+    c.bg[0] = c.bg[1] = c.bg[2] = 0.0;
+    std::vector<Proj> P;
+    project_all(s, c, 0, P);
+    for (int i = 0; i < N; ++i) {
+        Proj& p = P[i];
+        if (!p.tw.visible) continue;
+        double fm = 0.0;
+        for (int k = 0; k < K; ++k) fm += (double)s.weights[(size_t)i * K + k] * std::sqrt(p.f2d[k][0] * p.f2d[k][0] + p.f2d[k][1] * p.f2d[k][1]);
+        p.rgb[0] = fm; p.rgb[1] = p.t[2]; p.rgb[2] = 1.0;
+    }
+    const std::vector<int> ord = depth_order(P);
+    std::vector<uint32_t> nc((size_t)c.W * c.H), cnt((size_t)c.W * c.H * 3);
+    std::vector<int32_t> last((size_t)c.W * c.H);
+    std::vector<double> margin((size_t)c.W * c.H * 2);
+    const FwdOut out{image, final_T, nc.data(), last.data(), cnt.data(), margin.data()};
+    forward_painter(s, c, P, ord, out, nullptr);
+}
+
 // Literal render of selected pixels only (full-size spot checks).  pixels = [n][2] (x, y).
 // Outputs are per selected pixel: colour[n][3], final_T[n], n_contrib[n], last_id[n], margin[n][2].
 void orc_render_pixels(SCENE_ARGS, const double* cam, int n, const int32_t* pixels, double* colour,

@@ -110,6 +110,16 @@ def render_forward(scene, cam, literal: bool = False) -> dict:
     return o
 
 
+def render_aux(scene, cam) -> dict:
+    """Auxiliary renders: image[0] = blended sum_k omega_k |f2D_k|, image[1] = blended depth, image[2] = accumulated alpha."""
+    keep, args = _scene_args(scene)
+    cv = cam_vector(cam)
+    H, W = cam.height, cam.width
+    o = dict(image=np.zeros((3, H, W)), final_T=np.zeros((H, W)))
+    lib().orc_render_aux(*args, _p(cv), _p(o["image"]), _p(o["final_T"]))
+    return o
+
+
 def render_pixels(scene, cam, pixels) -> dict:
     keep, args = _scene_args(scene)
     cv = cam_vector(cam)
