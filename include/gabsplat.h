@@ -186,6 +186,15 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
                                  const gabsplat_fwd_out* fwd, const float* dL_dimage, gabsplat_grads* grads,
                                  void* grad_workspace, uint64_t grad_workspace_bytes, void* stream);
 
+/* Auxiliary renders (the frequency-map diagnostic of PAPER.md:764): the forward blend of S3 -- same
+ * lists, same alpha rules -- with the colour of primitive i replaced by (sum_k omega_k |f2D_k| in cycles per pixel,
+ * camera depth t_z, 1) over a zero background.  aux_image: [3][H][W] device = (blended frequency map, blended
+ * depth, accumulated alpha = 1 - final T).  workspace: device scratch of >= gabsplat_aux_workspace_bytes bytes. */
+uint64_t gabsplat_aux_workspace_bytes(int32_t N, int32_t width, int32_t height);
+int32_t gabsplat_render_aux(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                            const gabsplat_projected* proj, const gabsplat_binning* bin, float* aux_image,
+                            void* workspace, uint64_t workspace_bytes, void* stream);
+
 /* The training loss of PAPER.md:171 Eq.14 on the device:
  *     L = (1 - lambda) mean|image - target| + lambda (1 - mean SSIM(image, target)),
  * SSIM per channel with the 11x11 Gaussian window (sigma 1.5, normalised, zero padding) and C1 = 0.01^2, C2 = 0.03^2

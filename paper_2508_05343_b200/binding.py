@@ -98,6 +98,11 @@ def lib():
                                                C.c_uint64, P]
         L.gabsplat_render_host.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.c_uint64, P, P,
                                            C.POINTER(_Grads), P, C.c_uint64, P]
+        L.gabsplat_aux_workspace_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int32]
+        L.gabsplat_aux_workspace_bytes.restype = C.c_uint64
+        L.gabsplat_render_aux.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
+                                          C.POINTER(_Binning), P, P, C.c_uint64, P]
+        L.gabsplat_render_aux.restype = C.c_int32
         L.gabsplat_loss_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
         L.gabsplat_loss_workspace_bytes.restype = C.c_uint64
         L.gabsplat_loss.argtypes = [P, C.c_int32, C.c_int32, P, P, C.c_float, P, P, P, C.c_uint64, P]
@@ -383,6 +388,18 @@ STAGES = ("preprocess", "scan", "duplicate", "sort", "ranges", "blend_forward", 
 # are known before the instances are placed; larger images run "duplicate", "sort", "ranges")
 LAUNCH_ORDER = ("preprocess", "depth_sort", "scan", "duplicate", "ranges", "sort", "blend_forward", "blend_backward",
                 "preprocess_backward")
+
+
+def gabsplat_render_aux(ctx: Context, scene: DeviceScene, cam, proj: Projected, bin: Binning, stream=None) -> torch.Tensor:
+    """Auxiliary renders [3][H][W]: blended sum_k omega_k |f2D_k|, blended depth, accumulated alpha."""
+    dev = scene.means.device
+    out = torch.empty((3, cam.height, cam.width), dtype=torch.float32, device=dev)
+    nbytes = int(lib().gabsplat_aux_workspace_bytes(scene.N, cam.width, cam.height))
+    ws = torch.empty((nbytes,), dtype=torch.uint8, device=dev)
+    s, c, p, b = scene.struct(), camera_struct(cam), proj.struct(), bin.struct()
+    ctx.check(lib().gabsplat_render_aux(ctx._h, C.byref(s), C.byref(c), C.byref(p), C.byref(b), _ptr(out), _ptr(ws), nbytes,
+                                        _stream(stream)))
+    return out
 
 
 def gabsplat_loss(ctx: Context, image: torch.Tensor, target: torch.Tensor, lam: float = 0.2, want_grad: bool = True,

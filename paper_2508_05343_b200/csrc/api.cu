@@ -240,6 +240,33 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "render_backward (projection)");
 }
 
+uint64_t gabsplat_aux_workspace_bytes(int32_t N, int32_t width, int32_t height) {
+  if (N < 0 || width <= 0 || height <= 0) return 0;
+  return (uint64_t)N * 16 + 256 + (uint64_t)width * height * 8 + 512;
+}
+
+int32_t gabsplat_render_aux(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                            const gabsplat_projected* proj, const gabsplat_binning* bin, float* aux_image,
+                            void* workspace, uint64_t workspace_bytes, void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  if (!scene_ok(scene)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_aux: bad scene");
+  if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_aux: bad camera");
+  if (!projected_ok(proj, scene->N, scene->K)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_aux: null projected arrays");
+  if (!bin || !bin->tile_ranges || !bin->tile_order || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "render_aux: bad binning");
+  if (!aux_image) return fail(ctx, GABSPLAT_INVALID_ARG, "render_aux: null output");
+  if (!workspace || workspace_bytes < gabsplat_aux_workspace_bytes(scene->N, cam->width, cam->height))
+    return fail(ctx, GABSPLAT_CAPACITY, "render_aux: workspace too small");
+  const uint64_t hw = (uint64_t)cam->width * cam->height;
+  char* w = reinterpret_cast<char*>(((uintptr_t)workspace + 255) & ~(uintptr_t)255);
+  float4* aux = reinterpret_cast<float4*>(w);
+  w += ((uint64_t)scene->N * 16 + 255) & ~255ull;
+  float* final_T = reinterpret_cast<float*>(w);
+  uint32_t* n_contrib = reinterpret_cast<uint32_t*>(w + ((hw * 4 + 255) & ~255ull));
+  const cudaError_t e = launch_blend_aux(scene->N, scene->K, scene->weights, make_camera(*cam), *proj, *bin, aux, aux_image,
+                                         final_T, n_contrib, (cudaStream_t)stream);
+  return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "render_aux");
+}
+
 uint64_t gabsplat_loss_workspace_bytes(int32_t width, int32_t height) {
   return (width <= 0 || height <= 0) ? 0 : loss_workspace_bytes(width, height);
 }

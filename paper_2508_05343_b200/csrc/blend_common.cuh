@@ -87,10 +87,12 @@ __device__ __forceinline__ bool tile_may_pass(float mx, float my, float L11, flo
 // Stage up to kBatch list entries.  Candidate c (0 <= c < m) is list position first + c (REVERSE: first - c),
 // positions 0-based.  Returns the number of survivors, written in candidate order to s_rec.
 // Must be called by all threads of the CTA; ends with a __syncthreads().
+// `colour` (may be null): per-primitive (opacity, c0, c1, c2) that replaces float4 #2 of the packed record (the
+// auxiliary renders blend other per-primitive quantities through the same kernel).
 template <int K, bool REVERSE>
 __device__ __forceinline__ int stage_batch(const TileGeom& g, const uint32_t* __restrict__ ids, const float4* __restrict__ packed,
-                                           uint32_t list_begin, int first, int m, float4* __restrict__ s_rec,
-                                           uint32_t* __restrict__ s_cnt) {
+                                           const float4* __restrict__ colour, uint32_t list_begin, int first, int m,
+                                           float4* __restrict__ s_rec, uint32_t* __restrict__ s_cnt) {
   constexpr int R4 = packed_floats(K) / 4;
   constexpr int kPer = kBatch / kBlendThreads;
   const int tid = threadIdx.x;
@@ -152,7 +154,7 @@ __device__ __forceinline__ int stage_batch(const TileGeom& g, const uint32_t* __
   for (int c = tid; c < (int)total * T4; c += kBlendThreads) {
     const int rec = c / T4, ch = 2 + (c - rec * T4);
     const uint32_t pid = __float_as_uint(s_rec[rec * R4 + 1].w);
-    s_rec[rec * R4 + ch] = __ldg(packed + (size_t)pid * R4 + ch);
+    s_rec[rec * R4 + ch] = (ch == 2 && colour) ? __ldg(colour + pid) : __ldg(packed + (size_t)pid * R4 + ch);
   }
   __syncthreads();
   return (int)total;

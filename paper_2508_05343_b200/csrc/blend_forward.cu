@@ -17,6 +17,7 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
                                                                       const uint2* __restrict__ ranges,
                                                                       const uint32_t* __restrict__ ids,
                                                                       const float4* __restrict__ packed,
+                                                                      const float4* __restrict__ colour,
                                                                       float* __restrict__ image, float* __restrict__ final_T,
                                                                       uint32_t* __restrict__ n_contrib,
                                                                       uint32_t* __restrict__ counters, BlendState save) {
@@ -47,7 +48,7 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
     const bool all_done = done[0] && done[1] && done[2] && done[3];
     if (__syncthreads_and(all_done)) break;
     const int m = min(kBatch, n - b0);
-    const int ns = stage_batch<K, false>(g, ids, packed, range.x, b0, m, s_rec, s_cnt);
+    const int ns = stage_batch<K, false>(g, ids, packed, colour, range.x, b0, m, s_rec, s_cnt);
     if (__all_sync(kFull, all_done)) continue;  // warp-uniform: the votes below need every lane
     for (int j = 0; j < ns; ++j) {
       const float4 h0 = s_rec[j * R4], h1 = s_rec[j * R4 + 1];
@@ -133,29 +134,31 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
 }
 
 template <int K, bool COUNT, bool SAVE>
-cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, float* image,
-                     float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save, cudaStream_t st) {
+cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, const float4* colour,
+                     float* image, float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save,
+                     cudaStream_t st) {
   const int ntiles = cam.tiles_x * cam.tiles_y;
   blend_forward_kernel<K, COUNT, SAVE><<<ntiles, kBlendThreads, 0, st>>>(
-      cam, bin.tile_order, reinterpret_cast<const uint2*>(bin.tile_ranges), bin.ids, reinterpret_cast<const float4*>(proj.packed), image,
-      final_T, n_contrib, counters, save ? *save : BlendState{nullptr, nullptr, nullptr});
+      cam, bin.tile_order, reinterpret_cast<const uint2*>(bin.tile_ranges), bin.ids, reinterpret_cast<const float4*>(proj.packed),
+      colour, image, final_T, n_contrib, counters, save ? *save : BlendState{nullptr, nullptr, nullptr});
   launched();
   return cudaGetLastError();
 }
 
 template <bool COUNT, bool SAVE>
-cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, float* image,
-                     float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save, cudaStream_t st) {
+cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, const float4* colour,
+                     float* image, float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save,
+                     cudaStream_t st) {
   switch (K) {
-    case 0: return launch_k<0, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
-    case 1: return launch_k<1, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
-    case 2: return launch_k<2, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
-    case 3: return launch_k<3, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
-    case 4: return launch_k<4, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
-    case 5: return launch_k<5, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
-    case 6: return launch_k<6, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
-    case 7: return launch_k<7, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
-    case 8: return launch_k<8, COUNT, SAVE>(cam, proj, bin, image, final_T, n_contrib, counters, save, st);
+    case 0: return launch_k<0, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
+    case 1: return launch_k<1, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
+    case 2: return launch_k<2, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
+    case 3: return launch_k<3, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
+    case 4: return launch_k<4, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
+    case 5: return launch_k<5, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
+    case 6: return launch_k<6, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
+    case 7: return launch_k<7, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
+    case 8: return launch_k<8, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
   }
   return cudaErrorInvalidValue;
 }
@@ -165,13 +168,47 @@ cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, c
 cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projected& proj,
                                  const gabsplat_binning& bin, const gabsplat_fwd_out& out, const BlendState* save,
                                  cudaStream_t st) {
-  return save ? dispatch<false, true>(K, cam, proj, bin, out.image, out.final_T, out.n_contrib, nullptr, save, st)
-              : dispatch<false, false>(K, cam, proj, bin, out.image, out.final_T, out.n_contrib, nullptr, nullptr, st);
+  return save ? dispatch<false, true>(K, cam, proj, bin, nullptr, out.image, out.final_T, out.n_contrib, nullptr, save, st)
+              : dispatch<false, false>(K, cam, proj, bin, nullptr, out.image, out.final_T, out.n_contrib, nullptr, nullptr, st);
+}
+
+namespace {
+// (opacity, sum_k omega_k |f2D_k|, depth, 1) per primitive: the "colours" of the auxiliary renders
+__global__ void __launch_bounds__(256) aux_values_kernel(int N, int K, const uint32_t* __restrict__ tiles_touched,
+                                                         const float4* __restrict__ conic_opacity, const float* __restrict__ depth,
+                                                         const float2* __restrict__ freq2d, const float* __restrict__ weights,
+                                                         float4* __restrict__ aux) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (tiles_touched[i] != 0) {
+    float fm = 0.f;
+    for (int k = 0; k < K; ++k) {
+      const float2 f = freq2d[(size_t)i * K + k];
+      fm = fmaf(weights[(size_t)i * K + k], sqrtf(f.x * f.x + f.y * f.y), fm);
+    }
+    v = make_float4(conic_opacity[i].w, fm, depth[i], 1.0f);
+  }
+  aux[i] = v;
+}
+}  // namespace
+
+cudaError_t launch_blend_aux(int N, int K, const float* weights, const Camera& cam, const gabsplat_projected& proj,
+                             const gabsplat_binning& bin, float4* aux, float* image, float* final_T, uint32_t* n_contrib,
+                             cudaStream_t st) {
+  if (N > 0) {
+    aux_values_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, K, proj.tiles_touched, reinterpret_cast<const float4*>(proj.conic_opacity),
+                                                       proj.depth, reinterpret_cast<const float2*>(proj.freq2d), weights, aux);
+    launched();
+  }
+  Camera c = cam;
+  c.bg[0] = c.bg[1] = c.bg[2] = 0.f;
+  return dispatch<false, false>(K, c, proj, bin, aux, image, final_T, n_contrib, nullptr, nullptr, st);
 }
 
 cudaError_t launch_count_pairs(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
                                uint32_t* counters, cudaStream_t st) {
-  return dispatch<true, false>(K, cam, proj, bin, nullptr, nullptr, nullptr, counters, nullptr, st);
+  return dispatch<true, false>(K, cam, proj, bin, nullptr, nullptr, nullptr, nullptr, counters, nullptr, st);
 }
 
 }  // namespace gabsplat

@@ -128,6 +128,9 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
 cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projected& proj,
                                  const gabsplat_binning& bin, const gabsplat_fwd_out& out, const BlendState* save,
                                  cudaStream_t st);
+cudaError_t launch_blend_aux(int N, int K, const float* weights, const Camera& cam, const gabsplat_projected& proj,
+                             const gabsplat_binning& bin, float4* aux, float* image, float* final_T, uint32_t* n_contrib,
+                             cudaStream_t st);
 cudaError_t launch_count_pairs(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
                                uint32_t* counters, cudaStream_t st);
 cudaError_t launch_blend_backward(int N, int K, bool want_abs, const Camera& cam, const gabsplat_projected& proj,
