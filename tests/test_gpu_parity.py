@@ -247,3 +247,19 @@ def test_banded_placement(monkeypatch):
     monkeypatch.setenv("GABSPLAT_PLACE_BANDS", "3")
     g = _gpu(scene, cam)
     check_binning(g, orc.bin_sort(scene, cam))
+
+
+def test_full_size_gradients():
+    """BASELINE.json config 3 (1M primitives, 1297x840) forward + backward in the launch configuration bench.py
+    times, every gradient tensor against the oracle's analytic gradients (painter's-order loop, ~10 s on the host)."""
+    orc = _oracle()
+    scene = scenes.make_scene("unbounded")
+    cam = scenes.make_cameras("unbounded")[0]
+    dL = scenes.make_image_grad("unbounded", 0, cam)
+    g = _gpu(scene, cam, dL)
+    o = orc.render_backward(scene, cam, dL)
+    check_gradients(g, o)
+    # culled primitives get exactly zero
+    culled = g["tiles_touched"] == 0
+    for n in ("d_means", "d_scales", "d_rotations", "d_opacities", "d_sh", "d_freqs", "d_weights"):
+        assert not np.any(g[n][culled])
