@@ -486,24 +486,29 @@ __global__ void __launch_bounds__(256) tile_ranges_kernel(const u64* __restrict_
 // idle in the tail with tiles launched in raster order).  One CTA: max, 256-bucket counting sort by
 // work / max; the order inside a bucket is immaterial.
 // ------------------------------------------------------------------------------------------------
-template <bool SUM>
+// MODE 0: work(t) = pairs[t].y - pairs[t].x;  1: pairs[t].x + pairs[t].y;  2: ((const u32*)pairs)[t]
+template <int MODE>
 __global__ void __launch_bounds__(1024) tile_order_kernel(const uint2* __restrict__ pairs, u32 ntiles, u32* __restrict__ order) {
+  auto work = [&](u32 t) -> u32 {
+    if (MODE == 2) return reinterpret_cast<const u32*>(pairs)[t];
+    const uint2 p = pairs[t];
+    return MODE == 1 ? p.x + p.y : p.y - p.x;
+  };
   __shared__ u32 s_max, s_hist[256], s_base[256];
   if (threadIdx.x == 0) s_max = 0;
   if (threadIdx.x < 256) s_hist[threadIdx.x] = 0;
   __syncthreads();
   u32 mx = 0;
   for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) {
-    const uint2 p = pairs[t];
-    mx = max(mx, SUM ? p.x + p.y : p.y - p.x);
+    mx = max(mx, work(t));
   }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d));
   if ((threadIdx.x & 31) == 0) atomicMax(&s_max, mx);
   __syncthreads();
   const float scale = 255.0f / (float)max(s_max, 1u);
-  auto bucket = [&](const uint2 p) { return 255u - min(255u, (u32)((float)(SUM ? p.x + p.y : p.y - p.x) * scale)); };
-  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) atomicAdd(&s_hist[bucket(pairs[t])], 1u);
+  auto bucket = [&](u32 t) { return 255u - min(255u, (u32)((float)work(t) * scale)); };
+  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) atomicAdd(&s_hist[bucket(t)], 1u);
   __syncthreads();
   if (threadIdx.x < 32) {  // exclusive scan of 256 counts by one warp, 8 per lane
     u32 c[8], tot = 0;
@@ -514,7 +519,7 @@ __global__ void __launch_bounds__(1024) tile_order_kernel(const uint2* __restric
     for (int j = 0; j < 8; ++j) { s_base[threadIdx.x * 8 + j] = run; run += c[j]; }
   }
   __syncthreads();
-  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) order[atomicAdd(&s_base[bucket(pairs[t])], 1u)] = t;
+  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) order[atomicAdd(&s_base[bucket(t)], 1u)] = t;
 }
 
 __global__ void clamp_count_kernel(u32* sort_count, const u32* num_instances, u64 capacity) {
@@ -902,8 +907,15 @@ void radix_pass_small(const u32* kin, const u32* vin, u32* kout, u32* vout, cons
 
 cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint32_t* order, cudaStream_t st) {
   if (ntiles <= 0) return cudaSuccess;
-  if (sum) tile_order_kernel<true><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
-  else tile_order_kernel<false><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
+  if (sum) tile_order_kernel<1><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
+  else tile_order_kernel<0><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
+  launched();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_half_tile_order(const uint32_t* work, int n, uint32_t* order, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  tile_order_kernel<2><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(work), (u32)n, order);
   launched();
   return cudaGetLastError();
 }

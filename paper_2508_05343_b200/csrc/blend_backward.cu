@@ -71,7 +71,7 @@ constexpr int kReplay = 32;  // saved entries staged per warp and batch
 // A lane recomputes G, cos, sin and alpha of its blended pixels with the forward's own functions (bit-identical
 // alpha), recovers the transmittance in front of the primitive by division, and accumulates the gradient terms.
 template <int K, bool ABS>
-__global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera cam, const uint2* __restrict__ ranges,
+__global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, const uint2* __restrict__ ranges,
                                                                        BlendState saved, const float4* __restrict__ packed,
                                                                        const float* __restrict__ final_T,
                                                                        const float* __restrict__ dL_dimage,
@@ -80,16 +80,17 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
   constexpr int TL = K > 0 ? tail_floats(K) : 1;
   constexpr int NV = 9 + 3 * K + (ABS ? 2 : 0);
   constexpr int GF = grad2d_floats(K);
-  constexpr int kWarps = kBlendThreads / 32;
-  __shared__ float4 s_rec[kWarps][kReplay * R4];
-  __shared__ uint4 s_mask[kWarps][kReplay];
-  __shared__ uint32_t s_id[kWarps][kReplay];
-  const TileGeom g = tile_geom(cam, saved.order);
+  // one warp per CTA: CTA b replays half tile order[b] (half tiles by descending saved-list length)
+  __shared__ float4 s_rec1[kReplay * R4];
+  __shared__ uint4 s_mask1[kReplay];
+  __shared__ uint32_t s_id1[kReplay];
+  const uint32_t half = __ldg(saved.order + blockIdx.x);
+  const TileGeom g = tile_geom_at(cam, (int)(half >> 1), (int)(half & 1u), (int)threadIdx.x);
   const uint2 range = ranges[g.tile];
   const size_t HW = (size_t)cam.width * cam.height;
   const int cnt = (int)saved.counts[2 * g.tile + g.warp];
   const size_t base = 2 * (size_t)range.x + (size_t)g.warp * (range.y - range.x);
-  float4* __restrict__ rec = s_rec[g.warp];
+  float4* __restrict__ rec = s_rec1;
 
   float T[kSlots], gC[kSlots][3], B[kSlots][3];
 #pragma unroll
@@ -118,8 +119,8 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
       my_id = __ldg(saved.ids + base + (size_t)(end - 1 - g.lane));
       my_mask = __ldg(saved.masks + base + (size_t)(end - 1 - g.lane));
     }
-    s_id[g.warp][g.lane] = my_id;
-    s_mask[g.warp][g.lane] = my_mask;
+    s_id1[g.lane] = my_id;
+    s_mask1[g.lane] = my_mask;
 #pragma unroll
     for (int it = 0; it < R4; ++it) {
       const int idx = it * 32 + g.lane;
@@ -136,7 +137,7 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
     }
     __syncwarp();
     for (int j = 0; j < m; ++j) {
-      const uint4 mk = s_mask[g.warp][j];
+      const uint4 mk = s_mask1[j];
       const float4 a = rec[j * R4], l = rec[j * R4 + 1], oc = rec[j * R4 + 2];
       const bool hit[kSlots] = {((mk.x >> g.lane) & 1u) != 0u, ((mk.y >> g.lane) & 1u) != 0u,
                                 ((mk.z >> g.lane) & 1u) != 0u, ((mk.w >> g.lane) & 1u) != 0u};
@@ -217,7 +218,7 @@ __global__ void __launch_bounds__(kBlendThreads, 8) blend_backward_kernel(Camera
         acc[0] = -gdx; acc[1] = -gdy;
       }
       Butterfly<NV, 16>::run(acc, g.lane);
-      float* dst = grad2d + (size_t)s_id[g.warp][j] * GF;
+      float* dst = grad2d + (size_t)s_id1[j] * GF;
 #pragma unroll
       for (int i = 0; i < NL; ++i)
         if (my_idx[i] >= 0 && acc[i] != 0.f) atomicAdd(dst + my_idx[i], acc[i]);
@@ -230,7 +231,7 @@ template <int K, bool ABS>
 cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
                      const gabsplat_fwd_out& fwd, const BlendState& saved, const float* dL, float* grad2d, cudaStream_t st) {
   const int ntiles = cam.tiles_x * cam.tiles_y;
-  blend_backward_kernel<K, ABS><<<ntiles, kBlendThreads, 0, st>>>(
+  blend_backward_kernel<K, ABS><<<2 * ntiles, 32, 0, st>>>(
       cam, reinterpret_cast<const uint2*>(bin.tile_ranges), saved, reinterpret_cast<const float4*>(proj.packed),
       fwd.final_T, dL, grad2d);
   launched();
@@ -262,7 +263,7 @@ cudaError_t launch_blend_backward(int N, int K, bool want_abs, const Camera& cam
   // grad2d is all zero on entry: the caller zeroes the workspace once, the projection backward clears the rows it read
   (void)N;
   // launch order: half-tile pairs with the longest saved lists first
-  const cudaError_t eo = launch_tile_order(saved.counts, true, cam.tiles_x * cam.tiles_y, saved.order, st);
+  const cudaError_t eo = launch_half_tile_order(saved.counts, 2 * cam.tiles_x * cam.tiles_y, saved.order, st);
   if (eo != cudaSuccess) return eo;
   return want_abs ? dispatch<true>(K, cam, proj, bin, fwd, saved, dL_dimage, grad2d, st)
                   : dispatch<false>(K, cam, proj, bin, fwd, saved, dL_dimage, grad2d, st);

@@ -43,13 +43,18 @@ struct TileGeom {
 };
 
 // CTA b works on tile order[b]: the tiles by descending work (binning.cu tile_order_kernel)
+__device__ __forceinline__ TileGeom tile_geom_at(const Camera& cam, int tile, int warp, int lane);
 __device__ __forceinline__ TileGeom tile_geom(const Camera& cam, const uint32_t* __restrict__ order) {
+  return tile_geom_at(cam, (int)__ldg(order + blockIdx.x), threadIdx.x >> 5, threadIdx.x & 31);
+}
+// geometry of lane `lane` of half `warp` (rows 8 warp .. 8 warp + 7) of tile `tile`
+__device__ __forceinline__ TileGeom tile_geom_at(const Camera& cam, int tile, int warp, int lane) {
   TileGeom g;
-  g.tile = (int)__ldg(order + blockIdx.x);
+  g.tile = tile;
   g.tx = g.tile % cam.tiles_x;
   g.ty = g.tile / cam.tiles_x;
-  g.warp = threadIdx.x >> 5;
-  g.lane = threadIdx.x & 31;
+  g.warp = warp;
+  g.lane = lane;
   g.lxi = g.lane & 15;
   g.lx = (float)g.lxi;
   g.px = g.tx * kTile + g.lxi;

@@ -40,12 +40,12 @@ __host__ __device__ constexpr int grad2d_floats(int K) { return 4 * ((grad2d_val
 // 16x2 pixel strips, the ballot of the lanes whose pixel blended the primitive.
 struct BlendState {
   uint32_t* counts;  // [2 * tiles]
-  uint32_t* order;   // [tiles]  tiles by descending counts (launch order of the backward CTAs)
+  uint32_t* order;   // [2 * tiles]  half tiles by descending counts (launch order of the backward CTAs)
   uint32_t* ids;     // [2 * capacity]
   uint4* masks;      // [2 * capacity]
 };
 inline uint64_t blend_state_bytes(uint64_t tiles, uint64_t capacity) {
-  const uint64_t a = (2 * tiles * 4 + 255) & ~255ull, o = (tiles * 4 + 255) & ~255ull, b = (2 * capacity * 4 + 255) & ~255ull;
+  const uint64_t a = (2 * tiles * 4 + 255) & ~255ull, o = (2 * tiles * 4 + 255) & ~255ull, b = (2 * capacity * 4 + 255) & ~255ull;
   return a + o + b + 2 * capacity * 16 + 256;
 }
 inline BlendState make_blend_state(void* p, uint64_t tiles, uint64_t capacity) {
@@ -54,7 +54,7 @@ inline BlendState make_blend_state(void* p, uint64_t tiles, uint64_t capacity) {
   s.counts = reinterpret_cast<uint32_t*>(q);
   q += (2 * tiles * 4 + 255) & ~255ull;
   s.order = reinterpret_cast<uint32_t*>(q);
-  q += (tiles * 4 + 255) & ~255ull;
+  q += (2 * tiles * 4 + 255) & ~255ull;
   s.ids = reinterpret_cast<uint32_t*>(q);
   q += (2 * capacity * 4 + 255) & ~255ull;
   s.masks = reinterpret_cast<uint4*>(q);
@@ -144,6 +144,8 @@ void binning_visible_list(const gabsplat_binning& bin, int N, int ntiles, const 
 
 // order[] = the tiles by descending work, work(t) = pairs[t].y - pairs[t].x (sum == false) or pairs[t].x + pairs[t].y
 cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint32_t* order, cudaStream_t st);
+// order[] = the items 0..n-1 by descending work[item]
+cudaError_t launch_half_tile_order(const uint32_t* work, int n, uint32_t* order, cudaStream_t st);
 
 uint64_t loss_workspace_bytes(int W, int H);
 cudaError_t launch_loss(int W, int H, const float* image, const float* target, float lambda, float* loss_out,
