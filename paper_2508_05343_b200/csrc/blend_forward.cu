@@ -44,6 +44,8 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
 
   uint32_t n_saved = 0;                                        // warp-uniform
   const size_t save_at = 2 * (size_t)range.x + (size_t)g.warp * n;  // this warp's slice of save.ids / save.masks
+  uint32_t* save_id = SAVE ? save.ids + save_at : nullptr;          // lane 0's write cursors
+  uint4* save_mask = SAVE ? save.masks + save_at : nullptr;
   for (int b0 = 0; b0 < n; b0 += kBatch) {
     const bool all_done = done[0] && done[1] && done[2] && done[3];
     if (__syncthreads_and(all_done)) break;
@@ -100,13 +102,15 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
         if (COUNT) { ++n_blend[s]; n_env_last[s] = n_env[s]; }
       }
       if (SAVE) {
-        uint4 m;
-        m.x = __ballot_sync(kFull, blended[0]); m.y = __ballot_sync(kFull, blended[1]);
-        m.z = __ballot_sync(kFull, blended[2]); m.w = __ballot_sync(kFull, blended[3]);
-        if ((m.x | m.y | m.z | m.w) != 0u) {
+        // most evaluated entries blend at no pixel of the warp (M too small): one vote decides, the four ballots
+        // and the two stores are paid only by entries that go to the list
+        if (__any_sync(kFull, blended[0] || blended[1] || blended[2] || blended[3])) {
+          uint4 m;
+          m.x = __ballot_sync(kFull, blended[0]); m.y = __ballot_sync(kFull, blended[1]);
+          m.z = __ballot_sync(kFull, blended[2]); m.w = __ballot_sync(kFull, blended[3]);
           if (g.lane == 0) {
-            save.ids[save_at + n_saved] = __float_as_uint(h1.w);
-            save.masks[save_at + n_saved] = m;
+            *save_id++ = __float_as_uint(h1.w);
+            *save_mask++ = m;
           }
           ++n_saved;
         }
