@@ -74,10 +74,8 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
       const uint32_t pos = __float_as_uint(h1.z);
       ModulationEntry<K> me;
       modulation_entry<K>(tail, dx, me);
-      bool blended[kSlots];
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) {
-        blended[s] = false;
         if (!pass[s]) continue;
         if (COUNT) ++n_env[s];
         const float G = envelope_exp2(q[s]);
@@ -98,16 +96,17 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
         Cb[s] = __fmaf_rn(oc.w, wgt, Cb[s]);
         T[s] = Tn;
         last[s] = pos;
-        blended[s] = true;
         if (COUNT) { ++n_blend[s]; n_env_last[s] = n_env[s]; }
       }
       if (SAVE) {
         // most evaluated entries blend at no pixel of the warp (M too small): one vote decides, the four ballots
         // and the two stores are paid only by entries that go to the list
-        if (__any_sync(kFull, blended[0] || blended[1] || blended[2] || blended[3])) {
+        // (a pixel blended this entry iff its last-contributor position now is the entry's)
+        const bool b0 = last[0] == pos, b1 = last[1] == pos, b2 = last[2] == pos, b3 = last[3] == pos;
+        if (__any_sync(kFull, b0 || b1 || b2 || b3)) {
           uint4 m;
-          m.x = __ballot_sync(kFull, blended[0]); m.y = __ballot_sync(kFull, blended[1]);
-          m.z = __ballot_sync(kFull, blended[2]); m.w = __ballot_sync(kFull, blended[3]);
+          m.x = __ballot_sync(kFull, b0); m.y = __ballot_sync(kFull, b1);
+          m.z = __ballot_sync(kFull, b2); m.w = __ballot_sync(kFull, b3);
           if (g.lane == 0) {
             *save_id++ = __float_as_uint(h1.w);
             *save_mask++ = m;
