@@ -29,6 +29,12 @@ typedef uint64_t u64;
 // Device-wide prefix sum of u32 (three launches: block sums, scan of the sums, block scans).
 // GATHER: element i of the input is in[idx[i]].
 // ------------------------------------------------------------------------------------------------
+// radix passes: pairs per CTA (declared here: depth_keys_kernel bins its output by sort tile)
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 16;
+constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 pairs per block
+constexpr int kSortWarps = kSortThreads / 32;
+
 constexpr int kScanThreads = 256;
 constexpr int kScanItems = 16;
 constexpr int kScanTile = kScanThreads * kScanItems;  // 4096 elements per block
@@ -188,7 +194,8 @@ void device_scan(const u32* in, const u32* idx, u32* out, u32 n, const u32* n_de
 // passes sort n_vis pairs, not N.
 __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __restrict__ tiles_touched,
                                                          const float* __restrict__ depth, const u32* __restrict__ chunk_visible,
-                                                         u32* __restrict__ keys, u32* __restrict__ vals, u32* __restrict__ n_vis) {
+                                                         u32* __restrict__ keys, u32* __restrict__ vals, u32* __restrict__ n_vis,
+                                                         u32* __restrict__ table0) {
   __shared__ u32 s_part[8], s_off;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   u32 acc = 0;
@@ -219,8 +226,10 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __res
     for (int j = 0; j < 8; ++j) { const u32 c = s_part[j]; before += j < w ? c : 0u; total += c; }
     if (vis) {
       const u32 pos = run + before + (u32)__popc(bal & ((1u << lane) - 1u));
-      keys[pos] = __float_as_uint(depth[i]);
+      const u32 key = __float_as_uint(depth[i]);
+      keys[pos] = key;
       vals[pos] = (u32)i;
+      atomicAdd(&table0[(pos / kSortTile) * 256u + (key & 255u)], 1u);  // histogram of the first pass, per sort tile
     }
     run += total;
   }
@@ -311,10 +320,6 @@ __global__ void __launch_bounds__(kDupThreads) duplicate_kernel(const u32* __res
 // histogram, scan of the [digit][block] table, stable scatter.  FINAL (last pass of stage B): the output is
 // the 64-bit key (key << 32) | gather[value] and the value.
 // ------------------------------------------------------------------------------------------------
-constexpr int kSortThreads = 256;
-constexpr int kSortItems = 16;
-constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 pairs per block
-constexpr int kSortWarps = kSortThreads / 32;
 
 // BLOCK_MAJOR: table[block][digit] (read back by sort_scatter<., true>); else table[digit][block] (scanned in place)
 template <bool BLOCK_MAJOR>
@@ -359,7 +364,7 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
                                                             u32* __restrict__ kout, u32* __restrict__ vout,
                                                             u64* __restrict__ kout64, const u32* __restrict__ gather,
                                                             const u32* __restrict__ count, const u32* __restrict__ table,
-                                                            u32 nblocks, int shift) {
+                                                            u32 nblocks, int shift, u32* __restrict__ table_next) {
   __shared__ u32 warp_hist[kSortWarps][256];
   __shared__ u32 local_base[256];
   __shared__ u32 global_base[256];
@@ -463,6 +468,8 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
     if (FINAL) kout64[dst] = ((u64)key << 32) | (u64)__ldg(gather + val);
     else kout[dst] = key;
     vout[dst] = val;
+    // SELF: the next pass's per-tile histogram (of this pass's output arrangement), so that a pass is one launch
+    if (SELF && table_next) atomicAdd(&table_next[(dst / kSortTile) * 256u + ((key >> (shift + 8)) & 255u)], 1u);
   }
 }
 
@@ -839,6 +846,7 @@ struct Workspace {
   u32* count_a;     // [1] = N
   u32* count_b;     // [1] = D, or 0 when D > capacity
   u32* table;       // [256][nblocks]
+  u32* dtable[4];   // per depth pass: [sort_blocks(N)][256] histograms of that pass's input arrangement
   u32* pk[2];       // stage A key ping-pong [N]
   u32* pv[2];       // stage A value ping-pong [N]; pv[0] ends up holding the depth order
   u32* ik;          // stage B (radix path) alternate keys [capacity]
@@ -865,6 +873,11 @@ Workspace carve(void* base, int N, u64 capacity, int ntiles) {
   w.count_a = (u32*)take(16);
   w.count_b = (u32*)take(16);
   w.table = (u32*)take(table_n * 4);
+  {  // contiguous, zeroed by one memset per call
+    const u64 one = (u64)256 * (sort_blocks((u64)N) ? sort_blocks((u64)N) : 1);
+    u32* base4 = (u32*)take(4 * one * 4);
+    for (int i = 0; i < 4; ++i) w.dtable[i] = base4 + i * one;
+  }
   for (int i = 0; i < 2; ++i) { w.pk[i] = (u32*)take((u64)N * 4); w.pv[i] = (u32*)take((u64)N * 4); }
   w.n_vis = (u32*)take(16);
   w.bounds = (u32*)take((kChunks + 1) * 4);
@@ -889,18 +902,19 @@ void radix_pass(const u32* kin, const u32* vin, u32* kout, u32* vout, u64* kout6
   launched();
   device_scan<false, false>(ws.table, nullptr, ws.table, 256u * nblocks, nullptr, 0u, ws.scan_sums, nullptr, st);
   if (kout64)
-    sort_scatter<true, false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift);
+    sort_scatter<true, false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, nullptr);
   else
-    sort_scatter<false, false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift);
+    sort_scatter<false, false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, nullptr);
   launched();
 }
 
-// a pass over the visible primitives: histogram + self-scanning scatter
+// a pass over the visible primitives: ONE launch -- its per-tile histogram was accumulated by the producer of its
+// input (depth_keys_kernel for the first pass, the previous pass's scatter for the others)
 void radix_pass_small(const u32* kin, const u32* vin, u32* kout, u32* vout, const u32* count, u32 nblocks, int shift,
-                      const Workspace& ws, cudaStream_t st) {
-  sort_histogram<true><<<nblocks, kSortThreads, 0, st>>>(kin, count, ws.table, nblocks, shift);
-  sort_scatter<false, true><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, nullptr, nullptr, count, ws.table, nblocks, shift);
-  launched(2);
+                      const u32* table, u32* table_next, cudaStream_t st) {
+  sort_scatter<false, true><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, nullptr, nullptr, count, table, nblocks, shift,
+                                                            table_next);
+  launched();
 }
 
 }  // namespace
@@ -941,12 +955,15 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   }
   // A: depth order of the primitives (digits 0-3 of the 64-bit key)
   tm.begin(GABSPLAT_STAGE_DEPTH_SORT, st);
-  depth_keys_kernel<<<(N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK, 256, 0, st>>>(N, proj.tiles_touched, proj.depth,
-                                                                            proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis);
-  launched();
   const u32 nba = sort_blocks((u64)N);
+  cudaMemsetAsync(ws.dtable[0], 0, (size_t)4 * 256 * nba * sizeof(u32), st);
+  depth_keys_kernel<<<(N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK, 256, 0, st>>>(N, proj.tiles_touched, proj.depth,
+                                                                            proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis,
+                                                                            ws.dtable[0]);
+  launched();
   for (int p = 0; p < 4; ++p)
-    radix_pass_small(ws.pk[p & 1], ws.pv[p & 1], ws.pk[(p & 1) ^ 1], ws.pv[(p & 1) ^ 1], ws.n_vis, nba, 8 * p, ws, st);
+    radix_pass_small(ws.pk[p & 1], ws.pv[p & 1], ws.pk[(p & 1) ^ 1], ws.pv[(p & 1) ^ 1], ws.n_vis, nba, 8 * p, ws.dtable[p],
+                     p < 3 ? ws.dtable[p + 1] : nullptr, st);
   const u32* order = ws.pv[0];
   tm.end(st);
   // K2 (over the n_vis ranks)
