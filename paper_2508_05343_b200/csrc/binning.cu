@@ -34,6 +34,8 @@ constexpr int kSortThreads = 256;
 constexpr int kSortItems = 16;
 constexpr int kSortTile = kSortThreads * kSortItems;  // 4096 pairs per block
 constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSmallItems = 16;  // depth passes over the visible primitives (4 was measured slower: more CTAs to sum over)
+constexpr int kSmallTile = kSortThreads * kSmallItems;
 
 constexpr int kScanThreads = 256;
 constexpr int kScanItems = 16;
@@ -229,7 +231,7 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __res
       const u32 key = __float_as_uint(depth[i]);
       keys[pos] = key;
       vals[pos] = (u32)i;
-      atomicAdd(&table0[(pos / kSortTile) * 256u + (key & 255u)], 1u);  // histogram of the first pass, per sort tile
+      atomicAdd(&table0[(pos / kSmallTile) * 256u + (key & 255u)], 1u);  // histogram of the first pass, per sort tile
     }
     run += total;
   }
@@ -359,7 +361,9 @@ __global__ void __launch_bounds__(kSortThreads) sort_histogram(const u32* __rest
 // SELF: the table holds raw per-block counts, block-major; every CTA sums the columns of the blocks before it
 // and the digit totals itself (a few dozen blocks when the pairs are the visible primitives): two launches per
 // pass instead of five.  Otherwise the table holds the exclusive scan of the digit-major counts.
-template <bool FINAL, bool SELF>
+// ITEMS pairs per thread: 16 on the instance-sized lists; 4 on the visible primitives, where a pass is a single
+// wave of CTAs and its time is one CTA's latency (4 ranking rounds instead of 16)
+template <bool FINAL, bool SELF, int ITEMS = kSortItems>
 __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restrict__ kin, const u32* __restrict__ vin,
                                                             u32* __restrict__ kout, u32* __restrict__ vout,
                                                             u64* __restrict__ kout64, const u32* __restrict__ gather,
@@ -368,31 +372,32 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
   __shared__ u32 warp_hist[kSortWarps][256];
   __shared__ u32 local_base[256];
   __shared__ u32 global_base[256];
-  __shared__ u32 skeys[kSortTile];
-  __shared__ u32 svals[kSortTile];
+  constexpr int TILE = kSortThreads * ITEMS;
+  __shared__ u32 skeys[TILE];
+  __shared__ u32 svals[TILE];
   const u32 D = *count;
-  const u32 start = blockIdx.x * kSortTile;
+  const u32 start = blockIdx.x * TILE;
   if (start >= D) return;
-  const u32 n = min((u32)kSortTile, D - start);
+  const u32 n = min((u32)TILE, D - start);
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
 #pragma unroll
   for (int j = 0; j < kSortWarps; ++j) warp_hist[j][threadIdx.x] = 0;
   __syncthreads();
 
-  // warp w owns the contiguous run [w * 32 * kSortItems, (w+1) * 32 * kSortItems) of the block's tile, visited
+  // warp w owns the contiguous run [w * 32 * ITEMS, (w+1) * 32 * ITEMS) of the block's tile, visited
   // 32 consecutive pairs at a time: rank order = input order (stability)
-  u32 k[kSortItems], v[kSortItems], rank[kSortItems];
+  u32 k[ITEMS], v[ITEMS], rank[ITEMS];
   const u32 lt_mask = (1u << lane) - 1u;
 #pragma unroll
-  for (int r = 0; r < kSortItems; ++r) {
-    const u32 idx = (u32)w * 32u * kSortItems + (u32)r * 32u + (u32)lane;
+  for (int r = 0; r < ITEMS; ++r) {
+    const u32 idx = (u32)w * 32u * ITEMS + (u32)r * 32u + (u32)lane;
     const bool valid = idx < n;
     k[r] = valid ? kin[start + idx] : 0xffffffffu;
     v[r] = valid ? vin[start + idx] : 0;
   }
 #pragma unroll
-  for (int r = 0; r < kSortItems; ++r) {
-    const u32 idx = (u32)w * 32u * kSortItems + (u32)r * 32u + (u32)lane;
+  for (int r = 0; r < ITEMS; ++r) {
+    const u32 idx = (u32)w * 32u * ITEMS + (u32)r * 32u + (u32)lane;
     const bool valid = idx < n;
     const u32 d = (k[r] >> shift) & 255u;
     // lanes holding the same digit; invalid lanes get a digit value no valid lane can have
@@ -435,9 +440,10 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
     const u32 ex = block_exclusive_scan(tot, &total);
     local_base[d] = ex;
     if (SELF) {
-      const u32 nact = (D + kSortTile - 1) / kSortTile;
+      const u32 nact = (D + TILE - 1) / TILE;
       u32 below = 0, all = 0;
-      for (u32 bb = 0; bb < nact; ++bb) {
+#pragma unroll 8
+      for (u32 bb = 0; bb < nact; ++bb) {  // independent loads: keep 8 in flight
         const u32 c = __ldg(table + bb * 256u + (u32)d);
         all += c;
         below += bb < blockIdx.x ? c : 0u;
@@ -450,8 +456,8 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
   }
   __syncthreads();
 #pragma unroll
-  for (int r = 0; r < kSortItems; ++r) {
-    const u32 idx = (u32)w * 32u * kSortItems + (u32)r * 32u + (u32)lane;
+  for (int r = 0; r < ITEMS; ++r) {
+    const u32 idx = (u32)w * 32u * ITEMS + (u32)r * 32u + (u32)lane;
     if (idx < n) {
       const u32 d = (k[r] >> shift) & 255u;
       const u32 pos = local_base[d] + warp_hist[w][d] + rank[r];
@@ -469,7 +475,7 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
     else kout[dst] = key;
     vout[dst] = val;
     // SELF: the next pass's per-tile histogram (of this pass's output arrangement), so that a pass is one launch
-    if (SELF && table_next) atomicAdd(&table_next[(dst / kSortTile) * 256u + ((key >> (shift + 8)) & 255u)], 1u);
+    if (SELF && table_next) atomicAdd(&table_next[(dst / TILE) * 256u + ((key >> (shift + 8)) & 255u)], 1u);
   }
 }
 
@@ -874,7 +880,7 @@ Workspace carve(void* base, int N, u64 capacity, int ntiles) {
   w.count_b = (u32*)take(16);
   w.table = (u32*)take(table_n * 4);
   {  // contiguous, zeroed by one memset per call
-    const u64 one = (u64)256 * (sort_blocks((u64)N) ? sort_blocks((u64)N) : 1);
+    const u64 one = (u64)256 * (((u64)N + kSmallTile - 1) / kSmallTile + 1);
     u32* base4 = (u32*)take(4 * one * 4);
     for (int i = 0; i < 4; ++i) w.dtable[i] = base4 + i * one;
   }
@@ -912,8 +918,8 @@ void radix_pass(const u32* kin, const u32* vin, u32* kout, u32* vout, u64* kout6
 // input (depth_keys_kernel for the first pass, the previous pass's scatter for the others)
 void radix_pass_small(const u32* kin, const u32* vin, u32* kout, u32* vout, const u32* count, u32 nblocks, int shift,
                       const u32* table, u32* table_next, cudaStream_t st) {
-  sort_scatter<false, true><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, nullptr, nullptr, count, table, nblocks, shift,
-                                                            table_next);
+  sort_scatter<false, true, kSmallItems><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, nullptr, nullptr, count, table,
+                                                                         nblocks, shift, table_next);
   launched();
 }
 
@@ -955,8 +961,8 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   }
   // A: depth order of the primitives (digits 0-3 of the 64-bit key)
   tm.begin(GABSPLAT_STAGE_DEPTH_SORT, st);
-  const u32 nba = sort_blocks((u64)N);
-  cudaMemsetAsync(ws.dtable[0], 0, (size_t)4 * 256 * nba * sizeof(u32), st);
+  const u32 nba = (u32)(((u64)N + kSmallTile - 1) / kSmallTile);
+  cudaMemsetAsync(ws.dtable[0], 0, (size_t)4 * 256 * (nba + 1) * sizeof(u32), st);
   depth_keys_kernel<<<(N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK, 256, 0, st>>>(N, proj.tiles_touched, proj.depth,
                                                                             proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis,
                                                                             ws.dtable[0]);
