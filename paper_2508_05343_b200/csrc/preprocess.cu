@@ -103,7 +103,9 @@ __device__ Index index_track(const Camera& c, float mx, float my, float mz, cons
 
 // fp64 value track of one visible primitive; everything it stores is rounded once to fp32.
 __device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camera& c, const gabsplat_projected& out,
-                                            const int i, const Index& ix) {
+                                            const int i) {
+  // the fp32 mean of the indexing track (index_kernel wrote it): the packed record carries it with its fp64 residual
+  const float2 m2 = reinterpret_cast<const float2*>(out.mean2d)[i];
   const int K = s.K;
   const float mx = s.means[3 * i], my = s.means[3 * i + 1], mz = s.means[3 * i + 2];
   float sc[3], q[4];
@@ -164,14 +166,11 @@ __device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camer
   reinterpret_cast<float4*>(out.conic_opacity)[i] = make_float4((float)ca, (float)cb, (float)cc, opac);
   // mu2D
   const double m2x = c.fx * t[0] / tz + c.cx, m2y = c.fy * t[1] / tz + c.cy;
-  reinterpret_cast<float2*>(out.mean2d)[i] = make_float2(ix.m2x, ix.m2y);
-  out.depth[i] = ix.depth;
-  reinterpret_cast<int4*>(out.rect)[i] = make_int4(ix.x0, ix.y0, ix.x1, ix.y1);
 
   const int R = packed_floats(K);
   float* rec = out.packed + (size_t)i * R;
   reinterpret_cast<float4*>(rec)[0] =
-      make_float4(ix.m2x, ix.m2y, (float)(m2x - (double)ix.m2x), (float)(m2y - (double)ix.m2y));
+      make_float4(m2.x, m2.y, (float)(m2x - (double)m2.x), (float)(m2y - (double)m2.y));
   {
     // conic = l l^T (Cholesky); q = -1/2 d^T conic d = -(u^2 + v^2) with L = l / sqrt(2)
     const double l11 = sqrt(ca), l21 = cb / l11, l22 = sqrt(fmax(cc - l21 * l21, 0.0));
@@ -240,67 +239,72 @@ __device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camer
   }
 }
 
-// One CTA of kPreThreads threads per chunk of kPreChunk consecutive primitives, in two phases:
-//  1. every thread runs the fp32 indexing track of kPreChunk / kPreThreads primitives (coalesced loads; the
-//     depth test on the mean comes first, so a primitive behind the camera costs 12 bytes) and appends the
-//     visible ones to a list in shared memory;
-//  2. the threads walk the compacted list and run the fp64 value track.  In the paper-shaped scenes only
-//     10-20 % of the primitives are visible: without the compaction the value track runs with 3-6 live lanes
-//     per warp (ncu: 4.2-9.9 thread instructions per warp instruction, profiles/r01_*).
+// Two kernels over chunks of kPreChunk consecutive primitives:
+//  index_kernel  the fp32 indexing track of every primitive (coalesced loads; the depth test on the mean comes
+//                first, so a primitive behind the camera costs 12 bytes): tiles_touched and radius for all, mean2d,
+//                depth and rect for the visible ones, the number of visible primitives per chunk.  Few registers,
+//                many warps per SM: it is a streaming kernel.
+//  value_kernel  compacts the visible primitives of its chunk (from tiles_touched, in index order) and runs the fp64
+//                value track over the compacted list.  In the paper-shaped scenes only 10-20 % of the primitives
+//                are visible: without the compaction the value track runs with 3-6 live lanes per warp, and fused
+//                with the indexing track its 128 registers hold the streaming part down to 16 warps per SM.
 constexpr int kPreThreads = 256;
 constexpr int kPreChunk = GABSPLAT_CHUNK;
 
-__global__ void __launch_bounds__(kPreThreads, 2) preprocess_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
-  __shared__ int s_i[kPreChunk];
-  __shared__ float s_m2x[kPreChunk], s_m2y[kPreChunk], s_depth[kPreChunk];
-  __shared__ uint32_t s_xy0[kPreChunk], s_xy1[kPreChunk];
+__global__ void __launch_bounds__(kPreThreads) index_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
   __shared__ int s_n;
   if (threadIdx.x == 0) s_n = 0;
   __syncthreads();
   const int base = blockIdx.x * kPreChunk;
+  int mine = 0;
 #pragma unroll 1
   for (int r = 0; r < kPreChunk / kPreThreads; ++r) {
     const int i = base + r * kPreThreads + threadIdx.x;
-    bool vis = false;
-    Index ix;
-    if (i < s.N) {
-      const float mx = s.means[3 * i], my = s.means[3 * i + 1], mz = s.means[3 * i + 2];
-      const float tz = ffma(c.w[8], mx, ffma(c.w[9], my, ffma(c.w[10], mz, c.w[11])));
-      uint32_t tiles = 0;
-      int radius = 0;
-      if (tz > c.z_near) {
-        float sc[3], q[4];
+    if (i >= s.N) break;
+    const float mx = s.means[3 * i], my = s.means[3 * i + 1], mz = s.means[3 * i + 2];
+    const float tz = ffma(c.w[8], mx, ffma(c.w[9], my, ffma(c.w[10], mz, c.w[11])));
+    uint32_t tiles = 0;
+    int radius = 0;
+    if (tz > c.z_near) {
+      float sc[3], q[4];
 #pragma unroll
-        for (int a = 0; a < 3; ++a) sc[a] = s.scales[3 * i + a];
-        const float4 qv = reinterpret_cast<const float4*>(s.rotations)[i];
-        q[0] = qv.x; q[1] = qv.y; q[2] = qv.z; q[3] = qv.w;
-        ix = index_track(c, mx, my, mz, sc, q);
-        vis = ix.visible;
-        tiles = ix.tiles;
-        radius = ix.radius;
+      for (int a = 0; a < 3; ++a) sc[a] = s.scales[3 * i + a];
+      const float4 qv = reinterpret_cast<const float4*>(s.rotations)[i];
+      q[0] = qv.x; q[1] = qv.y; q[2] = qv.z; q[3] = qv.w;
+      const Index ix = index_track(c, mx, my, mz, sc, q);
+      tiles = ix.tiles;
+      radius = ix.radius;
+      if (ix.visible) {
+        ++mine;
+        reinterpret_cast<float2*>(out.mean2d)[i] = make_float2(ix.m2x, ix.m2y);
+        out.depth[i] = ix.depth;
+        reinterpret_cast<int4*>(out.rect)[i] = make_int4(ix.x0, ix.y0, ix.x1, ix.y1);
       }
-      out.tiles_touched[i] = tiles;
-      out.radius[i] = radius;
     }
-    if (vis) {
-      const int slot = atomicAdd(&s_n, 1);
-      s_i[slot] = i;
-      s_m2x[slot] = ix.m2x; s_m2y[slot] = ix.m2y; s_depth[slot] = ix.depth;
-      s_xy0[slot] = (uint32_t)ix.x0 | ((uint32_t)ix.y0 << 16);  // tile coordinates fit 16 bits (api.cu checks)
-      s_xy1[slot] = (uint32_t)ix.x1 | ((uint32_t)ix.y1 << 16);
-    }
+    out.tiles_touched[i] = tiles;
+    out.radius[i] = radius;
   }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, d);
+  if ((threadIdx.x & 31) == 0 && mine) atomicAdd(&s_n, mine);
+  __syncthreads();
+  if (threadIdx.x == 0) out.chunk_visible[blockIdx.x] = (uint32_t)s_n;
+}
+
+constexpr int kValThreads = 128;
+
+__global__ void __launch_bounds__(kValThreads, 4) value_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
+  __shared__ int s_i[kPreChunk];
+  __shared__ int s_n;
+  if (out.chunk_visible[blockIdx.x] == 0) return;
+  if (threadIdx.x == 0) s_n = 0;
+  __syncthreads();
+  const int base = blockIdx.x * kPreChunk;
+  for (int i = base + threadIdx.x; i < min(s.N, base + kPreChunk); i += kValThreads)
+    if (out.tiles_touched[i] != 0) s_i[atomicAdd(&s_n, 1)] = i;
   __syncthreads();
   const int n = s_n;
-  if (threadIdx.x == 0) out.chunk_visible[blockIdx.x] = (uint32_t)n;
-  for (int j = threadIdx.x; j < n; j += kPreThreads) {
-    Index ix;
-    ix.visible = true;
-    ix.m2x = s_m2x[j]; ix.m2y = s_m2y[j]; ix.depth = s_depth[j];
-    ix.x0 = (int)(s_xy0[j] & 0xffffu); ix.y0 = (int)(s_xy0[j] >> 16);
-    ix.x1 = (int)(s_xy1[j] & 0xffffu); ix.y1 = (int)(s_xy1[j] >> 16);
-    value_track(s, c, out, s_i[j], ix);
-  }
+  for (int j = threadIdx.x; j < n; j += kValThreads) value_track(s, c, out, s_i[j]);
 }
 
 }  // namespace
@@ -308,8 +312,10 @@ __global__ void __launch_bounds__(kPreThreads, 2) preprocess_kernel(gabsplat_sce
 cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& out,
                               cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
-  preprocess_kernel<<<(s.N + kPreChunk - 1) / kPreChunk, kPreThreads, 0, st>>>(s, cam, out);
-  launched();
+  const int chunks = (s.N + kPreChunk - 1) / kPreChunk;
+  index_kernel<<<chunks, kPreThreads, 0, st>>>(s, cam, out);
+  value_kernel<<<chunks, kValThreads, 0, st>>>(s, cam, out);
+  launched(2);
   return cudaGetLastError();
 }
 
