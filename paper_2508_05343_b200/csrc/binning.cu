@@ -1,15 +1,17 @@
 // S2 / K2-K5: tile binning.  (PAPER.md:103 "sorted by depth", :160 "tile-based rasterizer".)
 // The result is the list of (primitive, tile) instances ordered by the 64-bit key (tile << 32) | bits(depth),
 // ties by primitive index -- exactly what a stable LSD radix sort of the keys on one-byte digits gives -- plus
-// the [start,end) range of every tile.  The LSD passes are split around the duplication step so that the four
-// depth digits are sorted on the N primitives, not on the D >> N instances:
+// the [start,end) range of every tile.  The depth digits are sorted on the visible primitives, not on the D >> N
+// instances; the tile digit then takes one more stable pass:
 //   A   (bits(depth), index) of the n_vis visible primitives, compacted in index order; 4 stable one-byte
 //       passes over them -> `order`: visible primitives front to back, ties by index
-//   K2  inclusive prefix sum of tiles_touched taken in that order               -> offsets, D
-//   K3  one (tile,id) per (primitive, tile of its rectangle), emitted in depth order, row-major over the rectangle
-//   B   ceil(tile_bits / 8) stable one-byte passes on the tile id over the D instances; the last pass writes the
-//       64-bit key (tile | depth gathered by id) and the id
-//   K5  [start,end) of every tile in the sorted list
+//   K2  inclusive prefix over that order of the placement cost (B') or of tiles_touched (B) -> offsets (and D for B)
+//   B'  images of at most 26000 tiles: ONE stable counting pass on the whole tile id -- per-(tile, chunk) counts,
+//       their prefix (tile ranges and D fall out of it), then every instance id written once at its final slot;
+//       the 64-bit keys (tile | depth) are written by a coalesced pass if the caller wants them
+//   B   larger images: K3 one (tile,id) per (primitive, tile of its rectangle), emitted in depth order, row-major
+//       over the rectangle; ceil(tile_bits / 8) stable one-byte passes on the tile id over the D instances, the
+//       last one writing the 64-bit key and the id; K5 [start,end) of every tile from the sorted keys
 // LSD order is preserved: digits 0-3 (depth) before digits 4.. (tile), every pass stable.  Everything is
 // integer work; the result must equal std::stable_sort of the 64-bit keys bit for bit.
 // The instance count D lives on the device: every kernel is launched on a grid sized from the caller's

@@ -4,8 +4,10 @@
 // explicit round-to-nearest intrinsics (no compiler-chosen contraction), so that they take bit-identical
 // skip / clamp decisions.
 //
-// Mapping.  One CTA of 64 threads (2 warps) per 16x16 tile; every thread owns kSlots = 4 pixels: lane l of
-// warp w owns column l & 15 and rows 8w + 2s + (l >> 4), s = 0..3.  Slot s of a warp is therefore a 16x2 strip.
+// Mapping.  A warp owns half a 16x16 tile (16x8 pixels) and every thread kSlots = 4 pixels: lane l of warp w
+// owns column l & 15 and rows 8w + 2s + (l >> 4), s = 0..3.  Slot s of a warp is therefore a 16x2 strip.  The
+// forward runs the two warps of a tile as one CTA (they share the staging); the backward, whose warps replay
+// independent lists, runs every half tile as a CTA of its own.
 // A staged record is read from shared memory once per thread and used for 4 pixels.
 //
 // Staging.  The tile's list is consumed in batches of kBatch entries.  Each thread fetches the 32-byte head of
