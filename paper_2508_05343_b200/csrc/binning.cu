@@ -502,28 +502,22 @@ __global__ void __launch_bounds__(256) tile_ranges_kernel(const u64* __restrict_
 // work / max; the order inside a bucket is immaterial.
 // ------------------------------------------------------------------------------------------------
 // MODE 0: work(t) = pairs[t].y - pairs[t].x;  1: pairs[t].x + pairs[t].y;  2: ((const u32*)pairs)[t]
-template <int MODE>
-__global__ void __launch_bounds__(1024) tile_order_kernel(const uint2* __restrict__ pairs, u32 ntiles, u32* __restrict__ order) {
-  auto work = [&](u32 t) -> u32 {
-    if (MODE == 2) return reinterpret_cast<const u32*>(pairs)[t];
-    const uint2 p = pairs[t];
-    return MODE == 1 ? p.x + p.y : p.y - p.x;
-  };
+// order[] = the items 0..n-1 by descending work(item): one CTA, max, 256-bucket counting sort by work / max
+template <typename Work>
+__device__ __forceinline__ void block_order_descending(Work work, u32 n, u32* __restrict__ order) {
   __shared__ u32 s_max, s_hist[256], s_base[256];
   if (threadIdx.x == 0) s_max = 0;
   if (threadIdx.x < 256) s_hist[threadIdx.x] = 0;
   __syncthreads();
   u32 mx = 0;
-  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) {
-    mx = max(mx, work(t));
-  }
+  for (u32 t = threadIdx.x; t < n; t += blockDim.x) mx = max(mx, work(t));
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, d));
   if ((threadIdx.x & 31) == 0) atomicMax(&s_max, mx);
   __syncthreads();
   const float scale = 255.0f / (float)max(s_max, 1u);
   auto bucket = [&](u32 t) { return 255u - min(255u, (u32)((float)work(t) * scale)); };
-  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) atomicAdd(&s_hist[bucket(t)], 1u);
+  for (u32 t = threadIdx.x; t < n; t += blockDim.x) atomicAdd(&s_hist[bucket(t)], 1u);
   __syncthreads();
   if (threadIdx.x < 32) {  // exclusive scan of 256 counts by one warp, 8 per lane
     u32 c[8], tot = 0;
@@ -534,7 +528,16 @@ __global__ void __launch_bounds__(1024) tile_order_kernel(const uint2* __restric
     for (int j = 0; j < 8; ++j) { s_base[threadIdx.x * 8 + j] = run; run += c[j]; }
   }
   __syncthreads();
-  for (u32 t = threadIdx.x; t < ntiles; t += blockDim.x) order[atomicAdd(&s_base[bucket(t)], 1u)] = t;
+  for (u32 t = threadIdx.x; t < n; t += blockDim.x) order[atomicAdd(&s_base[bucket(t)], 1u)] = t;
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(1024) tile_order_kernel(const uint2* __restrict__ pairs, u32 ntiles, u32* __restrict__ order) {
+  block_order_descending([&](u32 t) -> u32 {
+    if (MODE == 2) return reinterpret_cast<const u32*>(pairs)[t];
+    const uint2 p = pairs[t];
+    return MODE == 1 ? p.x + p.y : p.y - p.x;
+  }, ntiles, order);
 }
 
 __global__ void clamp_count_kernel(u32* sort_count, const u32* num_instances, u64 capacity) {
@@ -563,11 +566,10 @@ constexpr int kStep = 32;          // primitives per step (one mask bit each)
 constexpr int kMaxTilesCounting = 26000;  // 2 * 4 B * tiles (and 4 B * (tiles_x+1)(tiles_y+1)) of shared memory must fit in 227 KB
 
 // boundary c of the chunking: the number of ranks r < n_vis whose inclusive cost prefix is <= c * total / kChunks
-__global__ void __launch_bounds__(256) chunk_bounds_kernel(const u32* __restrict__ offsets, const u32* __restrict__ n_vis_p,
-                                                           u32* __restrict__ bounds) {
+__device__ __forceinline__ void chunk_bound(const u32* __restrict__ offsets, const u32* __restrict__ n_vis_p,
+                                            u32* __restrict__ bounds, u32 c) {
   __shared__ u32 s_lo, s_hi, s_cnt[8];
   const u32 n_vis = *n_vis_p;
-  const u32 c = blockIdx.x;
   if (n_vis == 0) { if (threadIdx.x == 0) bounds[c] = 0; return; }
   const u64 total = (u64)__ldg(offsets + n_vis - 1);  // offsets = inclusive prefix of place_cost in depth order
   const u64 target = total * c / kChunks;
@@ -596,11 +598,15 @@ __global__ void __launch_bounds__(256) chunk_bounds_kernel(const u32* __restrict
 
 // record r of the depth-ordered visible primitives: (id, bits(depth), x0 | y0 << 16, x1 | y1 << 16): what the two
 // walks below read, coalesced, instead of chasing order -> rect / depth per primitive
-__global__ void __launch_bounds__(256) visible_records_kernel(const u32* __restrict__ order, const int4* __restrict__ rect,
-                                                              const float* __restrict__ depth, const u32* __restrict__ n_vis_p,
-                                                              uint4* __restrict__ recs) {
+// One launch for two independent jobs: CTAs 0..kChunks compute the chunk boundaries, the others write the records.
+constexpr int kRecordCtas = 148 * 4;
+__global__ void __launch_bounds__(256) bounds_records_kernel(const u32* __restrict__ offsets, const u32* __restrict__ order,
+                                                             const int4* __restrict__ rect, const float* __restrict__ depth,
+                                                             const u32* __restrict__ n_vis_p, u32* __restrict__ bounds,
+                                                             uint4* __restrict__ recs) {
+  if (blockIdx.x <= kChunks) { chunk_bound(offsets, n_vis_p, bounds, blockIdx.x); return; }
   const u32 n_vis = *n_vis_p;
-  for (u32 r = blockIdx.x * blockDim.x + threadIdx.x; r < n_vis; r += gridDim.x * blockDim.x) {
+  for (u32 r = (blockIdx.x - kChunks - 1) * blockDim.x + threadIdx.x; r < n_vis; r += kRecordCtas * blockDim.x) {
     const u32 id = __ldg(order + r);
     const int4 rc = __ldg(rect + id);
     recs[r] = make_uint4(id, __float_as_uint(__ldg(depth + id)), (u32)rc.x | ((u32)rc.y << 16), (u32)rc.z | ((u32)rc.w << 16));
@@ -680,7 +686,7 @@ __global__ void __launch_bounds__(256) tile_scan_kernel(int ntiles, u32* __restr
 // tile and for every tile when the instances do not fit the caller's buffers)
 __global__ void __launch_bounds__(1024) tile_ranges_scan_kernel(int ntiles, const u32* __restrict__ totals,
                                                                u32* __restrict__ num_instances, u64 capacity,
-                                                               uint2* __restrict__ ranges) {
+                                                               uint2* __restrict__ ranges, u32* __restrict__ order) {
   __shared__ u32 s_warp[32], s_carry;
   __shared__ unsigned long long s_total;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -716,6 +722,8 @@ __global__ void __launch_bounds__(1024) tile_ranges_scan_kernel(int ntiles, cons
     if (threadIdx.x == 1023) s_carry = start + v;
     __syncthreads();
   }
+  // launch order of the forward blend: tiles by descending list length
+  block_order_descending([&](u32 t) -> u32 { return fits ? totals[t] : 0u; }, (u32)ntiles, order);
 }
 
 constexpr int kFlat = 8;  // instances a thread keeps in registers during a step
@@ -995,18 +1003,16 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
     const int4* rect = reinterpret_cast<const int4*>(proj.rect);
     uint2* ranges = reinterpret_cast<uint2*>(bin.tile_ranges);
     tm.begin(GABSPLAT_STAGE_DUPLICATE, st);
-    chunk_bounds_kernel<<<kChunks + 1, 256, 0, st>>>(bin.offsets, ws.n_vis, ws.bounds);
-    visible_records_kernel<<<148 * 4, 256, 0, st>>>(order, rect, proj.depth, ws.n_vis, ws.recs);
+    bounds_records_kernel<<<kChunks + 1 + kRecordCtas, 256, 0, st>>>(bin.offsets, order, rect, proj.depth, ws.n_vis, ws.bounds,
+                                                                     ws.recs);
     tile_count_kernel<<<kChunks, kPlaceThreads, smem_count, st>>>(cam.tiles_x, cam.tiles_y, ws.recs, ws.bounds, ws.chunk_table);
-    launched(3);
+    launched(2);
     tm.end(st);
     tm.begin(GABSPLAT_STAGE_RANGES, st);
     tile_scan_kernel<<<(ntiles + 7) / 8, 256, 0, st>>>(ntiles, ws.chunk_table, ws.totals);
-    tile_ranges_scan_kernel<<<1, 1024, 0, st>>>(ntiles, ws.totals, bin.num_instances, bin.capacity, ranges);
+    tile_ranges_scan_kernel<<<1, 1024, 0, st>>>(ntiles, ws.totals, bin.num_instances, bin.capacity, ranges, bin.tile_order);
     launched(2);
-    const cudaError_t eo = launch_tile_order(bin.tile_ranges, false, ntiles, bin.tile_order, st);
     tm.end(st);
-    if (eo != cudaSuccess) return eo;
     tm.begin(GABSPLAT_STAGE_SORT, st);
     // bands of at most ~1280 tiles: measured best on both the 4346-tile and the 9840-tile configs
     // (GABSPLAT_PLACE_BANDS overrides the number of bands: a test / tuning hook)
