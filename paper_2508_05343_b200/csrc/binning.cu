@@ -142,11 +142,24 @@ __global__ void __launch_bounds__(kScanThreads) scan_of_sums(u32* __restrict__ s
   if (threadIdx.x == 0 && total_out) *total_out = carry;
 }
 
-template <bool INCLUSIVE, bool GATHER>
+// SELFSUM: `sums` holds the raw block sums and every CTA adds up those of the CTAs before it itself (a few hundred
+// at most): the scan is two launches; the last CTA writes the grand total.
+template <bool INCLUSIVE, bool GATHER, bool SELFSUM>
 __global__ void __launch_bounds__(kScanThreads) scan_apply(const u32* __restrict__ in, const u32* __restrict__ idx, u32 n,
                                                             const u32* __restrict__ n_dev, u32 cost_thr,
-                                                            const u32* __restrict__ sums, u32* __restrict__ out) {
+                                                            const u32* __restrict__ sums, u32* __restrict__ out,
+                                                            u32* __restrict__ total_out) {
   if (n_dev) n = min(n, *n_dev);
+  u32 before = 0;
+  if (SELFSUM) {
+    u32 acc = 0;
+    for (u32 b = threadIdx.x; b < blockIdx.x; b += kScanThreads) acc += __ldg(sums + b);
+    u32 tot;
+    block_exclusive_scan(acc, &tot);
+    before = tot;
+  } else {
+    before = sums[blockIdx.x];
+  }
   const u32 base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
   u32 v[kScanItems];
   scan_load<GATHER>(in, idx, base, n, cost_thr, v);
@@ -154,7 +167,8 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply(const u32* __restrict
 #pragma unroll
   for (int j = 0; j < kScanItems; ++j) s += v[j];
   u32 total;
-  u32 run = block_exclusive_scan(s, &total) + sums[blockIdx.x];
+  u32 run = block_exclusive_scan(s, &total) + before;
+  if (SELFSUM && total_out && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *total_out = before + total;
 #pragma unroll
   for (int j = 0; j < kScanItems; ++j) {
     const u32 e = run;
@@ -184,8 +198,13 @@ void device_scan(const u32* in, const u32* idx, u32* out, u32 n, const u32* n_de
     return;
   }
   scan_block_sums<GATHER><<<nb, kScanThreads, 0, st>>>(in, idx, n, n_dev, cost_thr, sums);
+  if (nb <= 2048) {
+    scan_apply<INCLUSIVE, GATHER, true><<<nb, kScanThreads, 0, st>>>(in, idx, n, n_dev, cost_thr, sums, out, total_out);
+    launched(2);
+    return;
+  }
   scan_of_sums<<<1, kScanThreads, 0, st>>>(sums, nb, total_out);
-  scan_apply<INCLUSIVE, GATHER><<<nb, kScanThreads, 0, st>>>(in, idx, n, n_dev, cost_thr, sums, out);
+  scan_apply<INCLUSIVE, GATHER, false><<<nb, kScanThreads, 0, st>>>(in, idx, n, n_dev, cost_thr, sums, out, nullptr);
   launched(3);
 }
 
