@@ -4,7 +4,7 @@
 // (reading C25).  It produces dL/dimage, the input of gabsplat_render_backward, without leaving the GPU.
 //
 // Two tiled passes, both HBM bound (26 MB in + 39 MB out, then 65 MB in + 13 MB out at 1297x840):
-//   ssim_maps_kernel   per 32x8 tile of one channel: the five windowed sums w*x, w*y, w*x^2, w*y^2, w*xy as a
+//   ssim_maps_kernel   per 32x16 tile of one channel: the five windowed sums w*x, w*y, w*x^2, w*y^2, w*xy as a
 //                      separable 11-tap filter through shared memory, SSIM and its three partial derivatives
 //                      (dS/dmx, dS/dExx, dS/dExy) per pixel, per-CTA partial sums of |x - y| and SSIM
 //   loss_grad_kernel   the same separable filter over the three derivative maps, combined with x, y and sign(x - y)
@@ -16,7 +16,7 @@ namespace gabsplat {
 namespace {
 
 constexpr int kR = 5;             // window radius
-constexpr int kTX = 32, kTY = 8;   // output tile: one pixel per thread
+constexpr int kTX = 32, kTY = 16;  // output tile: two pixels per thread (rows ty and ty + 8)
 constexpr int kHX = kTX + 2 * kR, kHY = kTY + 2 * kR;
 constexpr int kLossThreads = 256;
 constexpr double kC1 = 0.01 * 0.01, kC2 = 0.03 * 0.03;
@@ -32,10 +32,10 @@ inline Taps make_taps() {
 }
 
 // Separable filter of NQ quantities over one tile.  in(r, c, v) gives the NQ input values at halo position (r, c)
-// (zero outside the image); s_h[q][kHY][kTX] receives the horizontal sums; out[q] = the filtered value at the
-// thread's output pixel (tile row ty, column tx).
+// (zero outside the image); s_h[q][kHY][kTX] receives the horizontal sums; out[q][h] = the filtered value at the
+// thread's output pixels (tile rows ty + 8 h, column tx).
 template <int NQ, typename In>
-__device__ __forceinline__ void separable(const Taps& taps, In in, double (*s_h)[kHY][kTX], int tx, int ty, double (&out)[NQ]) {
+__device__ __forceinline__ void separable(const Taps& taps, In in, double (*s_h)[kHY][kTX], int tx, int ty, double (&out)[NQ][2]) {
   for (int e = threadIdx.x; e < kHY * kTX; e += kLossThreads) {
     const int r = e / kTX, c = e - r * kTX;
     double acc[NQ];
@@ -53,12 +53,14 @@ __device__ __forceinline__ void separable(const Taps& taps, In in, double (*s_h)
   }
   __syncthreads();
 #pragma unroll
-  for (int q = 0; q < NQ; ++q) {
-    double acc = 0.0;
+  for (int q = 0; q < NQ; ++q)
 #pragma unroll
-    for (int i = 0; i <= 2 * kR; ++i) acc += taps.g[i] * s_h[q][ty + i][tx];
-    out[q] = acc;
-  }
+    for (int h = 0; h < 2; ++h) {
+      double acc = 0.0;
+#pragma unroll
+      for (int i = 0; i <= 2 * kR; ++i) acc += taps.g[i] * s_h[q][ty + 8 * h + i][tx];
+      out[q][h] = acc;
+    }
 }
 
 __global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, Taps taps, const float* __restrict__ image,
@@ -81,15 +83,18 @@ __global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, T
   }
   __syncthreads();
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-  double f[5];
+  double f[5][2];
   separable<5>(taps, [&](int r, int c, double (&v)[5]) {
     const double a = s_x[r][c], b = s_y[r][c];
     v[0] = a; v[1] = b; v[2] = a * a; v[3] = b * b; v[4] = a * b;
   }, s_h, tx, ty, f);
   double sum_l1 = 0.0, sum_s = 0.0;
-  const int gx = blockIdx.x * kTX + tx, gy = blockIdx.y * kTY + ty;
-  if (gx < W && gy < H) {
-    const double mx = f[0], my = f[1], exx = f[2], eyy = f[3], exy = f[4];
+  const int gx = blockIdx.x * kTX + tx;
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int gy = blockIdx.y * kTY + ty + 8 * h;
+    if (gx >= W || gy >= H) continue;
+    const double mx = f[0][h], my = f[1][h], exx = f[2][h], eyy = f[3][h], exy = f[4][h];
     const double a1 = 2.0 * mx * my + kC1, a2 = 2.0 * (exy - mx * my) + kC2;
     const double b1 = mx * mx + my * my + kC1, b2 = (exx - mx * mx) + (eyy - my * my) + kC2;
     const double ib = 1.0 / (b1 * b2);
@@ -98,8 +103,8 @@ __global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, T
     maps[(0 * 3 + ch) * HW + p] = (float)((2.0 * my * a2 - 2.0 * my * a1) * ib - sv * (2.0 * mx / b1 - 2.0 * mx / b2));
     maps[(1 * 3 + ch) * HW + p] = (float)(-sv / b2);
     maps[(2 * 3 + ch) * HW + p] = (float)(2.0 * a1 * ib);
-    sum_s = sv;
-    sum_l1 = fabs((double)s_x[ty + kR][tx + kR] - (double)s_y[ty + kR][tx + kR]);
+    sum_s += sv;
+    sum_l1 += fabs((double)s_x[ty + 8 * h + kR][tx + kR] - (double)s_y[ty + 8 * h + kR][tx + kR]);
   }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) {
@@ -155,19 +160,22 @@ __global__ void __launch_bounds__(kLossThreads) loss_grad_kernel(int W, int H, T
   }
   __syncthreads();
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-  double f[3];
+  double f[3][2];
   separable<3>(taps, [&](int r, int c, double (&v)[3]) {
     v[0] = s_in[0][r][c]; v[1] = s_in[1][r][c]; v[2] = s_in[2][r][c];
   }, s_h, tx, ty, f);
   const double n = 3.0 * (double)HW;
   const double gs = -(double)lambda / n, g1 = (1.0 - (double)lambda) / n;
-  const int gx = blockIdx.x * kTX + tx, gy = blockIdx.y * kTY + ty;
-  if (gx < W && gy < H) {
+  const int gx = blockIdx.x * kTX + tx;
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const int gy = blockIdx.y * kTY + ty + 8 * h;
+    if (gx >= W || gy >= H) continue;
     const size_t p = (size_t)gy * W + gx;
     const double xv = image[ch * HW + p], yv = target[ch * HW + p];
     const double d = xv - yv;
     const double sgn = d > 0.0 ? 1.0 : (d < 0.0 ? -1.0 : 0.0);
-    dL_dimage[ch * HW + p] = (float)(gs * (f[0] + 2.0 * xv * f[1] + yv * f[2]) + g1 * sgn);
+    dL_dimage[ch * HW + p] = (float)(gs * (f[0][h] + 2.0 * xv * f[1][h] + yv * f[2][h]) + g1 * sgn);
   }
 }
 
