@@ -116,6 +116,7 @@ __device__ __forceinline__ void scan_load_raw(const u32* __restrict__ in, const 
 template <bool GATHER>
 __global__ void __launch_bounds__(kScanThreads) scan_block_sums(const u32* __restrict__ in, const u32* __restrict__ idx, u32 n,
                                                                  const u32* __restrict__ n_dev, u32 cost_thr, u32* __restrict__ sums) {
+  pdl_wait();
   if (n_dev) n = min(n, *n_dev);  // the element count lives on the device (n is its host-side bound)
   const u32 base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
   u32 v[kScanItems];
@@ -149,6 +150,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_apply(const u32* __restrict
                                                             const u32* __restrict__ n_dev, u32 cost_thr,
                                                             const u32* __restrict__ sums, u32* __restrict__ out,
                                                             u32* __restrict__ total_out) {
+  pdl_wait();
   if (n_dev) n = min(n, *n_dev);
   u32 before = 0;
   if (SELFSUM) {
@@ -197,14 +199,14 @@ void device_scan(const u32* in, const u32* idx, u32* out, u32 n, const u32* n_de
     launched();
     return;
   }
-  scan_block_sums<GATHER><<<nb, kScanThreads, 0, st>>>(in, idx, n, n_dev, cost_thr, sums);
+  launch_pdl(scan_block_sums<GATHER>, nb, kScanThreads, 0, st, in, idx, n, n_dev, cost_thr, sums);
   if (nb <= 2048) {
-    scan_apply<INCLUSIVE, GATHER, true><<<nb, kScanThreads, 0, st>>>(in, idx, n, n_dev, cost_thr, sums, out, total_out);
+    launch_pdl(scan_apply<INCLUSIVE, GATHER, true>, nb, kScanThreads, 0, st, in, idx, n, n_dev, cost_thr, sums, out, total_out);
     launched(2);
     return;
   }
   scan_of_sums<<<1, kScanThreads, 0, st>>>(sums, nb, total_out);
-  scan_apply<INCLUSIVE, GATHER, false><<<nb, kScanThreads, 0, st>>>(in, idx, n, n_dev, cost_thr, sums, out, nullptr);
+  launch_pdl(scan_apply<INCLUSIVE, GATHER, false>, nb, kScanThreads, 0, st, in, idx, n, n_dev, cost_thr, sums, out, (u32*)nullptr);
   launched(3);
 }
 
@@ -390,6 +392,7 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
                                                             u64* __restrict__ kout64, const u32* __restrict__ gather,
                                                             const u32* __restrict__ count, const u32* __restrict__ table,
                                                             u32 nblocks, int shift, u32* __restrict__ table_next) {
+  pdl_wait();
   __shared__ u32 warp_hist[kSortWarps][256];
   __shared__ u32 local_base[256];
   __shared__ u32 global_base[256];
@@ -623,6 +626,7 @@ __global__ void __launch_bounds__(256) bounds_records_kernel(const u32* __restri
                                                              const int4* __restrict__ rect, const float* __restrict__ depth,
                                                              const u32* __restrict__ n_vis_p, u32* __restrict__ bounds,
                                                              uint4* __restrict__ recs) {
+  pdl_wait();
   if (blockIdx.x <= kChunks) { chunk_bound(offsets, n_vis_p, bounds, blockIdx.x); return; }
   const u32 n_vis = *n_vis_p;
   for (u32 r = (blockIdx.x - kChunks - 1) * blockDim.x + threadIdx.x; r < n_vis; r += kRecordCtas * blockDim.x) {
@@ -654,6 +658,7 @@ __device__ __forceinline__ void for_rect_tiles(u32 xy0, u32 xy1, int tiles_x, in
 // array in shared memory: four corner updates per primitive, then prefix sums along x and along y.
 __global__ void __launch_bounds__(kPlaceThreads) tile_count_kernel(int tiles_x, int tiles_y, const uint4* __restrict__ recs,
                                                                    const u32* __restrict__ bounds, u32* __restrict__ table) {
+  pdl_wait();
   extern __shared__ int s_d[];  // [(tiles_y + 1)][(tiles_x + 1)]
   const int sx = tiles_x + 1, sy = tiles_y + 1;
   for (int t = threadIdx.x; t < sx * sy; t += kPlaceThreads) s_d[t] = 0;
@@ -686,6 +691,7 @@ __global__ void __launch_bounds__(kPlaceThreads) tile_count_kernel(int tiles_x, 
 
 // a warp per tile: exclusive prefix of table[tile][0..kChunks) in place, total to totals[tile]
 __global__ void __launch_bounds__(256) tile_scan_kernel(int ntiles, u32* __restrict__ table, u32* __restrict__ totals) {
+  pdl_wait();
   const int lane = threadIdx.x & 31;
   const int t = blockIdx.x * 8 + (threadIdx.x >> 5);
   if (t >= ntiles) return;
@@ -706,6 +712,7 @@ __global__ void __launch_bounds__(256) tile_scan_kernel(int ntiles, u32* __restr
 __global__ void __launch_bounds__(1024) tile_ranges_scan_kernel(int ntiles, const u32* __restrict__ totals,
                                                                u32* __restrict__ num_instances, u64 capacity,
                                                                uint2* __restrict__ ranges, u32* __restrict__ order) {
+  pdl_wait();
   __shared__ u32 s_warp[32], s_carry;
   __shared__ unsigned long long s_total;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -765,6 +772,7 @@ __global__ void __launch_bounds__(THREADS, THREADS == 1024 ? 2 : 4) tile_place_k
                                                                    const uint2* __restrict__ ranges,
                                                                    const u32* __restrict__ num_instances, u64 capacity,
                                                                    int band_rows, u32* __restrict__ ids) {
+  pdl_wait();
   constexpr u32 kStepInstances = kFlat * THREADS;
   // CTA (chunk, band): the chunk's primitives clipped to the band's tile rows [ylo, yhi).  Bands keep the two
   // per-tile arrays small (many CTAs per SM for this latency-bound walk) and, because the CTAs of a band are
@@ -937,9 +945,9 @@ void radix_pass(const u32* kin, const u32* vin, u32* kout, u32* vout, u64* kout6
   launched();
   device_scan<false, false>(ws.table, nullptr, ws.table, 256u * nblocks, nullptr, 0u, ws.scan_sums, nullptr, st);
   if (kout64)
-    sort_scatter<true, false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, nullptr);
+    launch_pdl(sort_scatter<true, false>, nblocks, kSortThreads, 0, st, kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, (u32*)nullptr);
   else
-    sort_scatter<false, false><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, nullptr);
+    launch_pdl(sort_scatter<false, false>, nblocks, kSortThreads, 0, st, kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, (u32*)nullptr);
   launched();
 }
 
@@ -947,8 +955,8 @@ void radix_pass(const u32* kin, const u32* vin, u32* kout, u32* vout, u64* kout6
 // input (depth_keys_kernel for the first pass, the previous pass's scatter for the others)
 void radix_pass_small(const u32* kin, const u32* vin, u32* kout, u32* vout, const u32* count, u32 nblocks, int shift,
                       const u32* table, u32* table_next, cudaStream_t st) {
-  sort_scatter<false, true, kSmallItems><<<nblocks, kSortThreads, 0, st>>>(kin, vin, kout, vout, nullptr, nullptr, count, table,
-                                                                         nblocks, shift, table_next);
+  launch_pdl(sort_scatter<false, true, kSmallItems>, nblocks, kSortThreads, 0, st, kin, vin, kout, vout, (u64*)nullptr,
+             (const u32*)nullptr, count, table, nblocks, shift, table_next);
   launched();
 }
 
@@ -1022,14 +1030,14 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
     const int4* rect = reinterpret_cast<const int4*>(proj.rect);
     uint2* ranges = reinterpret_cast<uint2*>(bin.tile_ranges);
     tm.begin(GABSPLAT_STAGE_DUPLICATE, st);
-    bounds_records_kernel<<<kChunks + 1 + kRecordCtas, 256, 0, st>>>(bin.offsets, order, rect, proj.depth, ws.n_vis, ws.bounds,
-                                                                     ws.recs);
-    tile_count_kernel<<<kChunks, kPlaceThreads, smem_count, st>>>(cam.tiles_x, cam.tiles_y, ws.recs, ws.bounds, ws.chunk_table);
+    launch_pdl(bounds_records_kernel, kChunks + 1 + kRecordCtas, 256, 0, st, bin.offsets, order, rect, proj.depth, ws.n_vis,
+               ws.bounds, ws.recs);
+    launch_pdl(tile_count_kernel, kChunks, kPlaceThreads, smem_count, st, cam.tiles_x, cam.tiles_y, ws.recs, ws.bounds, ws.chunk_table);
     launched(2);
     tm.end(st);
     tm.begin(GABSPLAT_STAGE_RANGES, st);
-    tile_scan_kernel<<<(ntiles + 7) / 8, 256, 0, st>>>(ntiles, ws.chunk_table, ws.totals);
-    tile_ranges_scan_kernel<<<1, 1024, 0, st>>>(ntiles, ws.totals, bin.num_instances, bin.capacity, ranges, bin.tile_order);
+    launch_pdl(tile_scan_kernel, (ntiles + 7) / 8, 256, 0, st, ntiles, ws.chunk_table, ws.totals);
+    launch_pdl(tile_ranges_scan_kernel, 1, 1024, 0, st, ntiles, ws.totals, bin.num_instances, bin.capacity, ranges, bin.tile_order);
     launched(2);
     tm.end(st);
     tm.begin(GABSPLAT_STAGE_SORT, st);
@@ -1043,8 +1051,8 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
     const size_t smem_place = 2 * (size_t)band_rows * cam.tiles_x * sizeof(u32);
     if (smem_place > 48 * 1024)
       cudaFuncSetAttribute(tile_place_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_place);
-    tile_place_kernel<256><<<dim3(kChunks, nb), 256, smem_place, st>>>(ntiles, cam.tiles_x, ws.recs, ws.bounds, ws.chunk_table,
-                                                                      ranges, bin.num_instances, bin.capacity, band_rows, bin.ids);
+    launch_pdl(tile_place_kernel<256>, dim3(kChunks, nb), 256, smem_place, st, ntiles, cam.tiles_x, ws.recs, ws.bounds,
+               ws.chunk_table, ranges, bin.num_instances, bin.capacity, band_rows, bin.ids);
     launched();
     if (bin.keys) {
       tile_keys_kernel<<<(ntiles + 1) / 2, 256, 0, st>>>(ntiles, ranges, bin.ids, proj.depth, bin.keys);

@@ -116,6 +116,24 @@ struct StageTimer {
   }
 };
 
+// ---- programmatic dependent launch ---------------------------------------------------------------------
+// The small kernels of a call form a chain of dependent launches whose cost is mostly launch latency.  Launched
+// with launch_pdl, a kernel may be scheduled while its predecessor in the stream drains; it must call pdl_wait()
+// before it touches anything the predecessor wrote (first statement of every kernel launched this way).
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+#endif
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // Number of kernels launched by this library since it was loaded (gabsplat_kernel_launches).
 extern unsigned long long g_kernel_launches;
 inline void launched(int n = 1) { g_kernel_launches += (unsigned long long)n; }
