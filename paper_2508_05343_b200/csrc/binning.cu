@@ -221,6 +221,7 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __res
                                                          const float* __restrict__ depth, const u32* __restrict__ chunk_visible,
                                                          u32* __restrict__ keys, u32* __restrict__ vals, u32* __restrict__ n_vis,
                                                          u32* __restrict__ table0) {
+  pdl_wait();
   __shared__ u32 s_part[8], s_off;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   u32 acc = 0;
@@ -555,6 +556,7 @@ __device__ __forceinline__ void block_order_descending(Work work, u32 n, u32* __
 
 template <int MODE>
 __global__ void __launch_bounds__(1024) tile_order_kernel(const uint2* __restrict__ pairs, u32 ntiles, u32* __restrict__ order) {
+  pdl_wait();
   block_order_descending([&](u32 t) -> u32 {
     if (MODE == 2) return reinterpret_cast<const u32*>(pairs)[t];
     const uint2 p = pairs[t];
@@ -867,6 +869,7 @@ __global__ void __launch_bounds__(THREADS, THREADS == 1024 ? 2 : 4) tile_place_k
 // kernels never read the keys; they are the inspectable statement of the order.)
 __global__ void __launch_bounds__(256) tile_keys_kernel(int ntiles, const uint2* __restrict__ ranges, const u32* __restrict__ ids,
                                                         const float* __restrict__ depth, u64* __restrict__ keys) {
+  pdl_wait();
   // half a CTA (128 threads) per tile, two instances per thread and iteration in flight
   const int t = blockIdx.x * 2 + (threadIdx.x >> 7);
   if (t >= ntiles) return;
@@ -964,15 +967,15 @@ void radix_pass_small(const u32* kin, const u32* vin, u32* kout, u32* vout, cons
 
 cudaError_t launch_tile_order(const uint32_t* pairs, bool sum, int ntiles, uint32_t* order, cudaStream_t st) {
   if (ntiles <= 0) return cudaSuccess;
-  if (sum) tile_order_kernel<1><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
-  else tile_order_kernel<0><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
+  if (sum) launch_pdl(tile_order_kernel<1>, 1, 1024, 0, st, reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
+  else launch_pdl(tile_order_kernel<0>, 1, 1024, 0, st, reinterpret_cast<const uint2*>(pairs), (u32)ntiles, order);
   launched();
   return cudaGetLastError();
 }
 
 cudaError_t launch_half_tile_order(const uint32_t* work, int n, uint32_t* order, cudaStream_t st) {
   if (n <= 0) return cudaSuccess;
-  tile_order_kernel<2><<<1, 1024, 0, st>>>(reinterpret_cast<const uint2*>(work), (u32)n, order);
+  launch_pdl(tile_order_kernel<2>, 1, 1024, 0, st, reinterpret_cast<const uint2*>(work), (u32)n, order);
   launched();
   return cudaGetLastError();
 }
@@ -1000,9 +1003,8 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   tm.begin(GABSPLAT_STAGE_DEPTH_SORT, st);
   const u32 nba = (u32)(((u64)N + kSmallTile - 1) / kSmallTile);
   cudaMemsetAsync(ws.dtable[0], 0, (size_t)4 * 256 * (nba + 1) * sizeof(u32), st);
-  depth_keys_kernel<<<(N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK, 256, 0, st>>>(N, proj.tiles_touched, proj.depth,
-                                                                            proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis,
-                                                                            ws.dtable[0]);
+  launch_pdl(depth_keys_kernel, (N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK, 256, 0, st, N, proj.tiles_touched, proj.depth,
+             proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis, ws.dtable[0]);
   launched();
   for (int p = 0; p < 4; ++p)
     radix_pass_small(ws.pk[p & 1], ws.pv[p & 1], ws.pk[(p & 1) ^ 1], ws.pv[(p & 1) ^ 1], ws.n_vis, nba, 8 * p, ws.dtable[p],
@@ -1055,7 +1057,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
                ws.chunk_table, ranges, bin.num_instances, bin.capacity, band_rows, bin.ids);
     launched();
     if (bin.keys) {
-      tile_keys_kernel<<<(ntiles + 1) / 2, 256, 0, st>>>(ntiles, ranges, bin.ids, proj.depth, bin.keys);
+      launch_pdl(tile_keys_kernel, (ntiles + 1) / 2, 256, 0, st, ntiles, (const uint2*)ranges, (const u32*)bin.ids, proj.depth, bin.keys);
       launched();
     }
     tm.end(st);

@@ -76,6 +76,7 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
                                                                        const float* __restrict__ final_T,
                                                                        const float* __restrict__ dL_dimage,
                                                                        float* __restrict__ grad2d) {
+  pdl_wait();
   constexpr int R4 = packed_floats(K) / 4;
   constexpr int TL = K > 0 ? tail_floats(K) : 1;
   constexpr int NV = 9 + 3 * K + (ABS ? 2 : 0);
@@ -231,9 +232,8 @@ template <int K, bool ABS>
 cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
                      const gabsplat_fwd_out& fwd, const BlendState& saved, const float* dL, float* grad2d, cudaStream_t st) {
   const int ntiles = cam.tiles_x * cam.tiles_y;
-  blend_backward_kernel<K, ABS><<<2 * ntiles, 32, 0, st>>>(
-      cam, reinterpret_cast<const uint2*>(bin.tile_ranges), saved, reinterpret_cast<const float4*>(proj.packed),
-      fwd.final_T, dL, grad2d);
+  launch_pdl(blend_backward_kernel<K, ABS>, 2 * ntiles, 32, 0, st, cam, reinterpret_cast<const uint2*>(bin.tile_ranges), saved,
+             reinterpret_cast<const float4*>(proj.packed), (const float*)fwd.final_T, dL, grad2d);
   launched();
   return cudaGetLastError();
 }

@@ -21,6 +21,7 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
                                                                       float* __restrict__ image, float* __restrict__ final_T,
                                                                       uint32_t* __restrict__ n_contrib,
                                                                       uint32_t* __restrict__ counters, BlendState save) {
+  pdl_wait();
   constexpr int R4 = packed_floats(K) / 4;
   constexpr int TL = K > 0 ? 4 * ((3 * K + 3) / 4) : 1;
   __shared__ float4 s_rec[kBatch * R4];
@@ -150,9 +151,9 @@ cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const ga
                      float* image, float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save,
                      cudaStream_t st) {
   const int ntiles = cam.tiles_x * cam.tiles_y;
-  blend_forward_kernel<K, COUNT, SAVE><<<ntiles, kBlendThreads, 0, st>>>(
-      cam, bin.tile_order, reinterpret_cast<const uint2*>(bin.tile_ranges), bin.ids, reinterpret_cast<const float4*>(proj.packed),
-      colour, image, final_T, n_contrib, counters, save ? *save : BlendState{nullptr, nullptr, nullptr});
+  launch_pdl(blend_forward_kernel<K, COUNT, SAVE>, ntiles, kBlendThreads, 0, st, cam, (const uint32_t*)bin.tile_order,
+             reinterpret_cast<const uint2*>(bin.tile_ranges), (const uint32_t*)bin.ids, reinterpret_cast<const float4*>(proj.packed),
+             colour, image, final_T, n_contrib, counters, save ? *save : BlendState{nullptr, nullptr, nullptr, nullptr});
   launched();
   return cudaGetLastError();
 }

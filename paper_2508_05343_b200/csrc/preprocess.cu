@@ -252,6 +252,7 @@ constexpr int kPreThreads = 256;
 constexpr int kPreChunk = GABSPLAT_CHUNK;
 
 __global__ void __launch_bounds__(kPreThreads) index_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
+  pdl_wait();
   __shared__ int s_n;
   if (threadIdx.x == 0) s_n = 0;
   __syncthreads();
@@ -294,6 +295,7 @@ __global__ void __launch_bounds__(kPreThreads) index_kernel(gabsplat_scene s, Ca
 constexpr int kValThreads = 128;
 
 __global__ void __launch_bounds__(kValThreads, 4) value_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
+  pdl_wait();
   __shared__ int s_i[kPreChunk];
   __shared__ int s_n;
   if (out.chunk_visible[blockIdx.x] == 0) return;
@@ -313,8 +315,8 @@ cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const 
                               cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
   const int chunks = (s.N + kPreChunk - 1) / kPreChunk;
-  index_kernel<<<chunks, kPreThreads, 0, st>>>(s, cam, out);
-  value_kernel<<<chunks, kValThreads, 0, st>>>(s, cam, out);
+  launch_pdl(index_kernel, chunks, kPreThreads, 0, st, s, cam, out);
+  launch_pdl(value_kernel, chunks, kValThreads, 0, st, s, cam, out);
   launched(2);
   return cudaGetLastError();
 }

@@ -242,6 +242,7 @@ __global__ void __launch_bounds__(kBwdThreads, 3) preprocess_backward_kernel(gab
                                                                          const uint32_t* __restrict__ n_vis,
                                                                          const uint8_t* __restrict__ rgb_clamped,
                                                                          float* grad2d, gabsplat_grads g) {
+  pdl_wait();
   const uint32_t r = blockIdx.x * kBwdThreads + threadIdx.x;
   if (r >= *n_vis) return;
   backward_one(s, c, rgb_clamped, grad2d, g, (int)order[r]);
@@ -283,8 +284,8 @@ cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& ca
   if (s.N == 0) return cudaGetLastError();
   const uint32_t *order, *n_vis;
   binning_visible_list(bin, s.N, cam.tiles_x * cam.tiles_y, &order, &n_vis);
-  preprocess_backward_kernel<<<(s.N + kBwdThreads - 1) / kBwdThreads, kBwdThreads, 0, st>>>(s, cam, order, n_vis,
-                                                                                       proj.rgb_clamped, grad2d, g);
+  launch_pdl(preprocess_backward_kernel, (s.N + kBwdThreads - 1) / kBwdThreads, kBwdThreads, 0, st, s, cam, order, n_vis,
+             (const uint8_t*)proj.rgb_clamped, grad2d, g);
   launched();
   return cudaGetLastError();
 }
