@@ -309,8 +309,9 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
 
     def step(i, do_backward, bins=bins):
         v = my_view(i)
-        gb.gabsplat_preprocess(ctx, ds, cams[v], proj)
-        gb.gabsplat_bin_sort(ctx, N, proj, cams[v], bin=bins, read_count=False)
+        # S1 + S2 through the fused entry point (same results as the two calls; the value track of the projection
+        # overlaps the binning)
+        gb.gabsplat_preprocess_bin_sort(ctx, ds, cams[v], proj, bins, read_count=False)
         # a forward that is followed by a backward records the blend state the backward replays;
         # a forward-only step (inference) does not
         gb.gabsplat_render_forward(ctx, ds, cams[v], proj, bins, fwd, save_state=do_backward)

@@ -172,6 +172,14 @@ int32_t gabsplat_preprocess(gabsplat_ctx* ctx, const gabsplat_scene* scene, cons
 int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected* proj, const gabsplat_camera* cam,
                           gabsplat_binning* bin, uint64_t* num_instances_host, void* stream);
 
+/* S1 + S2 in one call: the same results as gabsplat_preprocess followed by gabsplat_bin_sort, with the fp64 value
+ * track of the projection (needed only by the blend) running on the context's side stream beside the binning
+ * (which needs only the indexing track).  All outputs are ready, in the order of `stream`, when later work
+ * enqueued on `stream` runs. */
+int32_t gabsplat_preprocess_bin_sort(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                                     gabsplat_projected* proj, gabsplat_binning* bin, uint64_t* num_instances_host,
+                                     void* stream);
+
 /* S3.  One CTA per tile; Eq.12-13 with the alpha rules of DESIGN.md (alpha = min(0.99, o G M),
  * skip alpha < 1/255, stop before T(1-alpha) < 1e-4). */
 int32_t gabsplat_render_forward(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,

@@ -91,6 +91,9 @@ def lib():
         L.gabsplat_preprocess.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected), P]
         L.gabsplat_bin_sort.argtypes = [P, C.c_int32, C.POINTER(_Projected), C.POINTER(_Camera), C.POINTER(_Binning),
                                         C.POINTER(C.c_uint64), P]
+        L.gabsplat_preprocess_bin_sort.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
+                                                   C.POINTER(_Binning), C.POINTER(C.c_uint64), P]
+        L.gabsplat_preprocess_bin_sort.restype = C.c_int32
         L.gabsplat_render_forward.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
                                               C.POINTER(_Binning), C.POINTER(_FwdOut), P]
         L.gabsplat_render_backward.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
@@ -333,6 +336,17 @@ def gabsplat_bin_sort(ctx: Context, N: int, proj: Projected, cam, bin: Binning |
     d = C.c_uint64(0)
     ctx.check(lib().gabsplat_bin_sort(ctx._h, N, C.byref(p), C.byref(c), C.byref(b),
                                       C.byref(d) if read_count else None, _stream(stream)))
+    bin.D = int(d.value) if read_count else None
+    return bin
+
+
+def gabsplat_preprocess_bin_sort(ctx: Context, scene: DeviceScene, cam, proj: Projected, bin: Binning,
+                                 read_count: bool = True, stream=None) -> Binning:
+    """S1 + S2 in one call (the value track of the projection overlaps the binning); buffers are the caller's."""
+    s, c, p, b = scene.struct(), camera_struct(cam), proj.struct(), bin.struct()
+    d = C.c_uint64(0)
+    ctx.check(lib().gabsplat_preprocess_bin_sort(ctx._h, C.byref(s), C.byref(c), C.byref(p), C.byref(b),
+                                                 C.byref(d) if read_count else None, _stream(stream)))
     bin.D = int(d.value) if read_count else None
     return bin
 

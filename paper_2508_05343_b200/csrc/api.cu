@@ -137,9 +137,32 @@ int32_t gabsplat_preprocess(gabsplat_ctx* ctx, const gabsplat_scene* scene, cons
   if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess: bad camera");
   if (!projected_ok(out, scene->N, scene->K)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess: null output");
   ctx->timer.begin(GABSPLAT_STAGE_PREPROCESS, (cudaStream_t)stream);
-  const cudaError_t e = launch_preprocess(*scene, make_camera(*cam), *out, (cudaStream_t)stream);
+  const cudaError_t e = launch_preprocess(*scene, make_camera(*cam), *out, (cudaStream_t)stream, (cudaStream_t)stream, nullptr);
   ctx->timer.end((cudaStream_t)stream);
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "preprocess");
+}
+
+int32_t gabsplat_preprocess_bin_sort(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                                     gabsplat_projected* proj, gabsplat_binning* bin, uint64_t* num_instances_host,
+                                     void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  // with the stage timer on, or nothing to overlap, this is exactly the two calls
+  if (ctx->timer.on || !scene || scene->N <= 0) {
+    const int32_t rc = gabsplat_preprocess(ctx, scene, cam, proj, stream);
+    return rc != GABSPLAT_OK ? rc : gabsplat_bin_sort(ctx, scene->N, proj, cam, bin, num_instances_host, stream);
+  }
+  if (!scene_ok(scene)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess_bin_sort: bad scene");
+  if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess_bin_sort: bad camera");
+  if (!projected_ok(proj, scene->N, scene->K)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess_bin_sort: null output");
+  cudaStream_t st = (cudaStream_t)stream;
+  // the binning needs only the indexing track: the fp64 value track runs on the side stream beside it
+  cudaError_t e = launch_preprocess(*scene, make_camera(*cam), *proj, st, ctx->side, ctx->ev_fork);
+  if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_join, ctx->side);
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "preprocess_bin_sort (projection)");
+  const int32_t rc = gabsplat_bin_sort(ctx, scene->N, proj, cam, bin, num_instances_host, stream);
+  e = cudaStreamWaitEvent(st, ctx->ev_join, 0);  // join even when the binning reported an error
+  if (e != cudaSuccess) return cuda_fail(ctx, e, "preprocess_bin_sort (join)");
+  return rc;
 }
 
 int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected* proj, const gabsplat_camera* cam,

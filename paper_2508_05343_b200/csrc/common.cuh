@@ -140,7 +140,7 @@ inline void launched(int n = 1) { g_kernel_launches += (unsigned long long)n; }
 
 // ---- launchers (one per .cu file); each returns the cudaError_t of its last launch ---------------
 cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& out,
-                              cudaStream_t st);
+                              cudaStream_t st, cudaStream_t value_stream, cudaEvent_t index_done);
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
                             StageTimer& tm, cudaStream_t st);
 cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projected& proj,

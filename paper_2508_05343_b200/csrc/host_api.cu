@@ -116,10 +116,8 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* sh, const 
   GS_H2D(l.scene.freqs, sh->freqs, n * k * 3);
   GS_H2D(l.scene.weights, sh->weights, n * k);
   if (dL_dimage_host) GS_H2D(l.dL, dL_dimage_host, 3 * hw);
-  int32_t rc = gabsplat_preprocess(ctx, &l.scene, cam, &l.proj, stream);
-  if (rc != GABSPLAT_OK) return rc;
   uint64_t D = 0;
-  rc = gabsplat_bin_sort(ctx, sh->N, &l.proj, cam, &l.bin, &D, stream);
+  int32_t rc = gabsplat_preprocess_bin_sort(ctx, &l.scene, cam, &l.proj, &l.bin, &D, stream);
   if (rc != GABSPLAT_OK) return rc;
   if (!dL_dimage_host) l.fwd.blend_state = nullptr;  // inference: nothing to replay
   rc = gabsplat_render_forward(ctx, &l.scene, cam, &l.proj, &l.bin, &l.fwd, stream);

@@ -311,12 +311,19 @@ __global__ void __launch_bounds__(kValThreads, 4) value_kernel(gabsplat_scene s,
 
 }  // namespace
 
+// `value_stream` != st: the value track (needed only by the blend) runs there, so that the caller can overlap it
+// with the binning, which needs only the indexing track; the caller orders the two streams with events.
 cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& out,
-                              cudaStream_t st) {
+                              cudaStream_t st, cudaStream_t value_stream, cudaEvent_t index_done) {
   if (s.N == 0) return cudaSuccess;
   const int chunks = (s.N + kPreChunk - 1) / kPreChunk;
   launch_pdl(index_kernel, chunks, kPreThreads, 0, st, s, cam, out);
-  launch_pdl(value_kernel, chunks, kValThreads, 0, st, s, cam, out);
+  if (value_stream != st) {
+    cudaError_t e = cudaEventRecord(index_done, st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(value_stream, index_done, 0);
+    if (e != cudaSuccess) return e;
+  }
+  launch_pdl(value_kernel, chunks, kValThreads, 0, value_stream, s, cam, out);
   launched(2);
   return cudaGetLastError();
 }

@@ -182,3 +182,28 @@ def test_backward_leaves_its_workspace_zero():
     assert int(g.workspace.count_nonzero().item()) == 0
     for n, ref in first.items():
         assert torch.allclose(getattr(g, n), ref, rtol=1e-4, atol=2e-6 * float(ref.abs().max()))
+
+
+def test_fused_preprocess_bin_sort_equals_the_two_calls():
+    """gabsplat_preprocess_bin_sort (value track on the side stream beside the binning) gives bit-identical
+    projected arrays, lists and image."""
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("unbounded", N=60000)
+    base = scenes.make_cameras("unbounded")[2]
+    cam = scenes.make_camera(331, 213, 290.0, base.world_to_cam, base.bg)
+    ds = gb.upload_scene(scene)
+    p1 = gb.gabsplat_preprocess(ctx, ds, cam)
+    b1 = gb.gabsplat_bin_sort(ctx, ds.N, p1, cam)
+    f1 = gb.gabsplat_render_forward(ctx, ds, cam, p1, b1, save_state=False)
+    p2 = gb.Projected(ds.N, ds.K, ds.means.device)
+    b2 = gb.Binning(ds.N, cam, b1.capacity, ds.means.device)
+    for _ in range(3):       # repeated: the side stream must be ordered against the next call too
+        gb.gabsplat_preprocess_bin_sort(ctx, ds, cam, p2, b2)
+        f2 = gb.gabsplat_render_forward(ctx, ds, cam, p2, b2, save_state=False)
+    torch.cuda.synchronize()
+    assert b2.D == b1.D
+    for n in ("mean2d", "depth", "radius", "conic_opacity", "rgb", "rgb_clamped", "freq2d", "tiles_touched", "rect", "packed"):
+        assert torch.equal(getattr(p1, n), getattr(p2, n)), n
+    assert torch.equal(b1.ids[:b1.D], b2.ids[:b1.D]) and torch.equal(b1.tile_ranges, b2.tile_ranges)
+    assert torch.equal(b1.keys[:b1.D], b2.keys[:b1.D])
+    assert torch.equal(f1.image, f2.image)
