@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
 #pragma unroll
       for (int i = 0; i < NV; ++i) acc[i] = 0.f;
       // sums over the thread's pixels of terms whose common factors (dx, L, 2 pi f2D) are applied once, below
-      float Sq = 0.f, Sqy = 0.f, Sqyy = 0.f, Squ = 0.f, Sqv = 0.f;
+      float Suu = 0.f, Suv = 0.f, Svv = 0.f, Squ = 0.f, Sqv = 0.f;
       float Sg[K > 0 ? K : 1], Sgy[K > 0 ? K : 1];
 #pragma unroll
       for (int k = 0; k < K; ++k) Sg[k] = Sgy[k] = 0.f;
@@ -182,9 +182,12 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
           acc[5] += gG * e.M;
           const float ngM = -(gG * oc.x);   // -dL/dM
           const float gq = galpha * raw;    // dL/d(ln G)
-          const float gqy = gq * dy;
-          Sq += gq; Sqy += gqy; Sqyy += gqy * dy;
-          Squ += gq * u; Sqv += gq * v;
+          // the conic's gradient is accumulated in the whitened coordinates (u, v) of the envelope,
+          // S = sum gq w w^T: its entries are O(gq) whatever the anisotropy of the footprint, where the sums of
+          // gq dx^2, gq dx dy, gq dy^2 lose the thin direction of a needle that spans the screen in the other
+          const float gqu = gq * u, gqv = gq * v;
+          Suu += gqu * u; Suv += gqu * v; Svv += gqv * v;
+          Squ += gqu; Sqv += gqv;
           float pdx = 0.f, pdy = 0.f;       // per-pixel d/d(dx), d/d(dy) through the phases (AbsGS only)
 #pragma unroll
           for (int k = 0; k < K; ++k) {
@@ -202,10 +205,10 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
         }
       }
       {
-        // conic (a, b, c): dL/dq (-dx^2 / 2, -dx dy, -dy^2 / 2)
-        acc[2] = -0.5f * dx * dx * Sq;
-        acc[3] = -dx * Sqy;
-        acc[4] = -0.5f * Sqyy;
+        // conic, in whitened form: S = sum dL/d(ln G) w w^T  (the projection backward maps it to dL/dU)
+        acc[2] = Suu;
+        acc[3] = Suv;
+        acc[4] = Svv;
         // mean: d = p - mu2D, so dL/dmu2D = -dL/dd;  dL/dd = dL/dq ln 2 (-2 u L11, -2 (u L21 + v L22)) + sum_k gph_k 2 pi f2D_k
         float gdx = -1.3862943611198906f * l.x * Squ;
         float gdy = -1.3862943611198906f * (l.y * Squ + l.z * Sqv);

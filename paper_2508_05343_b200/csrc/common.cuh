@@ -28,7 +28,7 @@ __host__ __device__ constexpr int tail_floats(int K) { return 4 * ((3 * K + 3) /
 __host__ __device__ constexpr int packed_floats(int K) { return 12 + tail_floats(K); }
 
 // ---- 2D gradient record accumulated by the blend backward (grad workspace), floats ---------------
-//  [0..1] d mean2d   [2..4] d conic (a,b,c)   [5] d opacity   [6..8] d rgb
+//  [0..1] d mean2d   [2..4] S_uu, S_uv, S_vv: the conic's gradient in whitened form (blend_backward.cu)   [5] d opacity   [6..8] d rgb
 //  [9..9+2K) d (2 pi f2D) (x,y) * K   [9+2K..9+3K) d omega * K   [9+3K..11+3K) sum |d mean2d| (AbsGS statistic)
 //  padded to a multiple of 4 floats
 __host__ __device__ constexpr int grad2d_values(int K) { return 11 + 3 * K; }

@@ -63,16 +63,23 @@ __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Came
   const double idet = 1.0 / (A * C - U01 * U01);
   const double ca = C * idet, cb = -U01 * idet, cc = A * idet;
 
-  // conic -> U_d (= U + const):  G_U = -Cm Gc Cm,  Gc = [[ga, gb/2],[gb/2, gc]]
+  // conic -> U_d (= U + const).  The blend accumulated S = sum gq w w^T with w = L^T d the whitened pixel offset
+  // (L = sqrt(log2(e) / 2) * Cholesky factor of the conic, as packed for the blend) and gq = dL/d(ln G).  With
+  // G_c = sum gq (-1/2 d d^T):  G_U = -C G_c C = 1/2 sum gq (C d)(C d)^T = 2 ln^2(2) L S L^T.
   double GU[2][2];
   {
-    const double ga = g2[2], gb = 0.5 * (double)g2[3], gc = g2[4];
-    const double m00 = ca * ga + cb * gb, m01 = ca * gb + cb * gc;
-    const double m10 = cb * ga + cc * gb, m11 = cb * gb + cc * gc;
-    GU[0][0] = -(m00 * ca + m01 * cb);
-    GU[0][1] = -(m00 * cb + m01 * cc);
-    GU[1][0] = -(m10 * ca + m11 * cb);
-    GU[1][1] = -(m10 * cb + m11 * cc);
+    const double rs = 0.84932180028801904272;  // sqrt(0.5 * log2(e)), as in preprocess.cu
+    const double l11 = sqrt(ca), l21 = cb / l11, l22 = sqrt(fmax(cc - l21 * l21, 0.0));
+    const double L11 = l11 * rs, L21 = l21 * rs, L22 = l22 * rs;
+    const double suu = g2[2], suv = g2[3], svv = g2[4];
+    // M = L S  (L = [[L11, 0], [L21, L22]])
+    const double m00 = L11 * suu, m01 = L11 * suv;
+    const double m10 = L21 * suu + L22 * suv, m11 = L21 * suv + L22 * svv;
+    const double k = 2.0 * 0.69314718055994530942 * 0.69314718055994530942;
+    GU[0][0] = k * (m00 * L11);
+    GU[0][1] = k * (m00 * L21 + m01 * L22);
+    GU[1][0] = k * (m10 * L11);
+    GU[1][1] = k * (m10 * L21 + m11 * L22);
   }
   double gS[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, gT[2][3] = {{0, 0, 0}, {0, 0, 0}};
   // f2D_k = U^-1 T Sigma f_k  (U undilated)
