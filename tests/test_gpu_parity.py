@@ -254,7 +254,7 @@ def _decidable_mask(orc, scene, cam):
     return np.minimum(m[..., 0], m[..., 1]) > DELTA
 
 
-@pytest.mark.parametrize("view", [0, 5])
+@pytest.mark.parametrize("view", [0, 5, 7])
 def test_full_size_gradients(view):
     """BASELINE.json config 3 (1M primitives, 1297x840) forward + backward in the launch configuration bench.py
     times, every gradient tensor against the oracle's analytic gradients (painter's-order loop, ~10 s on the host).
@@ -264,7 +264,9 @@ def test_full_size_gradients(view):
     whole screen (view 5 has one 0.3 units in front of the camera, radius 10 006 px) collects those pixels' terms in
     a sum that otherwise cancels to a few per cent of one term.  The comparison is therefore made where the result
     is unique: dL/dimage is zeroed on the undecidable pixels (0.4 % of the image) for both sides.  There the two
-    agree to ~1e-5; the bar here is 1e-4, ten times tighter than north_star's 1e-3.  The unmasked comparison is kept
+    agree to ~1e-5 or better; the bar here is 1e-4, ten times tighter than north_star's 1e-3.  (View 7 holds a
+    needle of scales 1.6 x 0.003 x 0.02 spanning the screen: the case that needs the conic's gradient accumulated
+    in whitened coordinates.)  The unmasked comparison is kept
     as a gross-error bound."""
     orc = _oracle()
     scene = scenes.make_scene("unbounded")
