@@ -66,7 +66,8 @@ typedef struct {
   int32_t width, height;
   float fx, fy, cx, cy;
   float world_to_cam[12]; /* row-major 3x4 [W | tau]:  t = W mu + tau */
-  float z_near;           /* primitives with t_z <= z_near are culled */
+  float z_near;           /* > 0 (INVALID_ARG otherwise: the depth key orders the bit patterns of positive
+                             floats); primitives with t_z <= z_near are culled */
   float bg[3];            /* background colour, composited as C + T_final * bg */
 } gabsplat_camera;
 
@@ -258,6 +259,34 @@ uint64_t gabsplat_kernel_launches(void);
 int32_t gabsplat_count_pairs(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
                              const gabsplat_projected* proj, const gabsplat_binning* bin, uint32_t* counters,
                              void* stream);
+
+/* The forward blend's decisions at n selected pixels (instrumentation of the parity tests; reading C18: at a
+ * pixel where a skip / stop / clamp decision sits within fp32 error of its threshold both outcomes are correct, and
+ * the tests hand the CUDA path's decisions at exactly those pixels to the oracle).  One thread per pixel walks the
+ * pixel's tile list with the operation sequence of gabsplat_render_forward (Eq.12-13 :158-162; bit-identical alpha).
+ *   pixels   device [n][2] int32 (x, y), inside the image
+ *   offsets  device [n+1] uint32, ascending: pixel i may write entries[offsets[i] .. offsets[i+1])
+ *   entries  device: for every entry blended at pixel i, in order: its 1-based position in the tile list, bit 31 set
+ *            when min(0.99, .) was active (zero derivative in the backward); entries beyond the slice are dropped
+ *   colour_T device [n][4] float: the pixel's (r, g, b) incl. background and final T -- equal bit for bit to
+ *            gabsplat_fwd_out.image / final_T
+ *   info     device [n][4] uint32: n_contrib, number of blended entries (may exceed the slice), 1-based position of
+ *            the entry at which the pixel stopped (T (1 - alpha) < 1e-4; 0 = never), 0 */
+int32_t gabsplat_trace_pixels(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                              const gabsplat_projected* proj, const gabsplat_binning* bin, int32_t n, const int32_t* pixels,
+                              const uint32_t* offsets, uint32_t* entries, float* colour_T, uint32_t* info, void* stream);
+
+/* cos and sin of n raw radian phases (device arrays) exactly as the blend kernels evaluate the phases of Eq.12
+ * (:158): the MUFU path, no explicit range reduction.  For the committed measurement of its error bound
+ * (DESIGN.md "Tolerances"). */
+int32_t gabsplat_probe_sincos(gabsplat_ctx* ctx, int32_t n, const float* phase, float* cos_out, float* sin_out, void* stream);
+
+/* The ALU rooflines of the blend kernels measured on this device: results_host[16] (HOST) =
+ *   [0] FFMA lane-instructions/s   [1] packed FFMA2 lane-instructions/s   [2] MUFU.EX2 lane-ops/s
+ *   [3] MUFU.COS lane-ops/s        [4] 4 FFMA : 1 MUFU mix, lane-instructions/s   [5] integer ALU-pipe lane-instr/s
+ *   [6] SM clock (Hz) seen by the kernels   [7] number of SMs   [8..13] entries 0..5 per SM per clock.
+ * Dependency-free chains, 64 warps per SM, best of 3 after a warm-up.  Synchronises; takes a few milliseconds. */
+int32_t gabsplat_measure_peaks(gabsplat_ctx* ctx, float* results_host, void* stream);
 
 #ifdef __cplusplus
 }

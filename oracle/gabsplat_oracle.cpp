@@ -380,11 +380,40 @@ struct PixelState {
     int32_t last_id = -1;
     uint32_t examined = 0, envelope = 0, blended = 0;
     double margin = 1e300, margin_clamp = 1e300;
+    int32_t inj = -1;          // index into Inject (decision-injected mode), -1 = this pixel takes its own decisions
+    uint32_t inj_at = 0;       // cursor into the pixel's injected list
 };
 
+// Decision-injected mode (reading C18).  The image is discontinuous where alpha crosses 1/255, where
+// T (1 - alpha) crosses 1e-4 and (for the gradient) where o G M crosses 0.99: within the evaluation error of a
+// threshold BOTH outcomes are correct renderings.  To compare gradients and images at such pixels without masking
+// them, the caller may fix the outcome of every decision at selected pixels: for pixel pixels[i], the ascending
+// 1-based tile-list positions of the entries that are blended (bit 31: the 0.99 clamp counts as active) and the
+// position at which the pixel stops (0 = never).  The oracle evaluates every pair exactly as before, takes the
+// injected outcome, and COUNTS A VIOLATION whenever the injected outcome differs from its own while its own value
+// is farther than `delta` (relative) from the threshold concerned -- so an injected list is accepted only if it is a
+// correct rendering in the sense above.  Pixels without an injected list are untouched.
+struct Inject {
+    int n = 0;
+    const int32_t* pixels = nullptr;     // [n][2] (x, y)
+    const uint32_t* offsets = nullptr;   // [n+1]
+    const uint32_t* entries = nullptr;   // [offsets[n]]
+    const uint32_t* stop_pos = nullptr;  // [n]
+    double delta = 0.0;
+    uint64_t* violations = nullptr;      // [1], incremented atomically
+};
+
+inline void violation(const Inject& inj) {
+#pragma omp atomic
+    inj.violations[0] += 1;
+}
+
 // Visit primitive i (already known to cover the pixel's tile) at pixel (px,py).
-inline void visit(const Scene& s, const Proj& p, int i, double px, double py, PixelState& st) {
+inline void visit_injected(const Scene& s, const Proj& p, int i, double px, double py, PixelState& st, const Inject& inj);
+
+inline void visit(const Scene& s, const Proj& p, int i, double px, double py, PixelState& st, const Inject* inj = nullptr) {
     if (st.done) return;
+    if (st.inj >= 0) { visit_injected(s, p, i, px, py, st, *inj); return; }
     st.pos += 1;
     st.examined += 1;
     PairEval e;
@@ -402,6 +431,51 @@ inline void visit(const Scene& s, const Proj& p, int i, double px, double py, Pi
     st.last_pos = st.pos;
     st.last_id = i;
     st.blended += 1;
+}
+
+// The same visit with the outcome of every decision taken from the pixel's injected list (see Inject).
+inline void visit_injected(const Scene& s, const Proj& p, int i, double px, double py, PixelState& st, const Inject& inj) {
+    st.pos += 1;
+    st.examined += 1;
+    PairEval e;
+    eval_pair(s, p, i, px, py, e);
+    const uint32_t* lst = inj.entries + inj.offsets[st.inj];
+    const uint32_t len = inj.offsets[st.inj + 1] - inj.offsets[st.inj];
+    const bool take = st.inj_at < len && (lst[st.inj_at] & 0x7fffffffu) == st.pos;
+    const bool stop_here = inj.stop_pos[st.inj] == st.pos;
+    if (!e.power_pos && e.envelope_pass) st.envelope += 1;
+    // the oracle's own outcome in the injected state: 0 skip, 1 stop, 2 blend
+    const double Tn = st.T * (1.0 - e.alpha);
+    const double m_alpha = std::fabs(e.alpha - ALPHA_MIN) / ALPHA_MIN;
+    const double m_T = std::fabs(Tn - T_MIN) / T_MIN;
+    const int own = (e.power_pos || e.alpha < ALPHA_MIN) ? 0 : (Tn < T_MIN ? 1 : 2);
+    if (take) {
+        if (stop_here) violation(inj);                                   // malformed list
+        if (e.power_pos) violation(inj);
+        else if (own == 0 && m_alpha > inj.delta) violation(inj);
+        else if (own == 1 && m_T > inj.delta) violation(inj);
+        const bool clamp = (lst[st.inj_at] >> 31) != 0;
+        if (clamp != (e.raw > ALPHA_MAX) && std::fabs(e.raw - ALPHA_MAX) / ALPHA_MAX > inj.delta) violation(inj);
+        st.inj_at += 1;
+        for (int ch = 0; ch < 3; ++ch) st.C[ch] += p.rgb[ch] * e.alpha * st.T;              // Eq.13
+        st.T = Tn;
+        st.last_pos = st.pos;
+        st.last_id = i;
+        st.blended += 1;
+        return;
+    }
+    if (stop_here) {
+        // the pixel stops at this entry: correct iff its own outcome is "stop", or "blend" / "skip" within delta
+        if (own == 2 && m_T > inj.delta) violation(inj);
+        if (own == 0 && (e.power_pos || m_alpha > inj.delta)) violation(inj);
+        if (st.inj_at != len) violation(inj);                            // blended entries listed after the stop
+        st.done = true;
+        return;
+    }
+    // skipped: correct iff its own outcome is "skip", or "blend" within delta of 1/255; a pixel that would stop
+    // here on its own must also be within delta (the injected outcome says the walk goes on)
+    if (own == 2 && m_alpha > inj.delta) violation(inj);
+    if (own == 1 && m_alpha > inj.delta && m_T > inj.delta) violation(inj);
 }
 
 inline bool covers(const Twin& tw, int tx, int ty) {
@@ -429,10 +503,12 @@ inline void store_pixel(const Cam& c, const FwdOut& o, int x, int y, const Pixel
 
 // Painter's order, parallel over tile rows: primitive-major over the pixels of its rectangle.
 void forward_painter(const Scene& s, const Cam& c, const std::vector<Proj>& P, const std::vector<int>& ord,
-                     const FwdOut& out, std::vector<PixelState>* keep) {
+                     const FwdOut& out, std::vector<PixelState>* keep, const Inject* inj = nullptr) {
     std::vector<PixelState> local;
     std::vector<PixelState>& st = keep ? *keep : local;
     st.assign((size_t)c.W * c.H, PixelState());
+    if (inj)
+        for (int k = 0; k < inj->n; ++k) st[(size_t)inj->pixels[2 * k + 1] * c.W + inj->pixels[2 * k]].inj = k;
 #pragma omp parallel for schedule(dynamic, 1)
     for (int ty = 0; ty < c.gy; ++ty) {
         const int y0 = ty * TILE, y1 = std::min(c.H, y0 + TILE);
@@ -441,10 +517,15 @@ void forward_painter(const Scene& s, const Cam& c, const std::vector<Proj>& P, c
             if (ty < tw.rect[1] || ty >= tw.rect[3]) continue;
             const int x0 = tw.rect[0] * TILE, x1 = std::min(c.W, tw.rect[2] * TILE);
             for (int y = y0; y < y1; ++y)
-                for (int x = x0; x < x1; ++x) visit(s, P[i], i, (double)x, (double)y, st[(size_t)y * c.W + x]);
+                for (int x = x0; x < x1; ++x) visit(s, P[i], i, (double)x, (double)y, st[(size_t)y * c.W + x], inj);
         }
         for (int y = y0; y < y1; ++y)
-            for (int x = 0; x < c.W; ++x) store_pixel(c, out, x, y, st[(size_t)y * c.W + x]);
+            for (int x = 0; x < c.W; ++x) {
+                const PixelState& ps = st[(size_t)y * c.W + x];
+                // an injected list must have been consumed entirely
+                if (inj && ps.inj >= 0 && ps.inj_at != inj->offsets[ps.inj + 1] - inj->offsets[ps.inj]) violation(*inj);
+                store_pixel(c, out, x, y, ps);
+            }
     }
 }
 
@@ -457,7 +538,8 @@ struct Grad2D {
 };
 
 void backward_pixels(const Scene& s, const Cam& c, const std::vector<Proj>& P, const std::vector<int>& ord,
-                     const std::vector<PixelState>& st, const float* gimg, std::vector<Grad2D>& G2) {
+                     const std::vector<PixelState>& st, const float* gimg, std::vector<Grad2D>& G2,
+                     const Inject* inj = nullptr) {
     const size_t HW = (size_t)c.H * c.W;
     G2.assign(s.N, Grad2D{});
     // position of each visible primitive in the depth order (for the "not beyond last" test)
@@ -467,6 +549,12 @@ void backward_pixels(const Scene& s, const Cam& c, const std::vector<Proj>& P, c
         // per-pixel reverse state: transmittance T (in front of the current primitive), B = colour behind
         std::vector<double> Tcur((size_t)TILE * c.W), Bc((size_t)TILE * c.W * 3);
         std::vector<uint32_t> pos((size_t)TILE * c.W);
+        std::vector<uint32_t> icur((size_t)TILE * c.W, 0);   // injected pixels: entries of the list not yet walked
+        if (inj)
+            for (int y = y0; y < y1; ++y) for (int x = 0; x < c.W; ++x) {
+                const int k = st[(size_t)y * c.W + x].inj;
+                if (k >= 0) icur[(size_t)(y - y0) * c.W + x] = inj->offsets[k + 1] - inj->offsets[k];
+            }
         // pos counts, per pixel, how many covering primitives remain (1-based position of the current one)
         for (int y = y0; y < y1; ++y) for (int x = 0; x < c.W; ++x) {
             const size_t l = (size_t)(y - y0) * c.W + x;
@@ -491,10 +579,22 @@ void backward_pixels(const Scene& s, const Cam& c, const std::vector<Proj>& P, c
                 for (int y = y0; y < y1; ++y) for (int x = x0; x < x1; ++x) {
                     const PixelState& ps = st[(size_t)y * c.W + x];
                     if (mypos > ps.last_pos) continue;          // beyond the last blended primitive
-                    PairEval e;
-                    eval_pair(s, p, i, (double)x, (double)y, e);
-                    if (e.power_pos || e.alpha < ALPHA_MIN) continue;
                     const size_t l = (size_t)(y - y0) * c.W + x;
+                    PairEval e;
+                    bool clamp_active;
+                    if (ps.inj >= 0) {
+                        // decision-injected pixel: blended iff the position is the next one (from the back) of its list
+                        if (icur[l] == 0) continue;
+                        const uint32_t ent = inj->entries[inj->offsets[ps.inj] + icur[l] - 1];
+                        if ((ent & 0x7fffffffu) != mypos) continue;
+                        icur[l] -= 1;
+                        eval_pair(s, p, i, (double)x, (double)y, e);
+                        clamp_active = (ent >> 31) != 0;
+                    } else {
+                        eval_pair(s, p, i, (double)x, (double)y, e);
+                        if (e.power_pos || e.alpha < ALPHA_MIN) continue;
+                        clamp_active = e.raw > ALPHA_MAX;
+                    }
                     const double Ti = Tcur[l] / (1.0 - e.alpha);   // transmittance in front of i
                     Tcur[l] = Ti;
                     const size_t pix = (size_t)y * c.W + x;
@@ -505,7 +605,7 @@ void backward_pixels(const Scene& s, const Cam& c, const std::vector<Proj>& P, c
                         galpha += Ti * gC[ch] * (p.rgb[ch] - Bc[3 * l + ch]);
                         Bc[3 * l + ch] = e.alpha * p.rgb[ch] + (1.0 - e.alpha) * Bc[3 * l + ch];
                     }
-                    if (e.raw > ALPHA_MAX) continue;             // clamp active: zero derivative (reading C14)
+                    if (clamp_active) continue;                  // clamp active: zero derivative (reading C14)
                     const double o = s.opac[i];
                     acc.o += galpha * e.G * e.M;
                     const double gG = galpha * o * e.M, gM = galpha * o * e.G;
@@ -817,12 +917,52 @@ void orc_render_pixels(SCENE_ARGS, const double* cam, int n, const int32_t* pixe
     }
 }
 
+// The oracle's own decisions at selected pixels, in the format of Inject: for pixel k the ascending 1-based
+// tile-list positions of the entries it blends (bit 31: o G M > 0.99, clamp active) written to
+// entries[offsets[k] .. offsets[k+1]) (dropped beyond the slice), counts[k] = number blended, stop_pos[k] = position
+// of the entry at which T (1 - alpha) < 1e-4 stopped the pixel (0 = never).
+void orc_trace_pixels(SCENE_ARGS, const double* cam, int n, const int32_t* pixels, const uint32_t* offsets,
+                      uint32_t* entries, uint32_t* counts, uint32_t* stop_pos) {
+    const Scene s = make_scene(SCENE_PASS);
+    const Cam c = load_cam(cam);
+    std::vector<Proj> P;
+    project_all(s, c, 0, P);
+    const std::vector<int> ord = depth_order(P);
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int k = 0; k < n; ++k) {
+        const int x = pixels[2 * k], y = pixels[2 * k + 1];
+        PixelState st;
+        uint32_t nb = 0, stop = 0;
+        const uint32_t cap = offsets[k + 1] - offsets[k];
+        for (int i : ord) {
+            if (!covers(P[i].tw, x / TILE, y / TILE)) continue;
+            const uint32_t before = st.blended;
+            visit(s, P[i], i, (double)x, (double)y, st);
+            if (st.blended != before) {
+                PairEval e;
+                eval_pair(s, P[i], i, (double)x, (double)y, e);
+                if (nb < cap) entries[offsets[k] + nb] = st.pos | (e.raw > ALPHA_MAX ? 0x80000000u : 0u);
+                ++nb;
+            }
+            if (st.done) { stop = st.pos; break; }
+        }
+        counts[k] = nb;
+        stop_pos[k] = stop;
+    }
+}
+
 // Forward + analytic backward.  dL_dimage is [3][H][W] float32.  Gradient outputs are double, fully
-// overwritten (zero for culled primitives).  The 2D-gradient outputs may be null.
-void orc_render_backward(SCENE_ARGS, const double* cam, const float* dL_dimage, double* image,
-                         double* d_means, double* d_scales, double* d_quats, double* d_opac, double* d_sh,
-                         double* d_freqs, double* d_weights, double* d_mean2d, double* d_conic, double* d_rgb,
-                         double* d_freq2d, double* d_absmean2d) {
+// overwritten (zero for culled primitives).  The 2D-gradient outputs, final_T and n_contrib may be null.
+// n_inj > 0 selects the decision-injected mode (see Inject): inj_pixels [n_inj][2], inj_offsets [n_inj+1],
+// inj_entries, inj_stop [n_inj], accepted within the relative margin inj_delta; *violations counts the injected
+// outcomes that are NOT correct renderings.
+void orc_render_backward_ex(SCENE_ARGS, const double* cam, const float* dL_dimage, double* image, double* final_T,
+                            uint32_t* n_contrib,
+                            double* d_means, double* d_scales, double* d_quats, double* d_opac, double* d_sh,
+                            double* d_freqs, double* d_weights, double* d_mean2d, double* d_conic, double* d_rgb,
+                            double* d_freq2d, double* d_absmean2d,
+                            int n_inj, const int32_t* inj_pixels, const uint32_t* inj_offsets, const uint32_t* inj_entries,
+                            const uint32_t* inj_stop, double inj_delta, uint64_t* violations) {
     const Scene s = make_scene(SCENE_PASS);
     const Cam c = load_cam(cam);
     std::vector<Proj> P;
@@ -833,10 +973,20 @@ void orc_render_backward(SCENE_ARGS, const double* cam, const float* dL_dimage, 
     std::vector<uint32_t> nc(HW);
     std::vector<int32_t> lid(HW);
     std::vector<PixelState> st;
-    forward_painter(s, c, P, ord, FwdOut{img.data(), fT.data(), nc.data(), lid.data(), nullptr, nullptr}, &st);
+    Inject inj;
+    uint64_t dummy = 0;
+    if (n_inj > 0) {
+        inj.n = n_inj; inj.pixels = inj_pixels; inj.offsets = inj_offsets; inj.entries = inj_entries;
+        inj.stop_pos = inj_stop; inj.delta = inj_delta; inj.violations = violations ? violations : &dummy;
+        inj.violations[0] = 0;
+    }
+    const Inject* ip = n_inj > 0 ? &inj : nullptr;
+    forward_painter(s, c, P, ord, FwdOut{img.data(), fT.data(), nc.data(), lid.data(), nullptr, nullptr}, &st, ip);
     if (image) std::memcpy(image, img.data(), 3 * HW * sizeof(double));
+    if (final_T) std::memcpy(final_T, fT.data(), HW * sizeof(double));
+    if (n_contrib) std::memcpy(n_contrib, nc.data(), HW * sizeof(uint32_t));
     std::vector<Grad2D> G2;
-    backward_pixels(s, c, P, ord, st, dL_dimage, G2);
+    backward_pixels(s, c, P, ord, st, dL_dimage, G2, ip);
     const GradOut out{d_means, d_scales, d_quats, d_opac, d_sh, d_freqs, d_weights, d_mean2d, d_conic, d_rgb, d_freq2d, d_absmean2d};
     std::memset(d_means, 0, sizeof(double) * 3 * N); std::memset(d_scales, 0, sizeof(double) * 3 * N);
     std::memset(d_quats, 0, sizeof(double) * 4 * N); std::memset(d_opac, 0, sizeof(double) * N);
@@ -853,6 +1003,15 @@ void orc_render_backward(SCENE_ARGS, const double* cam, const float* dL_dimage, 
         for (int k = 0; k < K; ++k) for (int a = 0; a < 2; ++a) if (d_freq2d) d_freq2d[(size_t)(i * K + k) * 2 + a] = g.f2d[k][a];
         if (P[i].tw.visible) backward_primitive(s, c, P[i], i, g, out);
     }
+}
+
+void orc_render_backward(SCENE_ARGS, const double* cam, const float* dL_dimage, double* image,
+                         double* d_means, double* d_scales, double* d_quats, double* d_opac, double* d_sh,
+                         double* d_freqs, double* d_weights, double* d_mean2d, double* d_conic, double* d_rgb,
+                         double* d_freq2d, double* d_absmean2d) {
+    orc_render_backward_ex(SCENE_PASS, cam, dL_dimage, image, nullptr, nullptr, d_means, d_scales, d_quats, d_opac, d_sh,
+                           d_freqs, d_weights, d_mean2d, d_conic, d_rgb, d_freq2d, d_absmean2d, 0, nullptr, nullptr, nullptr,
+                           nullptr, 0.0, nullptr);
 }
 
 }  // extern "C"

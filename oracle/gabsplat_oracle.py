@@ -132,18 +132,54 @@ def render_pixels(scene, cam, pixels) -> dict:
     return o
 
 
-def render_backward(scene, cam, dL_dimage) -> dict:
+def trace_pixels(scene, cam, pixels, max_entries: int = 4096) -> dict:
+    """The oracle's own blend decisions at the pixels [n][2] (x, y), in the format render_backward's `inject` takes."""
+    keep, args = _scene_args(scene)
+    cv = cam_vector(cam)
+    px = np.ascontiguousarray(pixels, np.int32).reshape(-1, 2)
+    n = px.shape[0]
+    off = (np.arange(n + 1, dtype=np.uint64) * max_entries).astype(np.uint32)
+    ent = np.zeros(max(1, n * max_entries), np.uint32)
+    counts = np.zeros(n, np.uint32)
+    stop = np.zeros(n, np.uint32)
+    lib().orc_trace_pixels(*args, _p(cv), C.c_int(n), _p(px), _p(off), _p(ent), _p(counts), _p(stop))
+    assert n == 0 or counts.max() <= max_entries
+    # compact to CSR
+    offsets = np.zeros(n + 1, np.uint32)
+    offsets[1:] = np.cumsum(counts)
+    entries = np.concatenate([ent[off[k]:off[k] + counts[k]] for k in range(n)]) if n else np.zeros(0, np.uint32)
+    return dict(pixels=px, offsets=offsets, entries=entries.astype(np.uint32), stop_pos=stop, counts=counts)
+
+
+def render_backward(scene, cam, dL_dimage, inject: dict | None = None) -> dict:
+    """Forward + analytic backward.  `inject` (decision-injected mode, reading C18): dict with
+    pixels [n][2] int32 (x, y), offsets [n+1] uint32, entries uint32 (1-based list positions of the blended
+    entries, bit 31 = clamp active), stop_pos [n] uint32, delta (relative margin).  The result then carries
+    `violations`: the number of injected outcomes that are not correct renderings within delta (must be 0)."""
     keep, args = _scene_args(scene)
     cv = cam_vector(cam)
     N, K, H, W = scene.N, scene.K, cam.height, cam.width
     g = np.ascontiguousarray(dL_dimage, np.float32)
     assert g.shape == (3, H, W)
-    o = dict(image=np.zeros((3, H, W)), d_means=np.zeros((N, 3)), d_scales=np.zeros((N, 3)),
+    o = dict(image=np.zeros((3, H, W)), final_T=np.zeros((H, W)), n_contrib=np.zeros((H, W), np.uint32),
+             d_means=np.zeros((N, 3)), d_scales=np.zeros((N, 3)),
              d_rotations=np.zeros((N, 4)), d_opacities=np.zeros(N), d_sh=np.zeros((N, 16, 3)),
              d_freqs=np.zeros((N, K, 3)), d_weights=np.zeros((N, K)), d_mean2d=np.zeros((N, 2)),
              d_conic=np.zeros((N, 3)), d_rgb=np.zeros((N, 3)), d_freq2d=np.zeros((N, K, 2)),
              d_absmean2d=np.zeros((N, 2)))
-    lib().orc_render_backward(*args, _p(cv), _p(g), *[_p(o[k]) for k in (
-        "image", "d_means", "d_scales", "d_rotations", "d_opacities", "d_sh", "d_freqs", "d_weights",
-        "d_mean2d", "d_conic", "d_rgb", "d_freq2d", "d_absmean2d")])
+    viol = np.zeros(1, np.uint64)
+    if inject is not None and len(inject["pixels"]):
+        px = np.ascontiguousarray(inject["pixels"], np.int32).reshape(-1, 2)
+        off = np.ascontiguousarray(inject["offsets"], np.uint32)
+        ent = np.ascontiguousarray(inject["entries"], np.uint32)
+        stop = np.ascontiguousarray(inject["stop_pos"], np.uint32)
+        assert off.shape == (px.shape[0] + 1,) and stop.shape == (px.shape[0],) and ent.size >= int(off[-1])
+        assert np.all(px[:, 0] >= 0) and np.all(px[:, 0] < W) and np.all(px[:, 1] >= 0) and np.all(px[:, 1] < H)
+        inj = [C.c_int(px.shape[0]), _p(px), _p(off), _p(ent), _p(stop), C.c_double(float(inject["delta"])), _p(viol)]
+    else:
+        inj = [C.c_int(0), None, None, None, None, C.c_double(0.0), _p(viol)]
+    lib().orc_render_backward_ex(*args, _p(cv), _p(g), *[_p(o[k]) for k in (
+        "image", "final_T", "n_contrib", "d_means", "d_scales", "d_rotations", "d_opacities", "d_sh", "d_freqs",
+        "d_weights", "d_mean2d", "d_conic", "d_rgb", "d_freq2d", "d_absmean2d")], *inj)
+    o["violations"] = int(viol[0])
     return o

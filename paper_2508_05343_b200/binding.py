@@ -117,6 +117,13 @@ def lib():
                                            C.POINTER(C.c_int32)]
         L.gabsplat_count_pairs.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
                                            C.POINTER(_Binning), P, P]
+        L.gabsplat_trace_pixels.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
+                                            C.POINTER(_Binning), C.c_int32, P, P, P, P, P, P]
+        L.gabsplat_trace_pixels.restype = C.c_int32
+        L.gabsplat_probe_sincos.argtypes = [P, C.c_int32, P, P, P, P]
+        L.gabsplat_probe_sincos.restype = C.c_int32
+        L.gabsplat_measure_peaks.argtypes = [P, C.POINTER(C.c_float), P]
+        L.gabsplat_measure_peaks.restype = C.c_int32
         for f in (L.gabsplat_preprocess, L.gabsplat_bin_sort, L.gabsplat_render_forward, L.gabsplat_render_backward,
                   L.gabsplat_render_host, L.gabsplat_timing_enable, L.gabsplat_timing_read, L.gabsplat_count_pairs):
             f.restype = C.c_int32
@@ -456,6 +463,43 @@ def gabsplat_count_pairs(ctx: Context, scene: DeviceScene, cam, proj: Projected,
     s, c, p, b = scene.struct(), camera_struct(cam), proj.struct(), bin.struct()
     ctx.check(lib().gabsplat_count_pairs(ctx._h, C.byref(s), C.byref(c), C.byref(p), C.byref(b), _ptr(out),
                                          _stream(stream)))
+    return out
+
+
+def gabsplat_trace_pixels(ctx: Context, scene: DeviceScene, cam, proj: Projected, bin: Binning, pixels: torch.Tensor,
+                          offsets: torch.Tensor, stream=None):
+    """The forward's decisions at the pixels [n][2] (x, y) int32: returns (entries, colour_T [n][4], info [n][4]);
+    entries[offsets[i]:offsets[i+1]] = 1-based list positions of the entries blended at pixel i (bit 31: clamp active)."""
+    dev = scene.means.device
+    n = int(pixels.shape[0])
+    assert pixels.dtype == torch.int32 and pixels.is_contiguous() and offsets.dtype == torch.int32 and offsets.numel() == n + 1
+    entries = torch.zeros((max(1, int(offsets[-1].item())),), dtype=torch.int32, device=dev)
+    colour_T = torch.zeros((max(n, 1), 4), dtype=torch.float32, device=dev)
+    info = torch.zeros((max(n, 1), 4), dtype=torch.int32, device=dev)
+    s, c, p, b = scene.struct(), camera_struct(cam), proj.struct(), bin.struct()
+    ctx.check(lib().gabsplat_trace_pixels(ctx._h, C.byref(s), C.byref(c), C.byref(p), C.byref(b), n, _ptr(pixels),
+                                          _ptr(offsets), _ptr(entries), _ptr(colour_T), _ptr(info), _stream(stream)))
+    return entries, colour_T[:n], info[:n]
+
+
+def gabsplat_probe_sincos(ctx: Context, phase: torch.Tensor, stream=None):
+    """(cos, sin) of raw radian phases as the blend kernels evaluate them."""
+    assert phase.dtype == torch.float32 and phase.is_contiguous()
+    c, s = torch.empty_like(phase), torch.empty_like(phase)
+    ctx.check(lib().gabsplat_probe_sincos(ctx._h, phase.numel(), _ptr(phase), _ptr(c), _ptr(s), _stream(stream)))
+    return c, s
+
+
+PEAK_NAMES = ("ffma", "ffma2", "mufu_ex2", "mufu_cos", "mix_4ffma_1mufu", "alu_iadd")
+
+
+def gabsplat_measure_peaks(ctx: Context, stream=None) -> dict:
+    """Measured ALU rooflines of this device: lane-instructions (lane-ops) per second and per SM per clock."""
+    r = (C.c_float * 16)()
+    ctx.check(lib().gabsplat_measure_peaks(ctx._h, r, _stream(stream)))
+    out = {n: float(r[i]) for i, n in enumerate(PEAK_NAMES)}
+    out.update({n + "_per_sm_clk": float(r[8 + i]) for i, n in enumerate(PEAK_NAMES)})
+    out["sm_clock_hz"], out["sms"] = float(r[6]), int(r[7])
     return out
 
 

@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "_obj")
 LIB = os.path.join(HERE, "libgabsplat.so")
 SOURCES = ["api.cu", "host_api.cu", "preprocess.cu", "binning.cu", "blend_forward.cu", "blend_backward.cu",
-           "preprocess_backward.cu", "loss.cu"]
+           "preprocess_backward.cu", "loss.cu", "peaks.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

@@ -11,12 +11,13 @@ struct gabsplat_ctx {
   uint64_t* pinned_count;  // 8-byte pinned readback slot for D
   cudaStream_t side;       // side stream: the zeroing of the gradient arrays overlaps the blend backward
   cudaEvent_t ev_fork, ev_join;
+  void* scratch;           // 256 bytes of device scratch (instrumentation)
   gabsplat::StageTimer timer;
   char error[256];
 };
 
 namespace gabsplat {
-unsigned long long g_kernel_launches = 0;
+std::atomic<unsigned long long> g_kernel_launches{0};
 }
 
 namespace {
@@ -37,7 +38,8 @@ int32_t cuda_fail(gabsplat_ctx* ctx, cudaError_t e, const char* where) {
 }
 
 bool camera_ok(const gabsplat_camera* c) {
-  return c && c->width > 0 && c->height > 0 && c->fx > 0.f && c->fy > 0.f &&
+  // z_near > 0 (also rejects NaN): the depth key orders bits(t_z) as unsigned integers, valid for positive floats only
+  return c && c->width > 0 && c->height > 0 && c->fx > 0.f && c->fy > 0.f && c->z_near > 0.f &&
          (int64_t)((c->width + kTile - 1) / kTile) * ((c->height + kTile - 1) / kTile) < (1 << 30);
 }
 
@@ -89,8 +91,9 @@ int32_t gabsplat_create(gabsplat_ctx** out, int32_t device) {
     delete ctx;
     return GABSPLAT_CUDA;
   }
-  ctx->side = nullptr; ctx->ev_fork = ctx->ev_join = nullptr;
-  if (cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
+  ctx->side = nullptr; ctx->ev_fork = ctx->ev_join = nullptr; ctx->scratch = nullptr;
+  if (cudaMalloc(&ctx->scratch, 256) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess) {
     gabsplat_destroy(ctx);
@@ -107,6 +110,7 @@ void gabsplat_destroy(gabsplat_ctx* ctx) {
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->side) cudaStreamDestroy(ctx->side);
+  if (ctx->scratch) cudaFree(ctx->scratch);
   ctx->timer.destroy();
   delete ctx;
 }
@@ -254,9 +258,10 @@ int32_t gabsplat_render_backward(gabsplat_ctx* ctx, const gabsplat_scene* scene,
   e = launch_blend_backward(scene->N, scene->K, grads->d_mean2d_abs != nullptr, c, *proj, *bin, *fwd, saved,
                                         dL_dimage, grad2d, st);
   ctx->timer.end(st);
+  // join the side stream on every path: a later call must never race the zeroing of the gradient arrays
+  const cudaError_t ej = cudaStreamWaitEvent(st, ctx->ev_join, 0);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "render_backward (blend)");
-  e = cudaStreamWaitEvent(st, ctx->ev_join, 0);
-  if (e != cudaSuccess) return cuda_fail(ctx, e, "render_backward (join)");
+  if (ej != cudaSuccess) return cuda_fail(ctx, ej, "render_backward (join)");
   ctx->timer.begin(GABSPLAT_STAGE_PREPROCESS_BACKWARD, st);
   e = launch_preprocess_backward(*scene, c, *proj, *bin, grad2d, *grads, st);
   ctx->timer.end(st);
@@ -305,7 +310,35 @@ int32_t gabsplat_loss(gabsplat_ctx* ctx, int32_t width, int32_t height, const fl
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "loss");
 }
 
-uint64_t gabsplat_kernel_launches(void) { return g_kernel_launches; }
+uint64_t gabsplat_kernel_launches(void) { return g_kernel_launches.load(std::memory_order_relaxed); }
+
+int32_t gabsplat_trace_pixels(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                              const gabsplat_projected* proj, const gabsplat_binning* bin, int32_t n, const int32_t* pixels,
+                              const uint32_t* offsets, uint32_t* entries, float* colour_T, uint32_t* info, void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  if (!scene || scene->K < 0 || scene->K > kMaxK || scene->N < 0) return fail(ctx, GABSPLAT_INVALID_ARG, "trace_pixels: bad scene");
+  if (!camera_ok(cam)) return fail(ctx, GABSPLAT_INVALID_ARG, "trace_pixels: bad camera");
+  if (!proj || (scene->N > 0 && !proj->packed)) return fail(ctx, GABSPLAT_INVALID_ARG, "trace_pixels: null packed records");
+  if (!bin || !bin->tile_ranges || (bin->capacity > 0 && !bin->ids)) return fail(ctx, GABSPLAT_INVALID_ARG, "trace_pixels: bad binning");
+  if (n < 0 || (n > 0 && (!pixels || !offsets || !entries || !colour_T || !info)))
+    return fail(ctx, GABSPLAT_INVALID_ARG, "trace_pixels: null argument");
+  const cudaError_t e = launch_trace_pixels(scene->K, make_camera(*cam), *proj, *bin, n, pixels, offsets, entries, colour_T, info,
+                                            (cudaStream_t)stream);
+  return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "trace_pixels");
+}
+
+int32_t gabsplat_probe_sincos(gabsplat_ctx* ctx, int32_t n, const float* phase, float* cos_out, float* sin_out, void* stream) {
+  if (!ctx) return GABSPLAT_INVALID_ARG;
+  if (n < 0 || (n > 0 && (!phase || !cos_out || !sin_out))) return fail(ctx, GABSPLAT_INVALID_ARG, "probe_sincos: null argument");
+  const cudaError_t e = launch_probe_sincos(n, phase, cos_out, sin_out, (cudaStream_t)stream);
+  return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "probe_sincos");
+}
+
+int32_t gabsplat_measure_peaks(gabsplat_ctx* ctx, float* results_host, void* stream) {
+  if (!ctx || !results_host) return GABSPLAT_INVALID_ARG;
+  const cudaError_t e = measure_peaks(results_host, ctx->scratch, (cudaStream_t)stream);
+  return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "measure_peaks");
+}
 
 int32_t gabsplat_timing_enable(gabsplat_ctx* ctx, int32_t on) {
   if (!ctx) return GABSPLAT_INVALID_ARG;

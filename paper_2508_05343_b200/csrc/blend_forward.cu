@@ -225,3 +225,116 @@ cudaError_t launch_count_pairs(int K, const Camera& cam, const gabsplat_projecte
 }
 
 }  // namespace gabsplat
+
+// ---- instrumentation: the forward's decisions at selected pixels ---------------------------------------
+// gabsplat_trace_pixels: one thread per selected pixel walks its tile's list with the forward kernel's own functions
+// (blend_common.cuh: same operands, same round-to-nearest operation sequence, so every alpha, every skip / stop
+// decision and the accumulated colour are bit-identical to blend_forward_kernel's) and writes the 1-based list
+// position of every entry it blends, bit 31 set when min(0.99, .) was active (what the backward reads as "zero
+// derivative").  The parity tests hand these decisions to the oracle at the pixels whose decisions sit within
+// fp32 error of a threshold (reading C18) and compare the trace's colour with the image bit for bit.
+namespace gabsplat {
+namespace {
+
+template <int K>
+__global__ void __launch_bounds__(128) trace_pixels_kernel(Camera cam, const uint2* __restrict__ ranges,
+                                                           const uint32_t* __restrict__ ids, const float4* __restrict__ packed,
+                                                           int n, const int2* __restrict__ pixels,
+                                                           const uint32_t* __restrict__ offsets, uint32_t* __restrict__ entries,
+                                                           float4* __restrict__ colour_T, uint4* __restrict__ info) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  constexpr int R4 = packed_floats(K) / 4;
+  constexpr int TL = K > 0 ? tail_floats(K) : 1;
+  const int2 p = pixels[i];
+  const int tx = p.x / kTile, ty = p.y / kTile;
+  const uint2 range = ranges[ty * cam.tiles_x + tx];
+  const float x0 = (float)(tx * kTile), y0 = (float)(ty * kTile);
+  const float lx = (float)(p.x - tx * kTile), ly = (float)(p.y - ty * kTile);
+  const uint32_t cap = offsets[i + 1] - offsets[i];
+  uint32_t* out = entries + offsets[i];
+  float T = 1.0f, Cr = 0.f, Cg = 0.f, Cb = 0.f;
+  uint32_t last = 0, stop = 0, nb = 0;
+  for (uint32_t e = range.x; e < range.y; ++e) {
+    const uint32_t id = ids[e];
+    const float4* rec = packed + (size_t)id * R4;
+    const float4 a = rec[0], l = rec[1], oc = rec[2];
+    const float mx = __fadd_rn(__fsub_rn(a.x, x0), a.z), my = __fadd_rn(__fsub_rn(a.y, y0), a.w);
+    const float dx = __fsub_rn(lx, mx), dy = __fsub_rn(ly, my);
+    const float ux = __fmul_rn(l.x, dx);
+    float u, v;
+    const float q = envelope_q(ux, l.y, l.z, dy, u, v);
+    if (q < l.w) continue;  // envelope reject
+    float tail[TL];
+    if (K > 0) load_tail<K>(rec, tail);
+    ModulationEntry<K> me;
+    modulation_entry<K>(tail, dx, me);
+    Modulation<K> m;
+    modulation<K, false>(tail, me, dy, m);
+    const float raw = __fmul_rn(__fmul_rn(oc.x, envelope_exp2(q)), m.M);
+    const float alpha = fminf(kAlphaMax, raw);
+    if (!(alpha >= kAlphaMin)) continue;
+    const uint32_t pos = e - range.x + 1u;
+    const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
+    if (Tn < kTMin) { stop = pos; break; }
+    const float wgt = __fmul_rn(alpha, T);
+    Cr = __fmaf_rn(oc.y, wgt, Cr);
+    Cg = __fmaf_rn(oc.z, wgt, Cg);
+    Cb = __fmaf_rn(oc.w, wgt, Cb);
+    T = Tn;
+    last = pos;
+    if (nb < cap) out[nb] = pos | (raw > kAlphaMax ? 0x80000000u : 0u);
+    ++nb;
+  }
+  colour_T[i] = make_float4(__fmaf_rn(T, cam.bg[0], Cr), __fmaf_rn(T, cam.bg[1], Cg), __fmaf_rn(T, cam.bg[2], Cb), T);
+  info[i] = make_uint4(last, nb, stop, 0u);
+}
+
+}  // namespace
+
+cudaError_t launch_trace_pixels(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, int n,
+                                const int32_t* pixels, const uint32_t* offsets, uint32_t* entries, float* colour_T,
+                                uint32_t* info, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  const dim3 grid((n + 127) / 128), block(128);
+#define GABSPLAT_TRACE(KK)                                                                                              \
+  case KK:                                                                                                              \
+    trace_pixels_kernel<KK><<<grid, block, 0, st>>>(cam, reinterpret_cast<const uint2*>(bin.tile_ranges), bin.ids,      \
+                                                    reinterpret_cast<const float4*>(proj.packed), n,                    \
+                                                    reinterpret_cast<const int2*>(pixels), offsets, entries,            \
+                                                    reinterpret_cast<float4*>(colour_T), reinterpret_cast<uint4*>(info)); \
+    break;
+  switch (K) {
+    GABSPLAT_TRACE(0) GABSPLAT_TRACE(1) GABSPLAT_TRACE(2) GABSPLAT_TRACE(3) GABSPLAT_TRACE(4)
+    GABSPLAT_TRACE(5) GABSPLAT_TRACE(6) GABSPLAT_TRACE(7) GABSPLAT_TRACE(8)
+    default: return cudaErrorInvalidValue;
+  }
+#undef GABSPLAT_TRACE
+  launched();
+  return cudaGetLastError();
+}
+
+// instrumentation: cos / sin of a raw radian phase exactly as modulation<> evaluates them (the MUFU path)
+namespace {
+__global__ void __launch_bounds__(256) probe_sincos_kernel(int n, const float* __restrict__ phase, float* __restrict__ c,
+                                                           float* __restrict__ s) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float tail[4] = {0.f, 1.0f, 1.0f, 0.f};  // K = 1: (2 pi f2D.x, 2 pi f2D.y, omega)
+  ModulationEntry<1> me;
+  modulation_entry<1>(tail, 0.f, me);
+  Modulation<1> m;
+  modulation<1, true>(tail, me, phase[i], m);  // phase = fma(1, phase, 0)
+  c[i] = m.cs[0];
+  s[i] = m.sn[0];
+}
+}  // namespace
+
+cudaError_t launch_probe_sincos(int n, const float* phase, float* c, float* s, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  probe_sincos_kernel<<<(n + 255) / 256, 256, 0, st>>>(n, phase, c, s);
+  launched();
+  return cudaGetLastError();
+}
+
+}  // namespace gabsplat

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <vector>
 
 #include "../../include/gabsplat.h"
@@ -135,8 +136,8 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 }
 
 // Number of kernels launched by this library since it was loaded (gabsplat_kernel_launches).
-extern unsigned long long g_kernel_launches;
-inline void launched(int n = 1) { g_kernel_launches += (unsigned long long)n; }
+extern std::atomic<unsigned long long> g_kernel_launches;
+inline void launched(int n = 1) { g_kernel_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
 
 // ---- launchers (one per .cu file); each returns the cudaError_t of its last launch ---------------
 cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& out,
@@ -168,6 +169,13 @@ cudaError_t launch_half_tile_order(const uint32_t* work, int n, uint32_t* order,
 uint64_t loss_workspace_bytes(int W, int H);
 cudaError_t launch_loss(int W, int H, const float* image, const float* target, float lambda, float* loss_out,
                         float* dL_dimage, void* workspace, cudaStream_t st);
+
+// instrumentation (blend_forward.cu, peaks.cu)
+cudaError_t launch_trace_pixels(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, int n,
+                                const int32_t* pixels, const uint32_t* offsets, uint32_t* entries, float* colour_T,
+                                uint32_t* info, cudaStream_t st);
+cudaError_t launch_probe_sincos(int n, const float* phase, float* c, float* s, cudaStream_t st);
+cudaError_t measure_peaks(float* results_host, void* scratch, cudaStream_t st);
 
 uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles);
 bool keys_optional(int ntiles);  // true when the binning never reads gabsplat_binning.keys itself
