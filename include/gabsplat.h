@@ -83,8 +83,10 @@ typedef struct {
   const float* weights;   /* [N][K]     omega_{k,i}  (Eq.7)                          */
 } gabsplat_scene;
 
-/* Outputs of gabsplat_preprocess, one entry per primitive.  Entries of culled primitives are zero
- * (tiles_touched == 0 marks a culled primitive).  `packed` is the record the blend kernels gather. */
+/* Outputs of gabsplat_preprocess, one entry per primitive.  tiles_touched and radius are written for every
+ * primitive (0 = culled); every other array is written for the VISIBLE primitives only -- rows of culled primitives
+ * are left untouched (unspecified; nothing in the library reads them).  `packed` is the record the blend kernels
+ * gather. */
 typedef struct {
   float* mean2d;           /* [N][2]  mu2D in pixels (:99)                                         */
   float* depth;            /* [N]     camera-space t_z; its bit pattern is the low half of the key */
@@ -158,7 +160,8 @@ typedef struct {
  * records it wrote), so the caller zeroes it once, after allocating it. */
 uint64_t gabsplat_grad_workspace_bytes(int32_t N, int32_t K);
 
-/* S1.  Writes every array of `out` for all N primitives. */
+/* S1.  Writes tiles_touched, radius and chunk_visible for all N primitives and every other array of
+ * `out` for the visible ones (see gabsplat_projected). */
 int32_t gabsplat_preprocess(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
                             gabsplat_projected* out, void* stream);
 
@@ -280,6 +283,10 @@ int32_t gabsplat_trace_pixels(gabsplat_ctx* ctx, const gabsplat_scene* scene, co
  * (:158): the MUFU path, no explicit range reduction.  For the committed measurement of its error bound
  * (DESIGN.md "Tolerances"). */
 int32_t gabsplat_probe_sincos(gabsplat_ctx* ctx, int32_t n, const float* phase, float* cos_out, float* sin_out, void* stream);
+
+/* The placement pass of gabsplat_bin_sort works on bands of tile rows; bands > 0 forces that many bands (so that a
+ * test can run the multi-band code on a small image), 0 restores the automatic choice.  Results never depend on it. */
+int32_t gabsplat_set_place_bands(gabsplat_ctx* ctx, int32_t bands);
 
 /* The ALU rooflines of the blend kernels measured on this device: results_host[16] (HOST) =
  *   [0] FFMA lane-instructions/s   [1] packed FFMA2 lane-instructions/s   [2] MUFU.EX2 lane-ops/s

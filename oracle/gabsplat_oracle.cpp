@@ -48,9 +48,24 @@ constexpr double ALPHA_MIN = 1.0 / 255.0; // reading C8
 constexpr double T_MIN = 1e-4;            // reading C8
 constexpr double TWO_PI = 6.283185307179586476925286766559;
 
+// Variants of the primitive, bit flags:
+//  VARIANT_LINE_INTEGRAL  keep the per-component amplitude of the exact line integral along the ray that Eq.12 drops
+//      (Eq.25-27): component k is attenuated by C2_k = exp(-2 pi^2 (f_z'')^2 / S22), f_z'' the z
+//      component of f_proj (Eq.9) and S22 the zz entry of the inverse ray-space covariance (Eq.19).  The constants
+//      printed at :483 are garbled (C2 is printed with a positive exponent, C1 as a reciprocal); completing the
+//      square in Eq.24 gives the value used here (reading C4; pinned by the z-quadrature test).  The
+//      common factor C1 is dropped as in Eq.12, so the Gaussian term keeps weight 1 - sum w and a primitive with
+//      f = 0 is unchanged:  M = (1 - sum_k w_k) + sum_k w_k C2_k cos(phi_k).
+//  VARIANT_MIP_FILTER     the 2D Mip filter of Mip-Splatting in place of the 0.3 px^2 dilation (the
+//      "+Mip-Splatting+AbsGS" variant): the 2D covariance is dilated by 0.1 px^2 and the opacity is scaled by
+//      sqrt(det U / det(U + 0.1 I)) so that the splat keeps its integral.
+constexpr int VARIANT_LINE_INTEGRAL = 1, VARIANT_MIP_FILTER = 2;
+constexpr double MIP_DILATION = 0.1;
+
 struct Scene {
     int N, K, deg;
     const float *means, *scales, *quats, *opac, *sh, *freqs, *weights;
+    int variant = 0;
 };
 
 struct Cam {
@@ -133,7 +148,8 @@ Twin twin_index(const Scene& s, const Cam& c, int i) {
     const float U00 = std::fmaf(V[0][2], T[0][2], std::fmaf(V[0][1], T[0][1], V[0][0] * T[0][0]));
     const float U01 = std::fmaf(V[0][2], T[1][2], std::fmaf(V[0][1], T[1][1], V[0][0] * T[1][0]));
     const float U11 = std::fmaf(V[1][2], T[1][2], std::fmaf(V[1][1], T[1][1], V[1][0] * T[1][0]));
-    const float A = U00 + 0.3f, C = U11 + 0.3f;
+    const float dil = (s.variant & VARIANT_MIP_FILTER) ? 0.1f : 0.3f;
+    const float A = U00 + dil, C = U11 + dil;
     const float det = A * C - U01 * U01;
     if (!(det > 0.0f)) return o;
     // lambda_max = mid + sqrt(((A-C)/2)^2 + B^2)   (reading C9); radius = ceil(3 sqrt(lambda_max))
@@ -234,6 +250,9 @@ struct Proj {
     double dir[3], vlen;
     // exposed for the pins of Eq.9-11 / Eq.16-17
     double A3[3][3], fproj[KMAX][3], Sig3[3][3];
+    // variants (f4): att[k] = C2_k, computed for every primitive; att_used[k] = what the render multiplies w_k by
+    // (C2_k or 1); rho = Mip opacity factor (1 without the variant); o_eff = o * rho
+    double att[KMAX], att_used[KMAX], rho, o_eff, dilation;
 };
 
 void project_values(const Scene& s, const Cam& c, int i, int third_row, Proj& p) {
@@ -269,9 +288,13 @@ void project_values(const Scene& s, const Cam& c, int i, int third_row, Proj& p)
     p.U[1] = V[0][0] * p.T[1][0] + V[0][1] * p.T[1][1] + V[0][2] * p.T[1][2];
     p.U[2] = V[1][0] * p.T[1][0] + V[1][1] * p.T[1][1] + V[1][2] * p.T[1][2];
     // conic of the dilated 2D covariance                                            PAPER.md:101 Eq.3, reading C5
-    const double A = p.U[0] + DILATION, B = p.U[1], C = p.U[2] + DILATION;
+    p.dilation = (s.variant & VARIANT_MIP_FILTER) ? MIP_DILATION : DILATION;
+    const double A = p.U[0] + p.dilation, B = p.U[1], C = p.U[2] + p.dilation;
     const double det = A * C - B * B;
     p.conic[0] = C / det; p.conic[1] = -B / det; p.conic[2] = A / det;
+    // Mip filter: opacity factor sqrt(det U / det(U + 0.1 I))
+    p.rho = (s.variant & VARIANT_MIP_FILTER) ? std::sqrt(std::max(0.0, (p.U[0] * p.U[2] - p.U[1] * p.U[1]) / det)) : 1.0;
+    p.o_eff = (double)s.opac[i] * p.rho;
     // mu2D
     p.mean2d[0] = c.fx * p.t[0] / tz + c.cx;
     p.mean2d[1] = c.fy * p.t[1] / tz + c.cy;
@@ -301,9 +324,12 @@ void project_values(const Scene& s, const Cam& c, int i, int third_row, Proj& p)
         if (okA && okS) {
             p.f2d[k][0] = p.fproj[k][0] - S[0][2] / S[2][2] * p.fproj[k][2];            // Eq.10 / Eq.29
             p.f2d[k][1] = p.fproj[k][1] - S[1][2] / S[2][2] * p.fproj[k][2];
+            p.att[k] = std::exp(-2.0 * (TWO_PI / 2) * (TWO_PI / 2) * p.fproj[k][2] * p.fproj[k][2] / S[2][2]);  // C2_k
         } else {
             p.f2d[k][0] = p.f2d[k][1] = 0.0;
+            p.att[k] = 1.0;
         }
+        p.att_used[k] = (s.variant & VARIANT_LINE_INTEGRAL) ? p.att[k] : 1.0;
     }
     // colour from SH at the viewing direction (reading C22, C8)
     double cam_pos[3];
@@ -357,7 +383,7 @@ inline void eval_pair(const Scene& s, const Proj& p, int i, double px, double py
     const double q = -0.5 * (p.conic[0] * e.dx * e.dx + p.conic[2] * e.dy * e.dy) - p.conic[1] * e.dx * e.dy;  // Eq.3
     e.power_pos = q > 0.0;
     e.G = std::exp(q);
-    const double o = s.opac[i];
+    const double o = p.o_eff;
     e.envelope_pass = o * e.G >= ALPHA_MIN;
     double wsum = 0.0, mod = 0.0;
     for (int k = 0; k < s.K; ++k) {
@@ -366,7 +392,7 @@ inline void eval_pair(const Scene& s, const Proj& p, int i, double px, double py
         e.cosv[k] = std::cos(phi);
         e.sinv[k] = std::sin(phi);
         wsum += w;
-        mod += w * e.cosv[k];
+        mod += w * p.att_used[k] * e.cosv[k];
     }
     e.M = (1.0 - wsum) + mod;                                                           // Eq.12 bracket
     e.raw = o * e.G * e.M;
@@ -535,6 +561,7 @@ void forward_painter(const Scene& s, const Cam& c, const std::vector<Proj>& P, c
 // ---------------------------------------------------------------------------------------------
 struct Grad2D {
     double rgb[3], o, conic[3], mean2d[2], f2d[KMAX][2], w[KMAX], absmean2d[2];
+    double att[KMAX];   // dL/d att_used[k] (line-integral variant)
 };
 
 void backward_pixels(const Scene& s, const Cam& c, const std::vector<Proj>& P, const std::vector<int>& ord,
@@ -606,8 +633,8 @@ void backward_pixels(const Scene& s, const Cam& c, const std::vector<Proj>& P, c
                         Bc[3 * l + ch] = e.alpha * p.rgb[ch] + (1.0 - e.alpha) * Bc[3 * l + ch];
                     }
                     if (clamp_active) continue;                  // clamp active: zero derivative (reading C14)
-                    const double o = s.opac[i];
-                    acc.o += galpha * e.G * e.M;
+                    const double o = p.o_eff;
+                    acc.o += galpha * e.G * e.M;                 // dL/d o_eff
                     const double gG = galpha * o * e.M, gM = galpha * o * e.G;
                     const double gq = gG * e.G;
                     double gdx = gq * (-p.conic[0] * e.dx - p.conic[1] * e.dy);
@@ -617,8 +644,9 @@ void backward_pixels(const Scene& s, const Cam& c, const std::vector<Proj>& P, c
                     acc.conic[2] += gq * (-0.5 * e.dy * e.dy);
                     for (int k = 0; k < s.K; ++k) {
                         const double w = s.weights[(size_t)i * s.K + k];
-                        acc.w[k] += gM * (e.cosv[k] - 1.0);
-                        const double gphi = -gM * w * e.sinv[k];
+                        acc.w[k] += gM * (p.att_used[k] * e.cosv[k] - 1.0);
+                        acc.att[k] += gM * w * e.cosv[k];
+                        const double gphi = -gM * w * p.att_used[k] * e.sinv[k];
                         acc.f2d[k][0] += gphi * TWO_PI * e.dx;
                         acc.f2d[k][1] += gphi * TWO_PI * e.dy;
                         gdx += gphi * TWO_PI * p.f2d[k][0];
@@ -663,6 +691,45 @@ void backward_primitive(const Scene& s, const Cam& c, const Proj& p, int i, cons
     // f2D_k = U^-1 T Sigma f_k (U undilated; closed form of Eq.9-10, reading C2)
     const double Ud = p.U[0] * p.U[2] - p.U[1] * p.U[1];
     const double Ui[2][2] = {{p.U[2] / Ud, -p.U[1] / Ud}, {-p.U[1] / Ud, p.U[0] / Ud}};
+    // Mip filter: o_eff = o rho, rho = sqrt(det U / det U_d):  d rho = rho/2 tr((U^-1 - U_d^-1) dU)
+    double g_opacity = g.o;
+    if (s.variant & VARIANT_MIP_FILTER) {
+        g_opacity = g.o * p.rho;
+        const double grho = g.o * (double)s.opac[i];
+        for (int r = 0; r < 2; ++r) for (int q = 0; q < 2; ++q) GU[r][q] += grho * p.rho * 0.5 * (Ui[r][q] - Cm[r][q]);
+    }
+    // line-integral attenuation: att_k = exp(-2 pi^2 a_k^2 / b), a_k = v . f_k, b = v^T Sigma^-1 v, where v spans the
+    // null space of T = J W (the world-space direction of the ray): (f_z'')^2 / S22 = (v.f)^2 / (v^T Sigma^-1 v) for
+    // any completion of J (reading C2); v = W^T (u_x, u_y, 1), (u_x, u_y) the clamped ray direction of J.
+    double g_freq_extra[KMAX][3] = {{0}};
+    double gt_extra[3] = {0, 0, 0};
+    if ((s.variant & VARIANT_LINE_INTEGRAL) && K > 0) {
+        const double tz0 = p.t[2];
+        const double lx = 1.3 * (0.5 * c.W / c.fx), ly = 1.3 * (0.5 * c.H / c.fy);
+        const double cdir[3] = {std::min(lx, std::max(-lx, p.t[0] / tz0)), std::min(ly, std::max(-ly, p.t[1] / tz0)), 1.0};
+        double v[3], y[3];
+        for (int m = 0; m < 3; ++m) v[m] = c.Wm[0][m] * cdir[0] + c.Wm[1][m] * cdir[1] + c.Wm[2][m] * cdir[2];
+        double Si[3][3];
+        inv3(p.Sigma, Si);
+        for (int m = 0; m < 3; ++m) y[m] = Si[m][0] * v[0] + Si[m][1] * v[1] + Si[m][2] * v[2];
+        const double b = v[0] * y[0] + v[1] * y[1] + v[2] * y[2];
+        double gv[3] = {0, 0, 0}, gb = 0.0;
+        const double PI2 = (TWO_PI / 2) * (TWO_PI / 2);
+        for (int k = 0; k < K; ++k) {
+            const float* f = s.freqs + (size_t)(i * K + k) * 3;
+            const double a = v[0] * f[0] + v[1] * f[1] + v[2] * f[2];
+            const double gatt = g.att[k] * p.att[k];                       // dL/d(ln att_k)
+            const double ga = gatt * (-4.0 * PI2 * a / b);
+            gb += gatt * (2.0 * PI2 * a * a / (b * b));
+            for (int m = 0; m < 3; ++m) { g_freq_extra[k][m] = ga * v[m]; gv[m] += ga * f[m]; }
+        }
+        for (int m = 0; m < 3; ++m) gv[m] += gb * 2.0 * y[m];
+        for (int m = 0; m < 3; ++m) for (int n = 0; n < 3; ++n) gSigma[m][n] -= gb * y[m] * y[n];   // d(Sigma^-1) = -Sigma^-1 dSigma Sigma^-1
+        double gc[3];
+        for (int a = 0; a < 3; ++a) gc[a] = c.Wm[a][0] * gv[0] + c.Wm[a][1] * gv[1] + c.Wm[a][2] * gv[2];
+        if (!p.clampx) { gt_extra[0] += gc[0] / tz0; gt_extra[2] -= gc[0] * p.t[0] / (tz0 * tz0); }
+        if (!p.clampy) { gt_extra[1] += gc[1] / tz0; gt_extra[2] -= gc[1] * p.t[1] / (tz0 * tz0); }
+    }
     for (int k = 0; k < K; ++k) {
         const float* f = s.freqs + (size_t)(i * K + k) * 3;
         const double gf[2] = {g.f2d[k][0], g.f2d[k][1]};
@@ -675,7 +742,7 @@ void backward_primitive(const Scene& s, const Cam& c, const Proj& p, int i, cons
         for (int m = 0; m < 3; ++m) for (int n = 0; n < 3; ++n) gSigma[m][n] += 0.5 * (Th[m] * f[n] + f[m] * Th[n]);
         for (int r = 0; r < 2; ++r) for (int m = 0; m < 3; ++m) gT[r][m] += h[r] * Sf[m];
         for (int m = 0; m < 3; ++m)
-            out.d_freqs[(size_t)(i * K + k) * 3 + m] = p.Sigma[m][0] * Th[0] + p.Sigma[m][1] * Th[1] + p.Sigma[m][2] * Th[2];
+            out.d_freqs[(size_t)(i * K + k) * 3 + m] = p.Sigma[m][0] * Th[0] + p.Sigma[m][1] * Th[1] + p.Sigma[m][2] * Th[2] + g_freq_extra[k][m];
         out.d_weights[(size_t)i * K + k] = g.w[k];
     }
     // U = T Sigma T^T
@@ -692,7 +759,7 @@ void backward_primitive(const Scene& s, const Cam& c, const Proj& p, int i, cons
     const double tx = p.t[0], ty = p.t[1], tz = p.t[2];
     const double limx = 1.3 * (0.5 * c.W / c.fx), limy = 1.3 * (0.5 * c.H / c.fy);
     const double ux = std::min(limx, std::max(-limx, tx / tz)), uy = std::min(limy, std::max(-limy, ty / tz));
-    double gt[3] = {0, 0, 0};
+    double gt[3] = {gt_extra[0], gt_extra[1], gt_extra[2]};
     gt[2] += gJ[0][0] * (-c.fx / (tz * tz)) + gJ[1][1] * (-c.fy / (tz * tz));
     gt[2] += gJ[0][2] * (c.fx * ux / (tz * tz)) + gJ[1][2] * (c.fy * uy / (tz * tz));
     if (!p.clampx) { gt[0] += gJ[0][2] * (-c.fx / (tz * tz)); gt[2] += gJ[0][2] * (c.fx * tx / (tz * tz * tz)); }
@@ -738,12 +805,14 @@ void backward_primitive(const Scene& s, const Cam& c, const Proj& p, int i, cons
     const double dg = p.dir[0] * gdir[0] + p.dir[1] * gdir[1] + p.dir[2] * gdir[2];
     for (int m = 0; m < 3; ++m) gmu[m] += (gdir[m] - p.dir[m] * dg) / p.vlen;
     for (int m = 0; m < 3; ++m) out.d_means[3 * i + m] = gmu[m];
-    out.d_opac[i] = g.o;
+    out.d_opac[i] = g_opacity;
 }
 
+// deg carries the SH degree in its low byte and the variant flags in the next one (the C interface keeps one
+// argument list for every entry point)
 Scene make_scene(int N, int K, int deg, const float* means, const float* scales, const float* quats,
                  const float* opac, const float* sh, const float* freqs, const float* weights) {
-    return Scene{N, K, deg, means, scales, quats, opac, sh, freqs, weights};
+    return Scene{N, K, deg & 0xff, means, scales, quats, opac, sh, freqs, weights, (deg >> 8) & 0xff};
 }
 
 }  // namespace
@@ -773,7 +842,8 @@ void orc_sh_basis(int n, const double* dirs, double* Y, double* dY) {
 void orc_project(SCENE_ARGS, const double* cam, int third_row,
                  uint8_t* visible, double* t, double* mean2d, double* cov2d, double* conic, double* freq2d,
                  double* rgb, uint8_t* clamped, uint32_t* depth_bits, float* mean2d_f32, int32_t* radius,
-                 int32_t* rect, uint32_t* tiles_touched, double* A3, double* fproj, double* Sigma3) {
+                 int32_t* rect, uint32_t* tiles_touched, double* A3, double* fproj, double* Sigma3,
+                 double* att, double* rho) {
     const Scene s = make_scene(SCENE_PASS);
     const Cam c = load_cam(cam);
     std::vector<Proj> P;
@@ -798,7 +868,9 @@ void orc_project(SCENE_ARGS, const double* cam, int third_row,
         for (int k = 0; k < K; ++k) {
             for (int a = 0; a < 2; ++a) if (freq2d) freq2d[(size_t)(i * K + k) * 2 + a] = v ? p.f2d[k][a] : 0;
             for (int a = 0; a < 3; ++a) if (fproj) fproj[(size_t)(i * K + k) * 3 + a] = v ? p.fproj[k][a] : 0;
+            if (att) att[(size_t)i * K + k] = v ? p.att[k] : 0;
         }
+        if (rho) rho[i] = v ? p.rho : 0;
         for (int a = 0; a < 9; ++a) {
             if (A3) A3[9 * i + a] = v ? p.A3[a / 3][a % 3] : 0;
             if (Sigma3) Sigma3[9 * i + a] = v ? p.Sig3[a / 3][a % 3] : 0;

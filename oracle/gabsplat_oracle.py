@@ -14,6 +14,8 @@ import sys
 
 import numpy as np
 
+VARIANT_LINE_INTEGRAL, VARIANT_MIP_FILTER = 1, 2     # scene.variant bit flags
+
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liboracle_gabsplat.so")
 _lib = None
@@ -53,7 +55,8 @@ def cam_vector(cam) -> np.ndarray:
 def _scene_args(scene):
     arrs = [np.ascontiguousarray(a, np.float32) for a in
             (scene.means, scene.scales, scene.rotations, scene.opacities, scene.sh, scene.freqs, scene.weights)]
-    return arrs, [C.c_int(scene.N), C.c_int(scene.K), C.c_int(scene.sh_degree)] + [_p(a) for a in arrs]
+    deg = int(scene.sh_degree) | (int(getattr(scene, "variant", 0)) << 8)     # variant flags ride in the second byte
+    return arrs, [C.c_int(scene.N), C.c_int(scene.K), C.c_int(deg)] + [_p(a) for a in arrs]
 
 
 def max_threads() -> int:
@@ -81,10 +84,11 @@ def project(scene, cam, third_row: int = 0) -> dict:
         conic=np.zeros((N, 3)), freq2d=np.zeros((N, K, 2)), rgb=np.zeros((N, 3)), clamped=np.zeros((N, 3), np.uint8),
         depth_bits=np.zeros(N, np.uint32), mean2d_f32=np.zeros((N, 2), np.float32), radius=np.zeros(N, np.int32),
         rect=np.zeros((N, 4), np.int32), tiles_touched=np.zeros(N, np.uint32),
-        A3=np.zeros((N, 3, 3)), fproj=np.zeros((N, K, 3)), Sigma3=np.zeros((N, 3, 3)))
+        A3=np.zeros((N, 3, 3)), fproj=np.zeros((N, K, 3)), Sigma3=np.zeros((N, 3, 3)),
+        att=np.zeros((N, K)), rho=np.zeros(N))
     lib().orc_project(*args, _p(cv), C.c_int(third_row), *[_p(o[k]) for k in (
         "visible", "t", "mean2d", "cov2d", "conic", "freq2d", "rgb", "clamped", "depth_bits", "mean2d_f32",
-        "radius", "rect", "tiles_touched", "A3", "fproj", "Sigma3")])
+        "radius", "rect", "tiles_touched", "A3", "fproj", "Sigma3", "att", "rho")])
     return o
 
 

@@ -122,6 +122,8 @@ def lib():
         L.gabsplat_trace_pixels.restype = C.c_int32
         L.gabsplat_probe_sincos.argtypes = [P, C.c_int32, P, P, P, P]
         L.gabsplat_probe_sincos.restype = C.c_int32
+        L.gabsplat_set_place_bands.argtypes = [P, C.c_int32]
+        L.gabsplat_set_place_bands.restype = C.c_int32
         L.gabsplat_measure_peaks.argtypes = [P, C.POINTER(C.c_float), P]
         L.gabsplat_measure_peaks.restype = C.c_int32
         for f in (L.gabsplat_preprocess, L.gabsplat_bin_sort, L.gabsplat_render_forward, L.gabsplat_render_backward,
@@ -488,6 +490,10 @@ def gabsplat_probe_sincos(ctx: Context, phase: torch.Tensor, stream=None):
     c, s = torch.empty_like(phase), torch.empty_like(phase)
     ctx.check(lib().gabsplat_probe_sincos(ctx._h, phase.numel(), _ptr(phase), _ptr(c), _ptr(s), _stream(stream)))
     return c, s
+
+
+def gabsplat_set_place_bands(ctx: Context, bands: int) -> None:
+    ctx.check(lib().gabsplat_set_place_bands(ctx._h, int(bands)))
 
 
 PEAK_NAMES = ("ffma", "ffma2", "mufu_ex2", "mufu_cos", "mix_4ffma_1mufu", "alu_iadd")

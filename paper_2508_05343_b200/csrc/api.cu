@@ -12,6 +12,7 @@ struct gabsplat_ctx {
   cudaStream_t side;       // side stream: the zeroing of the gradient arrays overlaps the blend backward
   cudaEvent_t ev_fork, ev_join;
   void* scratch;           // 256 bytes of device scratch (instrumentation)
+  int place_bands;         // 0 = automatic (gabsplat_set_place_bands)
   gabsplat::StageTimer timer;
   char error[256];
 };
@@ -92,6 +93,7 @@ int32_t gabsplat_create(gabsplat_ctx** out, int32_t device) {
     return GABSPLAT_CUDA;
   }
   ctx->side = nullptr; ctx->ev_fork = ctx->ev_join = nullptr; ctx->scratch = nullptr;
+  ctx->place_bands = 0;
   if (cudaMalloc(&ctx->scratch, 256) != cudaSuccess ||
       cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -182,7 +184,7 @@ int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected
       bin->workspace_bytes < gabsplat_sort_workspace_bytes(N, bin->capacity, cam->width, cam->height))
     return fail(ctx, GABSPLAT_CAPACITY, "bin_sort: workspace too small");
   cudaStream_t st = (cudaStream_t)stream;
-  cudaError_t e = launch_bin_sort(N, *proj, make_camera(*cam), *bin, ctx->timer, st);
+  cudaError_t e = launch_bin_sort(N, *proj, make_camera(*cam), *bin, ctx->timer, ctx->place_bands, st);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "bin_sort");
   if (num_instances_host) {
     uint32_t* slot = reinterpret_cast<uint32_t*>(ctx->pinned_count);
@@ -332,6 +334,12 @@ int32_t gabsplat_probe_sincos(gabsplat_ctx* ctx, int32_t n, const float* phase, 
   if (n < 0 || (n > 0 && (!phase || !cos_out || !sin_out))) return fail(ctx, GABSPLAT_INVALID_ARG, "probe_sincos: null argument");
   const cudaError_t e = launch_probe_sincos(n, phase, cos_out, sin_out, (cudaStream_t)stream);
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "probe_sincos");
+}
+
+int32_t gabsplat_set_place_bands(gabsplat_ctx* ctx, int32_t bands) {
+  if (!ctx || bands < 0) return GABSPLAT_INVALID_ARG;
+  ctx->place_bands = bands;
+  return GABSPLAT_OK;
 }
 
 int32_t gabsplat_measure_peaks(gabsplat_ctx* ctx, float* results_host, void* stream) {

@@ -17,7 +17,6 @@
 // The instance count D lives on the device: every kernel is launched on a grid sized from the caller's
 // capacity and returns early past D, so the whole stage runs without a host round trip.
 #include <algorithm>
-#include <cstdlib>
 
 #include "common.cuh"
 
@@ -564,9 +563,23 @@ __global__ void __launch_bounds__(1024) tile_order_kernel(const uint2* __restric
   }, ntiles, order);
 }
 
-__global__ void clamp_count_kernel(u32* sort_count, const u32* num_instances, u64 capacity) {
-  // the sort kernels see 0 instances when the caller's buffers are too small
-  *sort_count = (u64)*num_instances > capacity ? 0u : *num_instances;
+// D in 64 bits on the radix path: the 32-bit prefix sum of tiles_touched wraps at 2^32 instances, and a wrapped
+// count could pass every `D > capacity` guard.  total64 (zeroed before) accumulates the tile counts of the visible
+// primitives; clamp_count_kernel then overwrites *num_instances with the saturated value.
+__global__ void __launch_bounds__(256) instance_total_kernel(int N, const u32* __restrict__ tiles_touched,
+                                                              unsigned long long* __restrict__ total64) {
+  unsigned long long acc = 0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) acc += tiles_touched[i];
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+  if ((threadIdx.x & 31) == 0 && acc) atomicAdd(total64, acc);
+}
+
+__global__ void clamp_count_kernel(u32* sort_count, u32* num_instances, const unsigned long long* total64, u64 capacity) {
+  // the sort kernels see 0 instances when the caller's buffers are too small; a count beyond 32 bits saturates
+  const unsigned long long D = *total64;
+  *num_instances = (u32)min(D, 0xffffffffull);
+  *sort_count = (D > capacity || D > 0xffffffffull) ? 0u : (u32)D;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -991,7 +1004,7 @@ void binning_visible_list(const gabsplat_binning& bin, int N, int ntiles, const 
 uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles) { return carve(nullptr, N, capacity, ntiles).bytes; }
 
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
-                            StageTimer& tm, cudaStream_t st) {
+                            StageTimer& tm, int place_bands, cudaStream_t st) {
   const int ntiles = cam.tiles_x * cam.tiles_y;
   const Workspace ws = carve(bin.workspace, N, bin.capacity, ntiles);
   if (N == 0) {
@@ -1044,9 +1057,9 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
     tm.end(st);
     tm.begin(GABSPLAT_STAGE_SORT, st);
     // bands of at most ~1280 tiles: measured best on both the 4346-tile and the 9840-tile configs
-    // (GABSPLAT_PLACE_BANDS overrides the number of bands: a test / tuning hook)
+    // (gabsplat_set_place_bands overrides the number of bands: instrumentation for the tests)
     u64 nbands = std::max<u64>(1, ((u64)ntiles + 1279) / 1280);
-    if (const char* e = std::getenv("GABSPLAT_PLACE_BANDS")) nbands = std::max(1, std::atoi(e));
+    if (place_bands > 0) nbands = (u64)place_bands;
     nbands = std::min<u64>(nbands, (u64)cam.tiles_y);
     const int band_rows = (int)(((u64)cam.tiles_y + nbands - 1) / nbands);
     const int nb = (cam.tiles_y + band_rows - 1) / band_rows;
@@ -1065,8 +1078,11 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   }
   // images with more tiles than the counting pass can histogram in shared memory: one-byte LSD passes on the
   // tile id over the duplicated instances
-  clamp_count_kernel<<<1, 1, 0, st>>>(ws.count_b, bin.num_instances, bin.capacity);
-  launched();
+  unsigned long long* total64 = reinterpret_cast<unsigned long long*>(ws.count_a);
+  cudaMemsetAsync(total64, 0, sizeof(unsigned long long), st);
+  instance_total_kernel<<<148 * 4, 256, 0, st>>>(N, proj.tiles_touched, total64);
+  clamp_count_kernel<<<1, 1, 0, st>>>(ws.count_b, bin.num_instances, total64, bin.capacity);
+  launched(2);
   // stage B passes: one per byte of the tile id.  The last pass reads the alternate buffers and writes
   // bin.keys / bin.ids; earlier passes ping-pong between (bin.keys viewed as u32, bin.ids) and the alternates.
   int tile_bits = 0;

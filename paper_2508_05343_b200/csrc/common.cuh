@@ -143,7 +143,7 @@ inline void launched(int n = 1) { g_kernel_launches.fetch_add((unsigned long lon
 cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const gabsplat_projected& out,
                               cudaStream_t st, cudaStream_t value_stream, cudaEvent_t index_done);
 cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera& cam, const gabsplat_binning& bin,
-                            StageTimer& tm, cudaStream_t st);
+                            StageTimer& tm, int place_bands, cudaStream_t st);
 cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projected& proj,
                                  const gabsplat_binning& bin, const gabsplat_fwd_out& out, const BlendState* save,
                                  cudaStream_t st);

@@ -65,6 +65,7 @@ class Scene:
     freqs: np.ndarray       # [N,K,3] cycles per world unit
     weights: np.ndarray     # [N,K]   in [0,1)
     sh_degree: int = 3
+    variant: int = 0        # primitive variant flags (gabsplat.h GABSPLAT_VARIANT_*): 1 line-integral amplitude, 2 Mip filter
 
     @property
     def N(self) -> int:
@@ -76,7 +77,8 @@ class Scene:
 
     def copy(self) -> "Scene":
         return Scene(*(a.copy() for a in (self.means, self.scales, self.rotations, self.opacities,
-                                           self.sh, self.freqs, self.weights)), sh_degree=self.sh_degree)
+                                           self.sh, self.freqs, self.weights)), sh_degree=self.sh_degree,
+                     variant=self.variant)
 
 
 @dataclass
