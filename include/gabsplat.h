@@ -42,7 +42,7 @@ extern "C" {
 #endif
 
 #define GABSPLAT_OK 0
-#define GABSPLAT_INVALID_ARG 1 /* null pointer, N < 0, K outside [0,8], sh_degree outside [0,3], bad size/focal */
+#define GABSPLAT_INVALID_ARG 1 /* null pointer, N < 0, K outside [0,8], sh_degree outside [0,3], variant outside [0,3], bad size/focal */
 #define GABSPLAT_CAPACITY 2    /* instance buffers or workspace too small */
 #define GABSPLAT_CUDA 3        /* a CUDA call failed; see gabsplat_last_error */
 #define GABSPLAT_UNSUPPORTED 4 /* no sm_100 device */
@@ -71,9 +71,20 @@ typedef struct {
   float bg[3];            /* background colour, composited as C + T_final * bg */
 } gabsplat_camera;
 
+/* Variants of the primitive, bit flags of gabsplat_scene.variant:
+ *  LINE_INTEGRAL  keep the per-component amplitude of the exact line integral along the ray that Eq.12 drops
+ *                 (Eq.25-27; constants as corrected in DESIGN.md reading C4):
+ *                 M = (1 - sum w_k) + sum w_k C2_k cos(phi_k),  C2_k = exp(-2 pi^2 f_z''^2 / S22)
+ *  MIP_FILTER     Mip-Splatting's 2D filter in place of the 0.3 px^2 dilation: dilation 0.1 px^2 and
+ *                 opacity scaled by sqrt(det Sigma2D / det(Sigma2D + 0.1 I)).
+ * Both fold into the per-primitive record the blend kernels gather; conic_opacity[.][3] stays the input opacity. */
+#define GABSPLAT_VARIANT_LINE_INTEGRAL 1
+#define GABSPLAT_VARIANT_MIP_FILTER 2
+
 /* The primitives.  N primitives, K Gabor components each. */
 typedef struct {
   int32_t N, K, sh_degree;
+  int32_t variant;        /* 0, or GABSPLAT_VARIANT_* flags or'ed; must be the same in every call of a pass */
   const float* means;     /* [N][3]                                                  */
   const float* scales;    /* [N][3]   Sigma = R diag(s^2) R^T  (:87)                 */
   const float* rotations; /* [N][4]   unit quaternion (w,x,y,z)                      */

@@ -35,7 +35,7 @@ class _Camera(C.Structure):
 
 
 class _Scene(C.Structure):
-    _fields_ = [("N", C.c_int32), ("K", C.c_int32), ("sh_degree", C.c_int32)] + [
+    _fields_ = [("N", C.c_int32), ("K", C.c_int32), ("sh_degree", C.c_int32), ("variant", C.c_int32)] + [
         (n, C.c_void_p) for n in ("means", "scales", "rotations", "opacities", "sh", "freqs", "weights")]
 
 
@@ -192,6 +192,7 @@ class DeviceScene:
     freqs: torch.Tensor
     weights: torch.Tensor
     sh_degree: int = 3
+    variant: int = 0        # GABSPLAT_VARIANT_* flags
 
     @property
     def N(self) -> int:
@@ -203,7 +204,7 @@ class DeviceScene:
 
     def struct(self) -> _Scene:
         s = _Scene()
-        s.N, s.K, s.sh_degree = self.N, self.K, self.sh_degree
+        s.N, s.K, s.sh_degree, s.variant = self.N, self.K, self.sh_degree, int(self.variant)
         for n in ("means", "scales", "rotations", "opacities", "sh", "freqs", "weights"):
             t = getattr(self, n)
             assert t.dtype == torch.float32 and t.is_contiguous()
@@ -214,7 +215,7 @@ class DeviceScene:
 def upload_scene(scene, device="cuda:0") -> DeviceScene:
     f = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(device)
     return DeviceScene(f(scene.means), f(scene.scales), f(scene.rotations), f(scene.opacities), f(scene.sh),
-                       f(scene.freqs), f(scene.weights), scene.sh_degree)
+                       f(scene.freqs), f(scene.weights), scene.sh_degree, int(getattr(scene, "variant", 0)))
 
 
 class Projected:
@@ -389,6 +390,7 @@ def gabsplat_render_host(ctx: Context, scene, cam, capacity: int, image_host: to
     under the attribute names of gabsplat_scene; `grads_host` maps d_* names to CPU tensors."""
     s = _Scene()
     s.N, s.K, s.sh_degree = int(scene.means.shape[0]), int(scene.freqs.shape[1]), int(scene.sh_degree)
+    s.variant = int(getattr(scene, "variant", 0))
     for n in ("means", "scales", "rotations", "opacities", "sh", "freqs", "weights"):
         t = getattr(scene, n)
         setattr(s, n, t.data_ptr() if t.numel() else None)

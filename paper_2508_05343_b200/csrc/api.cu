@@ -45,7 +45,7 @@ bool camera_ok(const gabsplat_camera* c) {
 }
 
 bool scene_ok(const gabsplat_scene* s) {
-  if (!s || s->N < 0 || s->K < 0 || s->K > kMaxK || s->sh_degree < 0 || s->sh_degree > 3) return false;
+  if (!s || s->N < 0 || s->K < 0 || s->K > kMaxK || s->sh_degree < 0 || s->sh_degree > 3 || s->variant < 0 || s->variant > 3) return false;
   if (s->N == 0) return true;
   if (!s->means || !s->scales || !s->rotations || !s->opacities || !s->sh) return false;
   if (s->K > 0 && (!s->freqs || !s->weights)) return false;

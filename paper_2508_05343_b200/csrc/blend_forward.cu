@@ -188,7 +188,7 @@ cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projec
 namespace {
 // (opacity, sum_k omega_k |f2D_k|, depth, 1) per primitive: the "colours" of the auxiliary renders
 __global__ void __launch_bounds__(256) aux_values_kernel(int N, int K, const uint32_t* __restrict__ tiles_touched,
-                                                         const float4* __restrict__ conic_opacity, const float* __restrict__ depth,
+                                                         const float* __restrict__ packed, const float* __restrict__ depth,
                                                          const float2* __restrict__ freq2d, const float* __restrict__ weights,
                                                          float4* __restrict__ aux) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -200,7 +200,7 @@ __global__ void __launch_bounds__(256) aux_values_kernel(int N, int K, const uin
       const float2 f = freq2d[(size_t)i * K + k];
       fm = fmaf(weights[(size_t)i * K + k], sqrtf(f.x * f.x + f.y * f.y), fm);
     }
-    v = make_float4(conic_opacity[i].w, fm, depth[i], 1.0f);
+    v = make_float4(packed[(size_t)i * packed_floats(K) + 8], fm, depth[i], 1.0f);  // the opacity the blend uses (variants fold into it)
   }
   aux[i] = v;
 }
@@ -210,7 +210,7 @@ cudaError_t launch_blend_aux(int N, int K, const float* weights, const Camera& c
                              const gabsplat_binning& bin, float4* aux, float* image, float* final_T, uint32_t* n_contrib,
                              cudaStream_t st) {
   if (N > 0) {
-    aux_values_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, K, proj.tiles_touched, reinterpret_cast<const float4*>(proj.conic_opacity),
+    aux_values_kernel<<<(N + 255) / 256, 256, 0, st>>>(N, K, proj.tiles_touched, proj.packed,
                                                        proj.depth, reinterpret_cast<const float2*>(proj.freq2d), weights, aux);
     launched();
   }

@@ -13,6 +13,7 @@ namespace gabsplat {
 
 // Named constants of the rasterizer the paper adopts from 3DGS (readings C5, C8).
 constexpr float kDilation = 0.3f;
+constexpr float kMipDilation = 0.1f;  // GABSPLAT_VARIANT_MIP_FILTER
 constexpr float kAlphaMax = 0.99f;
 constexpr float kAlphaMin = 1.0f / 255.0f;
 constexpr float kTMin = 1e-4f;

@@ -31,7 +31,7 @@ struct Index {  // result of the indexing track
   uint32_t tiles;
 };
 
-__device__ Index index_track(const Camera& c, float mx, float my, float mz, const float* __restrict__ sc,
+__device__ Index index_track(const Camera& c, float dilation, float mx, float my, float mz, const float* __restrict__ sc,
                              const float* __restrict__ q) {
   Index o;
   o.visible = false; o.tiles = 0; o.radius = 0; o.x0 = o.y0 = o.x1 = o.y1 = 0; o.depth = o.m2x = o.m2y = 0.f;
@@ -79,7 +79,7 @@ __device__ Index index_track(const Camera& c, float mx, float my, float mz, cons
   const float U00 = ffma(V[0][2], T[0][2], ffma(V[0][1], T[0][1], fmul(V[0][0], T[0][0])));
   const float U01 = ffma(V[0][2], T[1][2], ffma(V[0][1], T[1][1], fmul(V[0][0], T[1][0])));
   const float U11 = ffma(V[1][2], T[1][2], ffma(V[1][1], T[1][1], fmul(V[1][0], T[1][0])));
-  const float A = fadd(U00, kDilation), C = fadd(U11, kDilation);
+  const float A = fadd(U00, dilation), C = fadd(U11, dilation);
   const float det = fsub(fmul(A, C), fmul(U01, U01));
   if (!(det > 0.0f)) return o;
   const float mid = fmul(0.5f, fadd(A, C)), hd = fmul(0.5f, fsub(A, C));
@@ -102,6 +102,9 @@ __device__ Index index_track(const Camera& c, float mx, float my, float mz, cons
 }
 
 // fp64 value track of one visible primitive; everything it stores is rounded once to fp32.
+// VARIANT: compiled with the primitive variants of gabsplat_scene.variant (f4); the plain instantiation carries none of
+// their registers
+template <bool VARIANT>
 __device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camera& c, const gabsplat_projected& out,
                                             const int i) {
   // the fp32 mean of the indexing track (index_kernel wrote it): the packed record carries it with its fp64 residual
@@ -129,13 +132,13 @@ __device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camer
   for (int a = 0; a < 3; ++a) t[a] = Wm[a][0] * mu[0] + Wm[a][1] * mu[1] + Wm[a][2] * mu[2] + tau[a];
   const double tz = t[2];
   // Sigma = R diag(s^2) R^T
-  double Sg[3][3];
+  double Sg[3][3], R[3][3];
+  const double s2[3] = {(double)sc[0] * sc[0], (double)sc[1] * sc[1], (double)sc[2] * sc[2]};
   {
     const double w = q[0], x = q[1], y = q[2], z = q[3];
-    const double R[3][3] = {{1 - 2 * (y * y + z * z), 2 * (x * y - w * z), 2 * (x * z + w * y)},
-                            {2 * (x * y + w * z), 1 - 2 * (x * x + z * z), 2 * (y * z - w * x)},
-                            {2 * (x * z - w * y), 2 * (y * z + w * x), 1 - 2 * (x * x + y * y)}};
-    const double s2[3] = {(double)sc[0] * sc[0], (double)sc[1] * sc[1], (double)sc[2] * sc[2]};
+    R[0][0] = 1 - 2 * (y * y + z * z); R[0][1] = 2 * (x * y - w * z); R[0][2] = 2 * (x * z + w * y);
+    R[1][0] = 2 * (x * y + w * z); R[1][1] = 1 - 2 * (x * x + z * z); R[1][2] = 2 * (y * z - w * x);
+    R[2][0] = 2 * (x * z - w * y); R[2][1] = 2 * (y * z + w * x); R[2][2] = 1 - 2 * (x * x + y * y);
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -158,17 +161,46 @@ __device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camer
   const double U00 = V[0][0] * T[0][0] + V[0][1] * T[0][1] + V[0][2] * T[0][2];
   const double U01 = V[0][0] * T[1][0] + V[0][1] * T[1][1] + V[0][2] * T[1][2];
   const double U11 = V[1][0] * T[1][0] + V[1][1] * T[1][1] + V[1][2] * T[1][2];
-  // conic of the dilated covariance (Eq.3; reading C5)
-  const double A = U00 + 0.3, C = U11 + 0.3;
+  // conic of the dilated covariance (Eq.3; reading C5; the Mip filter variant dilates by 0.1 instead of 0.3)
+  const bool mip = VARIANT && (s.variant & GABSPLAT_VARIANT_MIP_FILTER) != 0;
+  const bool line = VARIANT && (s.variant & GABSPLAT_VARIANT_LINE_INTEGRAL) != 0 && K > 0;
+  const double dil = mip ? (double)kMipDilation : (double)kDilation;
+  const double A = U00 + dil, C = U11 + dil;
   const double idet = 1.0 / (A * C - U01 * U01);
   const double ca = C * idet, cb = -U01 * idet, cc = A * idet;
-  const float opac = s.opacities[i];
-  reinterpret_cast<float4*>(out.conic_opacity)[i] = make_float4((float)ca, (float)cb, (float)cc, opac);
+  const float opac_in = s.opacities[i];
+  reinterpret_cast<float4*>(out.conic_opacity)[i] = make_float4((float)ca, (float)cb, (float)cc, opac_in);
+  // ---- variants (f4): both fold into the record the blend kernels gather, as an effective opacity o' and effective
+  // weights u_k with  o' [(1 - sum u) + sum u cos] = o rho [(1 - sum w) + sum w C2 cos]:
+  //   beta = 1 - sum_k w_k (1 - C2_k),  o' = o rho beta,  u_k = w_k C2_k / beta   (beta <= 0: M <= 0 everywhere, o' = 0)
+  double o_eff = (double)opac_in;
+  if (mip) o_eff *= sqrt(fmax(0.0, (U00 * U11 - U01 * U01) * idet));   // rho = sqrt(det U / det(U + 0.1 I))
+  double att[VARIANT ? kMaxK : 1], beta = 1.0;
+  if (VARIANT && line) {
+    // C2_k = exp(-2 pi^2 (v.f_k)^2 / (v^T Sigma^-1 v)), v = W^T (u_x, u_y, 1) the world-space ray direction of J
+    // (= f_z''^2 / S22 of Eq.25-27 for any completion of J's third row: DESIGN.md readings C2, C4)
+    double v[3], b = 0.0;
+#pragma unroll
+    for (int m = 0; m < 3; ++m) v[m] = Wm[0][m] * ux + Wm[1][m] * uy + Wm[2][m];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      const double rv = R[0][j] * v[0] + R[1][j] * v[1] + R[2][j] * v[2];
+      b += rv * rv / s2[j];
+    }
+    const double pi2 = 9.8696044010893586188;
+    for (int k = 0; k < K; ++k) {
+      const float* f = s.freqs + ((size_t)i * K + k) * 3;
+      const double a = v[0] * (double)f[0] + v[1] * (double)f[1] + v[2] * (double)f[2];
+      att[k] = exp(-2.0 * pi2 * a * a / b);
+      beta -= (double)s.weights[(size_t)i * K + k] * (1.0 - att[k]);
+    }
+    o_eff = beta > 0.0 ? o_eff * beta : 0.0;
+  }
+  const float opac = (float)o_eff;
   // mu2D
   const double m2x = c.fx * t[0] / tz + c.cx, m2y = c.fy * t[1] / tz + c.cy;
 
-  const int R = packed_floats(K);
-  float* rec = out.packed + (size_t)i * R;
+  float* rec = out.packed + (size_t)i * packed_floats(K);
   reinterpret_cast<float4*>(rec)[0] =
       make_float4(m2.x, m2.y, (float)(m2x - (double)m2.x), (float)(m2y - (double)m2.y));
   {
@@ -233,7 +265,8 @@ __device__ __forceinline__ void value_track(const gabsplat_scene& s, const Camer
       out.freq2d[((size_t)i * K + k) * 2 + 1] = (float)fy2;
       rec[12 + 2 * k] = (float)(two_pi * fx2);      // the blend kernels work in radians per pixel
       rec[12 + 2 * k + 1] = (float)(two_pi * fy2);
-      rec[12 + 2 * K + k] = s.weights[(size_t)i * K + k];
+      const float wk = s.weights[(size_t)i * K + k];
+      rec[12 + 2 * K + k] = (VARIANT && line) ? (beta > 0.0 ? (float)((double)wk * att[VARIANT ? k : 0] / beta) : 0.f) : wk;
     }
     for (int k = 3 * K; k < tail_floats(K); ++k) rec[12 + k] = 0.f;
   }
@@ -272,7 +305,7 @@ __global__ void __launch_bounds__(kPreThreads) index_kernel(gabsplat_scene s, Ca
       for (int a = 0; a < 3; ++a) sc[a] = s.scales[3 * i + a];
       const float4 qv = reinterpret_cast<const float4*>(s.rotations)[i];
       q[0] = qv.x; q[1] = qv.y; q[2] = qv.z; q[3] = qv.w;
-      const Index ix = index_track(c, mx, my, mz, sc, q);
+      const Index ix = index_track(c, (s.variant & GABSPLAT_VARIANT_MIP_FILTER) ? kMipDilation : kDilation, mx, my, mz, sc, q);
       tiles = ix.tiles;
       radius = ix.radius;
       if (ix.visible) {
@@ -294,6 +327,7 @@ __global__ void __launch_bounds__(kPreThreads) index_kernel(gabsplat_scene s, Ca
 
 constexpr int kValThreads = 128;
 
+template <bool VARIANT>
 __global__ void __launch_bounds__(kValThreads, 4) value_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
   pdl_wait();
   __shared__ int s_i[kPreChunk];
@@ -306,7 +340,7 @@ __global__ void __launch_bounds__(kValThreads, 4) value_kernel(gabsplat_scene s,
     if (out.tiles_touched[i] != 0) s_i[atomicAdd(&s_n, 1)] = i;
   __syncthreads();
   const int n = s_n;
-  for (int j = threadIdx.x; j < n; j += kValThreads) value_track(s, c, out, s_i[j]);
+  for (int j = threadIdx.x; j < n; j += kValThreads) value_track<VARIANT>(s, c, out, s_i[j]);
 }
 
 }  // namespace
@@ -323,7 +357,8 @@ cudaError_t launch_preprocess(const gabsplat_scene& s, const Camera& cam, const 
     if (e == cudaSuccess) e = cudaStreamWaitEvent(value_stream, index_done, 0);
     if (e != cudaSuccess) return e;
   }
-  launch_pdl(value_kernel, chunks, kValThreads, 0, value_stream, s, cam, out);
+  if (s.variant) launch_pdl(value_kernel<true>, chunks, kValThreads, 0, value_stream, s, cam, out);
+  else launch_pdl(value_kernel<false>, chunks, kValThreads, 0, value_stream, s, cam, out);
   launched(2);
   return cudaGetLastError();
 }

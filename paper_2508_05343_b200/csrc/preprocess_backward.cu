@@ -11,6 +11,7 @@ namespace gabsplat {
 namespace {
 
 // chain rule of one visible primitive (fp64); writes its row of every gradient array
+template <bool VARIANT>
 __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Camera& c, const uint8_t* __restrict__ rgb_clamped,
                                              float* grad2d, const gabsplat_grads& g, const int i) {
   const int K = s.K;
@@ -59,9 +60,68 @@ __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Came
   const double U00 = V[0][0] * T[0][0] + V[0][1] * T[0][1] + V[0][2] * T[0][2];
   const double U01 = V[0][0] * T[1][0] + V[0][1] * T[1][1] + V[0][2] * T[1][2];
   const double U11 = V[1][0] * T[1][0] + V[1][1] * T[1][1] + V[1][2] * T[1][2];
-  const double A = U00 + 0.3, C = U11 + 0.3;
+  const bool mip = VARIANT && (s.variant & GABSPLAT_VARIANT_MIP_FILTER) != 0;
+  const bool line = VARIANT && (s.variant & GABSPLAT_VARIANT_LINE_INTEGRAL) != 0 && K > 0;
+  const double dil = mip ? (double)kMipDilation : (double)kDilation;
+  const double A = U00 + dil, C = U11 + dil;
   const double idet = 1.0 / (A * C - U01 * U01);
   const double ca = C * idet, cb = -U01 * idet, cc = A * idet;
+  // ---- variants (f4; preprocess.cu value_track): the blend saw o' = o rho beta and u_k = w_k C2_k / beta
+  const double opac = (double)s.opacities[i];
+  const double rho = mip ? sqrt(fmax(0.0, (U00 * U11 - U01 * U01) * idet)) : 1.0;
+  constexpr int KV = VARIANT ? kMaxK : 1;
+  double att[KV], av[KV], beta = 1.0, v[3] = {0, 0, 0}, yv[3] = {0, 0, 0}, bq = 1.0;
+#pragma unroll
+  for (int k = 0; k < KV; ++k) { att[k] = 1.0; av[k] = 0.0; }
+  if (VARIANT && line) {
+#pragma unroll
+    for (int m = 0; m < 3; ++m) v[m] = Wm[0][m] * ux + Wm[1][m] * uy + Wm[2][m];
+    // y = Sigma^-1 v = R diag(1/s^2) R^T v,  b = v^T y
+    double rv[3];
+    bq = 0.0;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      rv[j] = (R[0][j] * v[0] + R[1][j] * v[1] + R[2][j] * v[2]) / (sc[j] * sc[j]);
+      bq += rv[j] * (R[0][j] * v[0] + R[1][j] * v[1] + R[2][j] * v[2]);
+    }
+#pragma unroll
+    for (int m = 0; m < 3; ++m) yv[m] = R[m][0] * rv[0] + R[m][1] * rv[1] + R[m][2] * rv[2];
+    const double pi2 = 9.8696044010893586188;
+    for (int k = 0; k < K; ++k) {
+      const float* fp = s.freqs + ((size_t)i * K + k) * 3;
+      av[k] = v[0] * (double)fp[0] + v[1] * (double)fp[1] + v[2] * (double)fp[2];
+      att[k] = exp(-2.0 * pi2 * av[k] * av[k] / bq);
+      beta -= (double)s.weights[(size_t)i * K + k] * (1.0 - att[k]);
+    }
+  }
+  const bool live = !line || beta > 0.0;   // beta <= 0: the primitive was never blended, its 2D record is zero
+  const double g_oeff = live ? (double)g2[5] : 0.0;
+  // d o' -> (o, rho, beta);  d u_k -> (w_k, C2_k, beta)
+  double g_beta = g_oeff * opac * rho, g_att[KV];
+#pragma unroll
+  for (int k = 0; k < KV; ++k) g_att[k] = 0.0;
+  double g_w[KV];
+  for (int k = 0; VARIANT && k < K; ++k) {
+    const double gu = live ? (double)g2[9 + 2 * K + k] : 0.0;
+    if (line) {
+      const double w = (double)s.weights[(size_t)i * K + k];
+      const double ib = live ? 1.0 / beta : 0.0;
+      g_beta -= gu * (w * att[k] * ib) * ib;
+      g_w[k] = gu * att[k] * ib;
+      g_att[k] = gu * w * ib;
+    } else {
+      g_w[k] = gu;
+    }
+  }
+  if (VARIANT && line) {
+    for (int k = 0; k < K; ++k) {
+      const double w = (double)s.weights[(size_t)i * K + k];
+      g_w[k] -= g_beta * (1.0 - att[k]);
+      g_att[k] += g_beta * w;
+    }
+  }
+  const double g_opacity = g_oeff * rho * (line ? beta : 1.0);
+  const double g_rho = g_oeff * opac * (line ? beta : 1.0);
 
   // conic -> U_d (= U + const).  The blend accumulated S = sum gq w w^T with w = L^T d the whitened pixel offset
   // (L = sqrt(log2(e) / 2) * Cholesky factor of the conic, as packed for the blend) and gq = dL/d(ln G).  With
@@ -82,11 +142,41 @@ __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Came
     GU[1][1] = k * (m10 * L21 + m11 * L22);
   }
   double gS[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, gT[2][3] = {{0, 0, 0}, {0, 0, 0}};
+  double gt[3] = {0, 0, 0};
+  double gf_extra[KV][3];
+#pragma unroll
+  for (int k = 0; k < KV; ++k) gf_extra[k][0] = gf_extra[k][1] = gf_extra[k][2] = 0.0;
+  if (VARIANT && line && live) {
+    // C2_k = exp(-2 pi^2 a_k^2 / b), a_k = v . f_k, b = v^T Sigma^-1 v, v = W^T (u_x, u_y, 1)
+    const double pi2 = 9.8696044010893586188;
+    double gv[3] = {0, 0, 0}, gb = 0.0;
+    for (int k = 0; k < K; ++k) {
+      const float* fp = s.freqs + ((size_t)i * K + k) * 3;
+      const double gl = g_att[k] * att[k];  // dL/d(ln C2_k)
+      const double ga = gl * (-4.0 * pi2 * av[k] / bq);
+      gb += gl * (2.0 * pi2 * av[k] * av[k] / (bq * bq));
+#pragma unroll
+      for (int m = 0; m < 3; ++m) { gf_extra[k][m] = ga * v[m]; gv[m] += ga * (double)fp[m]; }
+    }
+#pragma unroll
+    for (int m = 0; m < 3; ++m) gv[m] += 2.0 * gb * yv[m];
+#pragma unroll
+    for (int m = 0; m < 3; ++m)
+#pragma unroll
+      for (int n = 0; n < 3; ++n) gS[m][n] -= gb * yv[m] * yv[n];  // d(Sigma^-1) = -Sigma^-1 dSigma Sigma^-1
+    const double gcx = Wm[0][0] * gv[0] + Wm[0][1] * gv[1] + Wm[0][2] * gv[2];
+    const double gcy = Wm[1][0] * gv[0] + Wm[1][1] * gv[1] + Wm[1][2] * gv[2];
+    if (!clampx) { gt[0] += gcx / tz; gt[2] -= gcx * t[0] / (tz * tz); }
+    if (!clampy) { gt[1] += gcy / tz; gt[2] -= gcy * t[1] / (tz * tz); }
+  }
   // f2D_k = U^-1 T Sigma f_k  (U undilated)
   {
     const double iu = 1.0 / (U00 * U11 - U01 * U01);
     const double Ui00 = U11 * iu, Ui01 = -U01 * iu, Ui11 = U00 * iu;
-    const int wo = 9 + 2 * K;
+    if (mip) {  // rho = sqrt(det U / det U_d):  d rho = rho / 2 tr((U^-1 - U_d^-1) dU)
+      const double h = 0.5 * g_rho * rho;
+      GU[0][0] += h * (Ui00 - ca); GU[0][1] += h * (Ui01 - cb); GU[1][0] += h * (Ui01 - cb); GU[1][1] += h * (Ui11 - cc);
+    }
     const double two_pi = 6.283185307179586476925286766559;  // grad2d holds d/d(2 pi f2D)
     for (int k = 0; k < K; ++k) {
       const float* fp = s.freqs + ((size_t)i * K + k) * 3;
@@ -114,8 +204,8 @@ __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Came
       for (int m = 0; m < 3; ++m) { gT[0][m] += h0 * Sf[m]; gT[1][m] += h1 * Sf[m]; }
 #pragma unroll
       for (int m = 0; m < 3; ++m)
-        g.d_freqs[((size_t)i * K + k) * 3 + m] = (float)(Sg[m][0] * Th[0] + Sg[m][1] * Th[1] + Sg[m][2] * Th[2]);
-      g.d_weights[(size_t)i * K + k] = g2[wo + k];
+        g.d_freqs[((size_t)i * K + k) * 3 + m] = (float)(Sg[m][0] * Th[0] + Sg[m][1] * Th[1] + Sg[m][2] * Th[2] + (VARIANT ? gf_extra[VARIANT ? k : 0][m] : 0.0));
+      g.d_weights[(size_t)i * K + k] = VARIANT ? (float)g_w[VARIANT ? k : 0] : g2[9 + 2 * K + k];
     }
   }
   // U = T Sigma T^T
@@ -135,7 +225,6 @@ __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Came
       for (int m = 0; m < 3; ++m) gT[r][m] += 2.0 * (GUT[r][0] * Sg[0][m] + GUT[r][1] * Sg[1][m] + GUT[r][2] * Sg[2][m]);
   }
   // T = J W  ->  g_J = g_T W^T;  J(t) and mu2D(t)
-  double gt[3] = {0, 0, 0};
   {
     double gJ[2][3];
 #pragma unroll
@@ -230,7 +319,7 @@ __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Came
   }
 #pragma unroll
   for (int m = 0; m < 3; ++m) g.d_means[3 * i + m] = (float)gmu[m];
-  g.d_opacities[i] = g2[5];
+  g.d_opacities[i] = (float)g_opacity;
   if (g.d_mean2d) { g.d_mean2d[2 * i] = g2[0]; g.d_mean2d[2 * i + 1] = g2[1]; }
   if (g.d_mean2d_abs) { g.d_mean2d_abs[2 * i] = g2[9 + 3 * K]; g.d_mean2d_abs[2 * i + 1] = g2[10 + 3 * K]; }
   // clear the primitive's 2D gradient record: the workspace is all zero again when the call returns (only visible
@@ -245,6 +334,7 @@ constexpr int kBwdThreads = 128;
 // there, compact, and keeps every lane of every live warp busy -- 10-20 % of the primitives are visible).  The
 // gradient arrays were zeroed by grad_zero_kernel (side stream, concurrently with the blend backward); rows of
 // culled primitives stay zero.
+template <bool VARIANT>
 __global__ void __launch_bounds__(kBwdThreads, 3) preprocess_backward_kernel(gabsplat_scene s, Camera c, const uint32_t* __restrict__ order,
                                                                          const uint32_t* __restrict__ n_vis,
                                                                          const uint8_t* __restrict__ rgb_clamped,
@@ -252,7 +342,7 @@ __global__ void __launch_bounds__(kBwdThreads, 3) preprocess_backward_kernel(gab
   pdl_wait();
   const uint32_t r = blockIdx.x * kBwdThreads + threadIdx.x;
   if (r >= *n_vis) return;
-  backward_one(s, c, rgb_clamped, grad2d, g, (int)order[r]);
+  backward_one<VARIANT>(s, c, rgb_clamped, grad2d, g, (int)order[r]);
 }
 
 // Zeroes every gradient array (coalesced 16-byte stores, grid-stride): 300 B per primitive of pure HBM writes,
@@ -291,8 +381,12 @@ cudaError_t launch_preprocess_backward(const gabsplat_scene& s, const Camera& ca
   if (s.N == 0) return cudaGetLastError();
   const uint32_t *order, *n_vis;
   binning_visible_list(bin, s.N, cam.tiles_x * cam.tiles_y, &order, &n_vis);
-  launch_pdl(preprocess_backward_kernel, (s.N + kBwdThreads - 1) / kBwdThreads, kBwdThreads, 0, st, s, cam, order, n_vis,
-             (const uint8_t*)proj.rgb_clamped, grad2d, g);
+  if (s.variant)
+    launch_pdl(preprocess_backward_kernel<true>, (s.N + kBwdThreads - 1) / kBwdThreads, kBwdThreads, 0, st, s, cam, order, n_vis,
+               (const uint8_t*)proj.rgb_clamped, grad2d, g);
+  else
+    launch_pdl(preprocess_backward_kernel<false>, (s.N + kBwdThreads - 1) / kBwdThreads, kBwdThreads, 0, st, s, cam, order, n_vis,
+               (const uint8_t*)proj.rgb_clamped, grad2d, g);
   launched();
   return cudaGetLastError();
 }
