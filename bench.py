@@ -35,8 +35,9 @@ UNIT = "Mpix/s"
 # ALU roofline constants: 148 SMs x 4 sub-partitions x 32 lanes x 1.965 GHz FP32-pipe
 # lane-instructions per second; MUFU: 16 lanes per SM per clock.
 SM_COUNT, SM_HZ = 148, 1.965e9
-FP32_PEAK = SM_COUNT * 128 * SM_HZ      # lane-instructions / s
-MUFU_PEAK = SM_COUNT * 16 * SM_HZ       # lane-ops / s
+FP32_NOMINAL = SM_COUNT * 128 * SM_HZ      # lane-instructions / s
+MUFU_NOMINAL = SM_COUNT * 16 * SM_HZ       # lane-ops / s
+REFERENCE_BUDGET_S = 900.0                 # --impl reference renders full frames while warmup + steps fit this
 
 
 def parse_args():
@@ -132,23 +133,32 @@ def oracle_view(orc, scene, cam, dL, backward: bool) -> float:
 
 
 def run_reference(args, name, scene, cams, rank) -> dict:
-    """--impl reference: the oracle as it stands, on the host cores; each step a band of rows of one view."""
+    """--impl reference: the oracle as it stands, on the host cores.  A step is one FULL frame of one view (the same
+    unit of work as a step of our arm) whenever warmup + steps full frames fit REFERENCE_BUDGET_S; only for a
+    larger request is a step a band of rows of the view (the projection and the sort of all primitives are then
+    still paid per step, which deflates the per-pixel rate: `same_work_per_step` says which it was)."""
     from oracle import gabsplat_oracle as orc
     from paper_2508_05343_b200 import scenes
     backward = not args.forward_only
     cores = orc.max_threads()
     H, W = cams[0].height, cams[0].width
-    budget = 150.0 / max(1, args.steps + args.warmup)
+    n_total = max(1, args.steps + args.warmup)
     cal_rows = min(H, 32)
     y_mid = max(0, (H // 2) // 16 * 16 - 16)
     dL0 = scenes.make_image_grad(name, 0, cams[0])
     t_cal = oracle_view(orc, scene, crop_camera(cams[0], y_mid, cal_rows), dL0[:, y_mid:y_mid + cal_rows], backward)
-    rows = int(min(H, max(16, cal_rows * int(budget / max(t_cal, 1e-6)))))
-    rows = H if rows >= H else rows // 16 * 16
+    t_full = oracle_view(orc, scene, cams[0], dL0, backward)      # untimed calibration frame
+    if t_full * n_total <= REFERENCE_BUDGET_S:
+        rows = H
+    else:
+        per_row = max((t_full - t_cal) / max(H - cal_rows, 1), 1e-9)
+        fixed = max(t_cal - per_row * cal_rows, 0.0)
+        rows = int(max(16, min(H, (REFERENCE_BUDGET_S / n_total - fixed) / per_row)))
+        rows = H if rows >= H else max(16, rows // 16 * 16)
     times = []
+    y0 = 0 if rows >= H else (y_mid if y_mid + rows <= H else 0)
     for i in range(args.warmup + args.steps):
         v = i % len(cams)
-        y0 = 0 if rows >= H else (y_mid if y_mid + rows <= H else 0)
         cam = crop_camera(cams[v], y0, rows) if rows < H else cams[v]
         dL = scenes.make_image_grad(name, v, cams[v])[:, y0:y0 + rows]
         dt = oracle_view(orc, scene, cam, np.ascontiguousarray(dL), backward)
@@ -156,13 +166,18 @@ def run_reference(args, name, scene, cams, rank) -> dict:
             times.append(dt)
     ms = 1e3 * float(np.mean(times))
     value = rows * W / 1e6 / (ms / 1e3)
-    sample = "rows [%d,%d) of each 1297x840-style view (%d of %d rows) rendered as a cropped camera, %s" % (
-        y0, y0 + rows, rows, H, "forward+backward" if backward else "forward")
+    if rows >= H:
+        sample = "full frames: every step renders all %d rows of one of the 8 views, %s" % (
+            H, "forward+backward" if backward else "forward")
+    else:
+        sample = "rows [%d,%d) of each view (%d of %d rows) rendered as a cropped camera, %s; all primitives are " \
+                 "projected and sorted every step" % (y0, y0 + rows, rows, H, "forward+backward" if backward else "forward")
     return {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic (seeded; DESIGN.md 'Input recipe')",
         "config": workload_config(args, name, scene, cams[0]),
+        "same_work_per_step": rows >= H, "rows_per_step": rows,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,

@@ -24,7 +24,7 @@ def test_tiny_variants(variant, K):
     o = orc.project(scene, cam)
     if variant & 1:
         att = o["att"][o["visible"].astype(bool)]
-        assert att.min() < 0.5 and att.max() > 0.9
+        assert att.min() < 0.75 and att.max() > 0.9   # the scene exercises the attenuation (a precondition, not a tolerance)
     check_projection(g, o, K)
     check_binning(g, orc.bin_sort(scene, cam))
     check_forward(g, orc.render_forward(scene, cam))
