@@ -52,6 +52,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     ap.add_argument("--forward-only", action="store_true", help="a step is S1-S3 only (config 2 is forward only)")
+    ap.add_argument("--dry-run", action="store_true",
+                    help="host logic of the N-rank run only (gloo, no CUDA, a stand-in step): what the CPU tests drive")
     return ap.parse_args()
 
 
@@ -217,7 +219,7 @@ def workload_config(args, name, scene, cam) -> dict:
 # ----------------------------------------------------------------------------------------------------
 # rooflines
 # ----------------------------------------------------------------------------------------------------
-def stage_work(K, N, stats, tiles, passes) -> dict:
+def stage_work(K, N, stats, tiles, passes, with_keys=False) -> dict:
     """Algorithmic work of every stage for one view."""
     n_vis, D = stats["n_visible"], stats["D"]
     E, P, B, Pb, Eb = stats["examined"], stats["envelope"], stats["blended"], stats["envelope_le_last"], stats["walked"]
@@ -233,11 +235,12 @@ def stage_work(K, N, stats, tiles, passes) -> dict:
         # counting pass on the tile id: C = 592 chunks of the depth-ordered primitives;
         # "duplicate" = chunk bounds + per-(tile, chunk) counts (rect + order of every visible primitive read,
         # the table written); "ranges" = prefix of the table over the chunks (read + written) and of the totals
-        # over the tiles; "sort" = placement: every instance written ONCE (8 B key + 4 B id), table read
+        # over the tiles; "sort" = placement: every instance written ONCE (4 B id; + 8 B key only when the keys are
+        # materialised, which the timed step does not do), table read
         C = 592
         w["duplicate"] = ("hbm", 20 * n_vis + 4 * tiles * C)
         w["ranges"] = ("hbm", 8 * tiles * C + 24 * tiles)
-        w["sort"] = ("hbm", 12 * D + 28 * n_vis + 4 * tiles * C + 8 * tiles)
+        w["sort"] = ("hbm", (12 if with_keys else 4) * D + 28 * n_vis + 4 * tiles * C + 8 * tiles)
     else:
         w["duplicate"] = ("hbm", 8 * N + 20 * n_vis + 8 * D)
         w["sort"] = ("hbm", D * (4 + (passes - 1) * 16 + 24))
@@ -256,17 +259,29 @@ def stage_work(K, N, stats, tiles, passes) -> dict:
     return w
 
 
-def roofline_entry(work, ms, hbm_peak, peak_kind) -> dict:
+def roofline_entry(work, ms, hbm_peak, peak_kind, alu=None) -> dict:
+    """work = ("hbm", bytes) or ("alu", FP32-pipe lane-instructions, MUFU lane-ops); alu = gabsplat_measure_peaks()."""
     t = ms / 1e3
     if work[0] == "hbm":
         ach = work[1] / t / 1e9
         return {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
                 "traffic": None, "peak_kind": peak_kind, "algorithmic_bytes": int(work[1])}
     fp32, mufu = work[1], work[2]
-    t_peak = max(fp32 / FP32_PEAK, mufu / MUFU_PEAK)
+    if alu is not None:
+        # measured on this device by dependency-free micro-kernels (csrc/peaks.cu): FFMA issue rate, and the slower
+        # of MUFU.EX2 / MUFU.COS (the blend's transcendental mix is 1 ex2 : K cos)
+        fp32_peak, mufu_peak = alu["ffma"], min(alu["mufu_ex2"], alu["mufu_cos"])
+        kind = "measured (gabsplat_measure_peaks: dependency-free FFMA / MUFU micro-kernels on this device)"
+    else:
+        fp32_peak, mufu_peak = FP32_NOMINAL, MUFU_NOMINAL
+        kind = "derived: 148 SM x 128 lanes x 1.965 GHz; MUFU 16 lanes/SM"
+    t_peak = max(fp32 / fp32_peak, mufu / mufu_peak)
     ach = fp32 / t / 1e12
-    return {"bound": "alu", "achieved": ach, "peak": FP32_PEAK / 1e12, "unit": "Tinstr/s (FP32-pipe lane-instructions)",
-            "frac": t_peak / t, "traffic": None, "peak_kind": "derived: 148 SM x 128 lanes x 1.965 GHz; MUFU 16 lanes/SM",
+    return {"bound": "alu", "achieved": ach, "peak": fp32_peak / 1e12, "unit": "Tinstr/s (FP32-pipe lane-instructions)",
+            "frac": t_peak / t, "traffic": None, "peak_kind": kind,
+            "peak_mufu": mufu_peak / 1e12, "peak_nominal": FP32_NOMINAL / 1e12, "peak_mufu_nominal": MUFU_NOMINAL / 1e12,
+            "frac_of_nominal": max(fp32 / FP32_NOMINAL, mufu / MUFU_NOMINAL) / t,
+            "limiter": "fp32 issue" if fp32 / fp32_peak >= mufu / mufu_peak else "mufu",
             "algorithmic_fp32_instr": int(fp32), "algorithmic_mufu_ops": int(mufu),
             "time_at_peak_ms": 1e3 * t_peak}
 
@@ -287,6 +302,7 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
     ctx = gb.Context(local_rank)
+    alu_peaks = gb.gabsplat_measure_peaks(ctx)     # FFMA issue and MUFU rates of THIS device, ~20 ms
     backward = not args.forward_only
     N, K = scene.N, scene.K
     V = len(cams)
@@ -381,11 +397,12 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     views_timed = [my_view(i) for i in range(args.steps)]
     mean_stats = {k: float(np.mean([stats[v][k] for v in views_timed])) for k in stats[0]}
     hbm_peak, peak_kind = peaks()
-    work = stage_work(K, N, mean_stats, tiles, passes)
+    work = stage_work(K, N, mean_stats, tiles, passes, with_keys=False)
     per_stage = {}
     for s, lst in stage_ms.items():
         m = float(np.sum(lst)) / args.steps          # per step (a stage may launch in several pieces)
-        per_stage[s] = {"ms": m, "share": m / (staged_ms / args.steps), **roofline_entry(work[s], m, hbm_peak, peak_kind)}
+        per_stage[s] = {"ms": m, "share": m / (staged_ms / args.steps),
+                        **roofline_entry(work[s], m, hbm_peak, peak_kind, alu_peaks)}
     dominant = max(per_stage, key=lambda s: per_stage[s]["ms"])
     roofline = {"kernel": dominant, **{k: per_stage[dominant][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
                 "peak_kind": per_stage[dominant]["peak_kind"]}
@@ -462,6 +479,11 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
         torch.cuda.synchronize()
         loss_ms = e0.elapsed_time(e1) / 20
         del img, tgt, ws
+        # csrc/loss.cu: pass 1 reads image + target (2 x 3HW floats) and writes 9 maps; pass 2 reads the 9 maps,
+        # image and target and writes dL/dimage (3HW floats): 26 floats per pixel of HBM traffic as designed
+        per_stage["loss (f2, beside the step)"] = {
+            "ms": loss_ms, "share": None,
+            **roofline_entry(("hbm", 26 * 4 * H * W), loss_ms, hbm_peak, peak_kind)}
 
     if dist is not None:
         dist.barrier()
@@ -496,12 +518,53 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     return out
 
 
+def spawn_ranks(n: int) -> int:
+    """`python bench.py --gpus N` without a launcher: re-run this command line under torchrun, one rank per GPU
+    (replicas only).  The ranks' output (rank 0 prints the JSON line) passes through."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--standalone", "--nnodes=1", "--nproc-per-node", str(n),
+           "--local-addr", "127.0.0.1", os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")          # the communicator log shows the rank count
+    env.setdefault("OMP_NUM_THREADS", "1")
+    return subprocess.call(cmd, env=env)
+
+
+def run_dry(args, rank, world) -> dict | None:
+    """The N-rank host logic with a stand-in step and no device: rendezvous (gloo), the view of every step, max over
+    ranks, whole-job value, one line from rank 0.  Used by tests/test_multi_rank.py; never a measurement."""
+    import torch.distributed as dist
+    if world > 1:
+        dist.init_process_group("gloo")
+    views = [view_of_step(i, rank, 8) for i in range(args.steps)]
+    ms = max_over_ranks(1.0 + 0.5 * rank, dist if world > 1 else None)     # the slowest rank decides
+    gathered = [None] * world
+    if world > 1:
+        dist.all_gather_object(gathered, views)
+        dist.barrier()
+        dist.destroy_process_group()
+    else:
+        gathered = [views]
+    if rank != 0:
+        return None
+    return {"metric": METRIC, "value": job_value(1297 * 840, world, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dry_run": True, "views_per_rank": gathered,
+            "multi_gpu": "replicas only: each rank renders its own views of a replicated scene, no data-path collective"}
+
+
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        return spawn_ranks(args.gpus)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference" and rank != 0:
+        return 0
+    if args.dry_run:
+        out = run_dry(args, rank, world)
+        if out is not None:
+            print(json.dumps(out), flush=True)
         return 0
     from paper_2508_05343_b200 import scenes
     name = args.config

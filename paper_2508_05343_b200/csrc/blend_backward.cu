@@ -3,73 +3,54 @@
 // Same CTA / pixel mapping as the forward kernel (blend_common.cuh): 64 threads per tile, 4 pixels per thread.
 // Each warp replays the list of blended primitives the forward saved for its half tile, back to front, and
 // recovers the transmittance in front of each primitive by division.  Per primitive a thread first sums the
-// gradient contributions of its 4 pixels in registers; the 9+3K (+2) sums are then reduced over the warp with a
-// butterfly that halves the number of live values at every exchange (one shuffle per value pair instead of
-// five per value) and leaves value i on lane idx(i), so the warp issues ONE vector of atomic adds per primitive.
+// gradient contributions of its 4 pixels in registers; the 9+3K (+2) sums are then reduced over the warp through
+// shared memory, a few entries at a time (one row per value, one lane per row), and every row total is ONE atomic add.
 #include "blend_common.cuh"
 
 namespace gabsplat {
 namespace {
 
-// ---- multi-value warp reduction ---------------------------------------------------------------------
-// v[0..n) on every lane.  Exchange distance D: lanes with bit D clear keep values [0,H), the others keep
-// [H,n) (H = ceil(n/2)); each sends the half it does not keep.  After distances 16,8,4,2,1 v[0] holds the warp
-// total of value reduce_index(lane) (or padding).
-template <int n, int D>
-struct Butterfly {
-  template <int N>
-  static __device__ __forceinline__ void run(float (&v)[N], int lane) {
-    constexpr int H = (n + 1) / 2;
-    const bool upper = (lane & D) != 0;
-#pragma unroll
-    for (int i = 0; i < H; ++i) {
-      const float lo = v[i];
-      const float hi = (i + H < n) ? v[i + H] : 0.f;
-      const float send = upper ? lo : hi;
-      const float keep = upper ? hi : lo;
-      v[i] = keep + __shfl_xor_sync(kFull, send, D);
-    }
-    Butterfly<H, D / 2>::run(v, lane);
-  }
-};
-template <int n>
-struct Butterfly<n, 0> {
-  template <int N>
-  static __device__ __forceinline__ void run(float (&)[N], int) {}
-};
+// ---- reduction of the per-lane sums over the warp ----------------------------------------------------
+// A lane ends every saved entry with NV partial sums (its 4 pixels).  They are reduced over the 32 lanes through
+// shared memory instead of shuffles: the lane stores value i of the group's entry e to row e * NV + i, column
+// `lane` (one conflict-free store per value), and once kGroup entries are pending every lane adds up one row -- 8
+// vector loads and 31 additions per round of 32 rows -- and issues its atomic.  Per entry that is NV stores plus
+// ~39 * NV / 32 instructions where a shuffle butterfly took ~4.4 per value (23 SHFL + 23 FADD + 46 FSEL at NV = 21),
+// and the additions of different rows are independent (no 5-deep shuffle chain).
+constexpr int kRowStride = 36;   // floats: 16-byte aligned rows whose vector loads spread over the banks
+constexpr int kMaxRows = 64;     // rows a group may fill (two rounds)
 
-// Number of values left on every lane after the five exchanges (1 for N <= 32).
-__host__ __device__ constexpr int reduce_left(int N) {
-  for (int L = 0; L < 5; ++L) N = (N + 1) / 2;
-  return N;
-}
-
-// Which of the N values lane `lane` holds in v[i] after Butterfly<N,16>; -1 if it holds padding.
-template <int N>
-__device__ __forceinline__ int reduce_index(int lane, int i) {
-  int cnt[5];
-  int n = N;
-#pragma unroll
-  for (int L = 0; L < 5; ++L) { cnt[L] = n; n = (n + 1) / 2; }
-  int rel = i;
-  bool valid = true;
-#pragma unroll
-  for (int L = 4; L >= 0; --L) {
-    if (lane & (16 >> L)) rel += (cnt[L] + 1) / 2;
-    valid = valid && rel < cnt[L];
+__host__ __device__ constexpr int group_entries(int NV) {
+  int best = 1, best_fill = 0;
+  for (int g = 1; g <= 8; ++g) {
+    const int rows = g * NV;
+    if (rows > kMaxRows) break;
+    const int rounds = (rows + 31) / 32;
+    const int fill = rows * 1000 / (32 * rounds);
+    if (fill > best_fill) { best = g; best_fill = fill; }
   }
-  return valid ? rel : -1;
+  return best;
 }
+__host__ __device__ constexpr int group_rows(int NV) { return NV > kMaxRows ? NV : group_entries(NV) * NV; }
 
 constexpr int kReplay = 32;  // saved entries staged per warp and batch
+
+__device__ __forceinline__ float rcp_fast(float x) {  // x in [0.01, 1]: no denormal, no special case
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
 
 // ABS: also accumulate sum |dL/dmu2D| per pixel (AbsGS densification statistic).
 //
 // Every warp replays, back to front, the list the forward saved for its half tile (BlendState): the
 // primitives that were blended at one of the warp's 128 pixels, with the ballots of the blending lanes.  No
-// tile list is walked, no skip / stop decision is re-taken, and the two warps of a CTA never synchronise.
+// tile list is walked, no skip / stop decision is re-taken, and the two warps of a tile never synchronise.
 // A lane recomputes G, cos, sin and alpha of its blended pixels with the forward's own functions (bit-identical
 // alpha), recovers the transmittance in front of the primitive by division, and accumulates the gradient terms.
+// Per pixel the colour behind the primitive enters only through <dL/dC, B>, so that scalar is what is carried
+// (A <- A + alpha (<dL/dC, c> - A)), and every factor that is constant over the entry (omega_k, 2 pi f2D_k, L, dx)
+// is applied once per entry to sums taken over the lane's pixels.
 template <int K, bool ABS>
 __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, const uint2* __restrict__ ranges,
                                                                        BlendState saved, const float4* __restrict__ packed,
@@ -81,10 +62,15 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
   constexpr int TL = K > 0 ? tail_floats(K) : 1;
   constexpr int NV = 9 + 3 * K + (ABS ? 2 : 0);
   constexpr int GF = grad2d_floats(K);
+  constexpr int KK = K > 0 ? K : 1;
+  constexpr int kGroup = group_entries(NV);
+  constexpr int kRows = group_rows(NV);
+  constexpr int kRounds = (kRows + 31) / 32;
   // one warp per CTA: CTA b replays half tile order[b] (half tiles by descending saved-list length)
   __shared__ float4 s_rec1[kReplay * R4];
   __shared__ uint4 s_mask1[kReplay];
   __shared__ uint32_t s_id1[kReplay];
+  __shared__ __align__(16) float s_red[kRounds * 32 * kRowStride];
   const uint32_t half = __ldg(saved.order + blockIdx.x);
   const TileGeom g = tile_geom_at(cam, (int)(half >> 1), (int)(half & 1u), (int)threadIdx.x);
   const uint2 range = ranges[g.tile];
@@ -93,7 +79,8 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
   const size_t base = 2 * (size_t)range.x + (size_t)g.warp * (range.y - range.x);
   float4* __restrict__ rec = s_rec1;
 
-  float T[kSlots], gC[kSlots][3], B[kSlots][3];
+  // per pixel: T in front of the entries still to come (starts at the final T), dL/dC, and A = <dL/dC, colour behind>
+  float T[kSlots], gC[kSlots][3], A[kSlots];
 #pragma unroll
   for (int s = 0; s < kSlots; ++s) {
     T[s] = 0.f;
@@ -103,13 +90,38 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
       T[s] = final_T[pix];
       gC[s][0] = dL_dimage[pix]; gC[s][1] = dL_dimage[HW + pix]; gC[s][2] = dL_dimage[2 * HW + pix];
     }
-    B[s][0] = cam.bg[0]; B[s][1] = cam.bg[1]; B[s][2] = cam.bg[2];  // colour behind the current primitive
+    A[s] = gC[s][0] * cam.bg[0] + gC[s][1] * cam.bg[1] + gC[s][2] * cam.bg[2];
   }
 
-  constexpr int NL = reduce_left(NV);
-  int my_idx[NL];
+  // rows this lane sums in a flush: row r = round * 32 + lane holds value r % NV of the group's entry r / NV
+  int row_e[kRounds], row_v[kRounds];
 #pragma unroll
-  for (int i = 0; i < NL; ++i) my_idx[i] = reduce_index<NV>(g.lane, i);
+  for (int r = 0; r < kRounds; ++r) {
+    const int row = r * 32 + g.lane;
+    row_e[r] = row / NV;
+    row_v[r] = row - row_e[r] * NV;
+  }
+  const uint32_t lane_bit = 1u << g.lane;
+
+  // adds up the rows of the `pend` pending entries (the group started at staged entry j0) into the gradient records
+  auto flush = [&](int pend, int j0) {
+    __syncwarp();
+#pragma unroll
+    for (int r = 0; r < kRounds; ++r) {
+      if (row_e[r] < pend) {
+        const float4* rowp = reinterpret_cast<const float4*>(s_red + (r * 32 + g.lane) * kRowStride);
+        float4 x[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = rowp[i];
+        float p[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) p[i] = (x[i].x + x[i].y) + (x[i].z + x[i].w);
+        const float sum = ((p[0] + p[1]) + (p[2] + p[3])) + ((p[4] + p[5]) + (p[6] + p[7]));
+        if (sum != 0.f) atomicAdd(grad2d + (size_t)s_id1[j0 + row_e[r]] * GF + row_v[r], sum);
+      }
+    }
+    __syncwarp();
+  };
 
   // batches from the back: lane l of a batch stages saved entry end - 1 - l
   for (int end = cnt; end > 0; end -= kReplay) {
@@ -137,25 +149,29 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
       }
     }
     __syncwarp();
+    int pend = 0, j0 = 0;
     for (int j = 0; j < m; ++j) {
       const uint4 mk = s_mask1[j];
       const float4 a = rec[j * R4], l = rec[j * R4 + 1], oc = rec[j * R4 + 2];
-      const bool hit[kSlots] = {((mk.x >> g.lane) & 1u) != 0u, ((mk.y >> g.lane) & 1u) != 0u,
-                                ((mk.z >> g.lane) & 1u) != 0u, ((mk.w >> g.lane) & 1u) != 0u};
+      const bool hit[kSlots] = {(mk.x & lane_bit) != 0u, (mk.y & lane_bit) != 0u, (mk.z & lane_bit) != 0u, (mk.w & lane_bit) != 0u};
       float tail[TL];
       if (K > 0) load_tail<K>(rec + j * R4, tail);
       const float dx = __fsub_rn(g.lx, a.x);
       const float ux = __fmul_rn(l.x, dx);
       ModulationEntry<K> me;
       modulation_entry<K>(tail, dx, me);
-      float acc[NV];
+      // sums over the lane's blended pixels; the entry's constant factors are applied below
+      float Suu = 0.f, Suv = 0.f, Svv = 0.f, Squ = 0.f, Sqv = 0.f;   // dL/d(ln G) times w w^T and w, w = (u, v)
+      float So = 0.f, Sr = 0.f, Sgn = 0.f, Sb = 0.f;                 // d opacity, d rgb
+      float Sm = 0.f;                                                // sum of -dL/dM
+      float Sc[KK], St[KK], Sty[KK];                                 // sums of -dL/dM cos_k, -dL/dM sin_k, -dL/dM sin_k dy
+      float Sax = 0.f, Say = 0.f;                                    // AbsGS
+      float wfx[KK], wfy[KK];
 #pragma unroll
-      for (int i = 0; i < NV; ++i) acc[i] = 0.f;
-      // sums over the thread's pixels of terms whose common factors (dx, L, 2 pi f2D) are applied once, below
-      float Suu = 0.f, Suv = 0.f, Svv = 0.f, Squ = 0.f, Sqv = 0.f;
-      float Sg[K > 0 ? K : 1], Sgy[K > 0 ? K : 1];
-#pragma unroll
-      for (int k = 0; k < K; ++k) Sg[k] = Sgy[k] = 0.f;
+      for (int k = 0; k < K; ++k) {
+        Sc[k] = St[k] = Sty[k] = 0.f;
+        if (ABS) { wfx[k] = tail[2 * K + k] * tail[2 * k]; wfy[k] = tail[2 * K + k] * tail[2 * k + 1]; }
+      }
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) {
         if (!hit[s]) continue;
@@ -167,67 +183,72 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
         modulation<K, true>(tail, me, dy, e);
         const float raw = __fmul_rn(__fmul_rn(oc.x, G), e.M);
         const float alpha = fminf(kAlphaMax, raw);
-        const float om = 1.0f - alpha;
-        const float Ti = __fdividef(T[s], om);  // transmittance in front of this primitive
+        const float Ti = T[s] * rcp_fast(1.0f - alpha);  // transmittance in front of this primitive (1 - alpha >= 0.01)
         T[s] = Ti;
         const float aT = alpha * Ti;
-        acc[6] += aT * gC[s][0]; acc[7] += aT * gC[s][1]; acc[8] += aT * gC[s][2];
-        const float d0 = oc.y - B[s][0], d1 = oc.z - B[s][1], d2 = oc.w - B[s][2];  // colour minus what is behind
-        const float galpha = Ti * (gC[s][0] * d0 + gC[s][1] * d1 + gC[s][2] * d2);
-        B[s][0] = fmaf(alpha, d0, B[s][0]);  // = alpha c + (1 - alpha) B
-        B[s][1] = fmaf(alpha, d1, B[s][1]);
-        B[s][2] = fmaf(alpha, d2, B[s][2]);
+        Sr = fmaf(aT, gC[s][0], Sr); Sgn = fmaf(aT, gC[s][1], Sgn); Sb = fmaf(aT, gC[s][2], Sb);
+        // dL/dalpha = T <dL/dC, c - B>;  <dL/dC, B> is the carried scalar: B <- alpha c + (1 - alpha) B
+        const float dd = fmaf(gC[s][2], oc.w, fmaf(gC[s][1], oc.z, gC[s][0] * oc.y)) - A[s];
+        const float galpha = Ti * dd;
+        A[s] = fmaf(alpha, dd, A[s]);
         if (!(raw > kAlphaMax)) {  // the clamp min(0.99, .) has zero derivative when active
           const float gG = galpha * G;
-          acc[5] += gG * e.M;
+          So = fmaf(gG, e.M, So);
           const float ngM = -(gG * oc.x);   // -dL/dM
           const float gq = galpha * raw;    // dL/d(ln G)
           // the conic's gradient is accumulated in the whitened coordinates (u, v) of the envelope,
           // S = sum gq w w^T: its entries are O(gq) whatever the anisotropy of the footprint, where the sums of
           // gq dx^2, gq dx dy, gq dy^2 lose the thin direction of a needle that spans the screen in the other
           const float gqu = gq * u, gqv = gq * v;
-          Suu += gqu * u; Suv += gqu * v; Svv += gqv * v;
+          Suu = fmaf(gqu, u, Suu); Suv = fmaf(gqu, v, Suv); Svv = fmaf(gqv, v, Svv);
           Squ += gqu; Sqv += gqv;
+          Sm += ngM;
           float pdx = 0.f, pdy = 0.f;       // per-pixel d/d(dx), d/d(dy) through the phases (AbsGS only)
 #pragma unroll
           for (int k = 0; k < K; ++k) {
-            acc[9 + 2 * K + k] -= ngM * (e.cs[k] - 1.0f);
-            const float gph = ngM * tail[2 * K + k] * e.sn[k];  // dL/d(phase in radians)
-            Sg[k] += gph;
-            Sgy[k] += gph * dy;
-            if (ABS) { pdx += gph * tail[2 * k]; pdy += gph * tail[2 * k + 1]; }
+            Sc[k] = fmaf(ngM, e.cs[k], Sc[k]);
+            const float t = ngM * e.sn[k];  // dL/d(phase_k) = omega_k t
+            St[k] += t;
+            Sty[k] = fmaf(t, dy, Sty[k]);
+            if (ABS) { pdx = fmaf(t, wfx[k], pdx); pdy = fmaf(t, wfy[k], pdy); }
           }
           if (ABS) {
             // G = 2^q, q = -(u^2 + v^2), u = L11 dx + L21 dy, v = L22 dy:  dL/dq = gq ln 2
-            acc[9 + 3 * K] += fabsf(pdx + gq * (-1.3862943611198906f * u * l.x));
-            acc[10 + 3 * K] += fabsf(pdy + gq * (-1.3862943611198906f * (u * l.y + v * l.z)));
+            Sax += fabsf(pdx + gq * (-1.3862943611198906f * u * l.x));
+            Say += fabsf(pdy + gq * (-1.3862943611198906f * (u * l.y + v * l.z)));
           }
         }
       }
       {
-        // conic, in whitened form: S = sum dL/d(ln G) w w^T  (the projection backward maps it to dL/dU)
-        acc[2] = Suu;
-        acc[3] = Suv;
-        acc[4] = Svv;
+        float* col = s_red + pend * (NV * kRowStride) + g.lane;
         // mean: d = p - mu2D, so dL/dmu2D = -dL/dd;  dL/dd = dL/dq ln 2 (-2 u L11, -2 (u L21 + v L22)) + sum_k gph_k 2 pi f2D_k
         float gdx = -1.3862943611198906f * l.x * Squ;
         float gdy = -1.3862943611198906f * (l.y * Squ + l.z * Sqv);
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-          gdx += Sg[k] * tail[2 * k];
-          gdy += Sg[k] * tail[2 * k + 1];
-          acc[9 + 2 * k] = Sg[k] * dx;
-          acc[9 + 2 * k + 1] = Sgy[k];
+          const float w = tail[2 * K + k];
+          const float sg = w * St[k];            // sum of dL/d(phase_k)
+          gdx = fmaf(sg, tail[2 * k], gdx);
+          gdy = fmaf(sg, tail[2 * k + 1], gdy);
+          col[(9 + 2 * k) * kRowStride] = sg * dx;
+          col[(9 + 2 * k + 1) * kRowStride] = w * Sty[k];
+          col[(9 + 2 * K + k) * kRowStride] = Sm - Sc[k];   // -sum dL/dM (cos_k - 1)
         }
-        acc[0] = -gdx; acc[1] = -gdy;
+        col[0] = -gdx; col[kRowStride] = -gdy;
+        // conic, in whitened form: S = sum dL/d(ln G) w w^T  (the projection backward maps it to dL/dU)
+        col[2 * kRowStride] = Suu; col[3 * kRowStride] = Suv; col[4 * kRowStride] = Svv;
+        col[5 * kRowStride] = So;
+        col[6 * kRowStride] = Sr; col[7 * kRowStride] = Sgn; col[8 * kRowStride] = Sb;
+        if (ABS) { col[(9 + 3 * K) * kRowStride] = Sax; col[(10 + 3 * K) * kRowStride] = Say; }
       }
-      Butterfly<NV, 16>::run(acc, g.lane);
-      float* dst = grad2d + (size_t)s_id1[j] * GF;
-#pragma unroll
-      for (int i = 0; i < NL; ++i)
-        if (my_idx[i] >= 0 && acc[i] != 0.f) atomicAdd(dst + my_idx[i], acc[i]);
+      if (++pend == kGroup) {
+        flush(pend, j0);
+        pend = 0;
+        j0 = j + 1;
+      }
     }
-    __syncwarp();
+    if (pend) flush(pend, j0);
+    else __syncwarp();
   }
 }
 

@@ -8,8 +8,8 @@
 //   [3] MUFU.COS  cos.approx.ftz.f32 (range multiply + MUFU.COS), 8 chains             lane-ops / s
 //   [4] MIX       4 FFMA : 1 MUFU.EX2 per chain step (the blend's mix), all instructions  lane-instructions / s
 //   [5] IADD      add.s32 on the ALU pipe, 16 chains (the other half of the issue budget) lane-instructions / s
-// [8..13] the same six per SM per clock (from clock64 of one CTA: its SM's share while 8 CTAs are resident -- an
-// estimate), [6] = SM clock in Hz seen by the kernels (clock64 / %globaltimer of that CTA), [7] = number of SMs.  Nothing here is used to render.
+// [8..13] the same six per SM per clock (rate / (SMs x [6])), [6] = SM clock in Hz seen by the kernels (clock64 ticks per
+// %globaltimer ns of CTA 0), [7] = number of SMs.  Nothing here is used to render.
 #include "common.cuh"
 
 namespace gabsplat {
@@ -178,9 +178,10 @@ cudaError_t measure_peaks(float* results_host, void* scratch, cudaStream_t st) {
       if (rep == 0) continue;
       const double lane_instr = (double)grid * kPeakThreads * (double)kPeakIters * kInstrPerIter[mode];
       const double rate = lane_instr / (ms * 1e-3);
-      // one CTA's share of its SM: kPeakCtasPerSm CTAs run concurrently, each for `cyc` cycles
-      const double per_clk = (double)kPeakCtasPerSm * kPeakThreads * (double)kPeakIters * kInstrPerIter[mode] / (double)cyc;
-      if (rate > best_rate) { best_rate = rate; best_per_clk = per_clk; clock_hz = cn[1] > 0 ? (double)cyc / ((double)cn[1] * 1e-9) : 0.0; }
+      // per SM and clock: the device-wide rate over (SMs x the SM clock CTA 0 saw: clock64 ticks per %globaltimer ns)
+      const double hz = cn[1] > 0 ? (double)cyc / ((double)cn[1] * 1e-9) : 0.0;
+      const double per_clk = hz > 0.0 ? rate / ((double)sms * hz) : 0.0;
+      if (rate > best_rate) { best_rate = rate; best_per_clk = per_clk; clock_hz = hz; }
     }
     results_host[mode] = (float)best_rate;
     results_host[8 + mode] = (float)best_per_clk;

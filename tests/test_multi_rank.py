@@ -52,3 +52,24 @@ def test_single_rank_is_identity():
     import bench
     assert bench.max_over_ranks(3.5, None) == 3.5
     assert [bench.view_of_step(i, 0, 8) for i in range(9)] == [0, 1, 2, 3, 4, 5, 6, 7, 0]
+
+
+def test_bench_gpus_2_spawns_two_ranks():
+    """`python bench.py --gpus 2` with no launcher around it starts two ranks by itself (torchrun, 127.0.0.1) and
+    rank 0 prints one line for the whole job; --dry-run keeps it on the CPU (gloo, a stand-in step)."""
+    import json
+    import subprocess
+    env = dict(os.environ)
+    for k in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT"):
+        env.pop(k, None)
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "16", "--dry-run"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                   # one line, from rank 0
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["scaling"] == "weak"
+    assert out["ms_per_step"] == 1.5                         # max over ranks (rank 1 is the slow one)
+    assert out["value"] == 2 * 1297 * 840 / 1e6 / 1.5e-3     # both ranks' pixels over the slowest rank's time
+    v0, v1 = out["views_per_rank"]
+    assert all(a != b for a, b in zip(v0, v1)) and set(v0) == set(v1) == set(range(8))
