@@ -18,7 +18,10 @@ namespace {
 // ~39 * NV / 32 instructions where a shuffle butterfly took ~4.4 per value (23 SHFL + 23 FADD + 46 FSEL at NV = 21),
 // and the additions of different rows are independent (no 5-deep shuffle chain).
 constexpr int kRowStride = 36;   // floats: 16-byte aligned rows whose vector loads spread over the banks
-constexpr int kMaxRows = 64;     // rows a group may fill (two rounds)
+#ifndef GS_BWD_MAXROWS
+#define GS_BWD_MAXROWS 64
+#endif
+constexpr int kMaxRows = GS_BWD_MAXROWS;     // rows a group may fill (two rounds)
 
 __host__ __device__ constexpr int group_entries(int NV) {
   int best = 1, best_fill = 0;
@@ -33,7 +36,10 @@ __host__ __device__ constexpr int group_entries(int NV) {
 }
 __host__ __device__ constexpr int group_rows(int NV) { return NV > kMaxRows ? NV : group_entries(NV) * NV; }
 
-constexpr int kReplay = 32;  // saved entries staged per warp and batch
+#ifndef GS_BWD_REPLAY
+#define GS_BWD_REPLAY 32
+#endif
+constexpr int kReplay = GS_BWD_REPLAY;  // saved entries staged per warp and batch
 
 __device__ __forceinline__ float rcp_fast(float x) {  // x in [0.01, 1]: no denormal, no special case
   float r;
@@ -51,8 +57,11 @@ __device__ __forceinline__ float rcp_fast(float x) {  // x in [0.01, 1]: no deno
 // Per pixel the colour behind the primitive enters only through <dL/dC, B>, so that scalar is what is carried
 // (A <- A + alpha (<dL/dC, c> - A)), and every factor that is constant over the entry (omega_k, 2 pi f2D_k, L, dx)
 // is applied once per entry to sums taken over the lane's pixels.
+#ifndef GS_BWD_MINB
+#define GS_BWD_MINB 16
+#endif
 template <int K, bool ABS>
-__global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, const uint2* __restrict__ ranges,
+__global__ void __launch_bounds__(32, GS_BWD_MINB) blend_backward_kernel(Camera cam, const uint2* __restrict__ ranges,
                                                                        BlendState saved, const float4* __restrict__ packed,
                                                                        const float* __restrict__ final_T,
                                                                        const float* __restrict__ dL_dimage,
@@ -70,7 +79,7 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
   __shared__ float4 s_rec1[kReplay * R4];
   __shared__ uint4 s_mask1[kReplay];
   __shared__ uint32_t s_id1[kReplay];
-  __shared__ __align__(16) float s_red[kRounds * 32 * kRowStride];
+  __shared__ __align__(16) float s_red[kRows * kRowStride];
   const uint32_t half = __ldg(saved.order + blockIdx.x);
   const TileGeom g = tile_geom_at(cam, (int)(half >> 1), (int)(half & 1u), (int)threadIdx.x);
   const uint2 range = ranges[g.tile];
@@ -131,11 +140,11 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
     if (g.lane < m) {
       my_id = __ldg(saved.ids + base + (size_t)(end - 1 - g.lane));
       my_mask = __ldg(saved.masks + base + (size_t)(end - 1 - g.lane));
+      s_id1[g.lane] = my_id;
+      s_mask1[g.lane] = my_mask;
     }
-    s_id1[g.lane] = my_id;
-    s_mask1[g.lane] = my_mask;
 #pragma unroll
-    for (int it = 0; it < R4; ++it) {
+    for (int it = 0; it < (kReplay * R4 + 31) / 32; ++it) {
       const int idx = it * 32 + g.lane;
       const int r = idx / R4, part = idx - r * R4;
       const uint32_t id_r = __shfl_sync(kFull, my_id, r);
@@ -174,7 +183,9 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
       }
 #pragma unroll
       for (int s = 0; s < kSlots; ++s) {
+#ifndef GS_BWD_BRANCHFREE
         if (!hit[s]) continue;
+#endif
         float u, v;
         const float dy = __fsub_rn(g.ly[s], a.y);
         const float q = envelope_q(ux, l.y, l.z, dy, u, v);
@@ -182,16 +193,27 @@ __global__ void __launch_bounds__(32, 16) blend_backward_kernel(Camera cam, cons
         Modulation<K> e;
         modulation<K, true>(tail, me, dy, e);
         const float raw = __fmul_rn(__fmul_rn(oc.x, G), e.M);
+#ifdef GS_BWD_BRANCHFREE
+        // the four pixels of a lane as four independent chains without branches: a pixel that did not blend the entry
+        // takes alpha = 0 (T, A unchanged) and dL/dalpha = 0 (every sum receives zeros) by selects
+        const float alpha = hit[s] ? fminf(kAlphaMax, raw) : 0.0f;
+#else
         const float alpha = fminf(kAlphaMax, raw);
+#endif
         const float Ti = T[s] * rcp_fast(1.0f - alpha);  // transmittance in front of this primitive (1 - alpha >= 0.01)
         T[s] = Ti;
         const float aT = alpha * Ti;
         Sr = fmaf(aT, gC[s][0], Sr); Sgn = fmaf(aT, gC[s][1], Sgn); Sb = fmaf(aT, gC[s][2], Sb);
         // dL/dalpha = T <dL/dC, c - B>;  <dL/dC, B> is the carried scalar: B <- alpha c + (1 - alpha) B
         const float dd = fmaf(gC[s][2], oc.w, fmaf(gC[s][1], oc.z, gC[s][0] * oc.y)) - A[s];
-        const float galpha = Ti * dd;
         A[s] = fmaf(alpha, dd, A[s]);
+#ifdef GS_BWD_BRANCHFREE
+        const float galpha = (hit[s] && !(raw > kAlphaMax)) ? Ti * dd : 0.0f;  // the clamp min(0.99, .) has zero derivative when active
+        {
+#else
+        const float galpha = Ti * dd;
         if (!(raw > kAlphaMax)) {  // the clamp min(0.99, .) has zero derivative when active
+#endif
           const float gG = galpha * G;
           So = fmaf(gG, e.M, So);
           const float ngM = -(gG * oc.x);   // -dL/dM
