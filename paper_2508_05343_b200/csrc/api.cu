@@ -6,17 +6,6 @@
 
 #include "common.cuh"
 
-struct gabsplat_ctx {
-  int device;
-  uint64_t* pinned_count;  // 8-byte pinned readback slot for D
-  cudaStream_t side;       // side stream: the zeroing of the gradient arrays overlaps the blend backward
-  cudaEvent_t ev_fork, ev_join;
-  void* scratch;           // 256 bytes of device scratch (instrumentation)
-  int place_bands;         // 0 = automatic (gabsplat_set_place_bands)
-  gabsplat::StageTimer timer;
-  char error[256];
-};
-
 namespace gabsplat {
 std::atomic<unsigned long long> g_kernel_launches{0};
 }
@@ -93,8 +82,13 @@ int32_t gabsplat_create(gabsplat_ctx** out, int32_t device) {
     return GABSPLAT_CUDA;
   }
   ctx->side = nullptr; ctx->ev_fork = ctx->ev_join = nullptr; ctx->scratch = nullptr;
+  ctx->copy_in = ctx->copy_out = nullptr;
+  for (cudaEvent_t& e : ctx->ev_copy) e = nullptr;
   ctx->place_bands = 0;
-  if (cudaMalloc(&ctx->scratch, 256) != cudaSuccess ||
+  bool ok = cudaStreamCreateWithFlags(&ctx->copy_in, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&ctx->copy_out, cudaStreamNonBlocking) == cudaSuccess;
+  for (cudaEvent_t& e : ctx->ev_copy) ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+  if (!ok || cudaMalloc(&ctx->scratch, 256) != cudaSuccess ||
       cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess) {
@@ -112,6 +106,9 @@ void gabsplat_destroy(gabsplat_ctx* ctx) {
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
   if (ctx->side) cudaStreamDestroy(ctx->side);
+  if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
+  if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
+  for (cudaEvent_t e : ctx->ev_copy) if (e) cudaEventDestroy(e);
   if (ctx->scratch) cudaFree(ctx->scratch);
   ctx->timer.destroy();
   delete ctx;
@@ -151,9 +148,18 @@ int32_t gabsplat_preprocess(gabsplat_ctx* ctx, const gabsplat_scene* scene, cons
 int32_t gabsplat_preprocess_bin_sort(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
                                      gabsplat_projected* proj, gabsplat_binning* bin, uint64_t* num_instances_host,
                                      void* stream) {
+  return gabsplat_preprocess_bin_sort_ordered(ctx, scene, cam, proj, bin, num_instances_host, stream, nullptr);
+}
+
+}  // extern "C"
+
+int32_t gabsplat_preprocess_bin_sort_ordered(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                                             gabsplat_projected* proj, gabsplat_binning* bin, uint64_t* num_instances_host,
+                                             void* stream, cudaEvent_t value_inputs_ready) {
   if (!ctx) return GABSPLAT_INVALID_ARG;
   // with the stage timer on, or nothing to overlap, this is exactly the two calls
   if (ctx->timer.on || !scene || scene->N <= 0) {
+    if (value_inputs_ready && cudaStreamWaitEvent((cudaStream_t)stream, value_inputs_ready, 0) != cudaSuccess) return GABSPLAT_CUDA;
     const int32_t rc = gabsplat_preprocess(ctx, scene, cam, proj, stream);
     return rc != GABSPLAT_OK ? rc : gabsplat_bin_sort(ctx, scene->N, proj, cam, bin, num_instances_host, stream);
   }
@@ -162,7 +168,8 @@ int32_t gabsplat_preprocess_bin_sort(gabsplat_ctx* ctx, const gabsplat_scene* sc
   if (!projected_ok(proj, scene->N, scene->K)) return fail(ctx, GABSPLAT_INVALID_ARG, "preprocess_bin_sort: null output");
   cudaStream_t st = (cudaStream_t)stream;
   // the binning needs only the indexing track: the fp64 value track runs on the side stream beside it
-  cudaError_t e = launch_preprocess(*scene, make_camera(*cam), *proj, st, ctx->side, ctx->ev_fork);
+  cudaError_t e = value_inputs_ready ? cudaStreamWaitEvent(ctx->side, value_inputs_ready, 0) : cudaSuccess;
+  if (e == cudaSuccess) e = launch_preprocess(*scene, make_camera(*cam), *proj, st, ctx->side, ctx->ev_fork);
   if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_join, ctx->side);
   if (e != cudaSuccess) return cuda_fail(ctx, e, "preprocess_bin_sort (projection)");
   const int32_t rc = gabsplat_bin_sort(ctx, scene->N, proj, cam, bin, num_instances_host, stream);
@@ -170,6 +177,8 @@ int32_t gabsplat_preprocess_bin_sort(gabsplat_ctx* ctx, const gabsplat_scene* sc
   if (e != cudaSuccess) return cuda_fail(ctx, e, "preprocess_bin_sort (join)");
   return rc;
 }
+
+extern "C" {
 
 int32_t gabsplat_bin_sort(gabsplat_ctx* ctx, int32_t N, const gabsplat_projected* proj, const gabsplat_camera* cam,
                           gabsplat_binning* bin, uint64_t* num_instances_host, void* stream) {

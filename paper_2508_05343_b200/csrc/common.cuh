@@ -182,3 +182,25 @@ uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles);
 bool keys_optional(int ntiles);  // true when the binning never reads gabsplat_binning.keys itself
 
 }  // namespace gabsplat
+
+// The context (opaque to callers).  It owns no per-call state: a pinned readback slot, a side stream for work that has
+// no consumer on the critical path, two copy streams for gabsplat_render_host, and the events that order them.
+struct gabsplat_ctx {
+  int device;
+  uint64_t* pinned_count;  // 8-byte pinned readback slot for D
+  cudaStream_t side;       // side stream: the zeroing of the gradient arrays overlaps the blend backward
+  cudaEvent_t ev_fork, ev_join;
+  cudaStream_t copy_in, copy_out;            // gabsplat_render_host: uploads / downloads beside the kernels
+  cudaEvent_t ev_copy[5];                    // ... and their ordering
+  void* scratch;           // 256 bytes of device scratch (instrumentation)
+  int place_bands;         // 0 = automatic (gabsplat_set_place_bands)
+  gabsplat::StageTimer timer;
+  char error[256];
+};
+
+// S1 + S2 as gabsplat_preprocess_bin_sort runs them; `value_inputs_ready` (may be null) is an event the fp64 value track
+// waits for on the side stream: gabsplat_render_host starts the indexing track and the binning as soon as means, scales
+// and rotations have arrived, while the rest of the scene is still on its way.
+int32_t gabsplat_preprocess_bin_sort_ordered(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
+                                             gabsplat_projected* proj, gabsplat_binning* bin, uint64_t* num_instances_host,
+                                             void* stream, cudaEvent_t value_inputs_ready);

@@ -102,42 +102,69 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* sh, const 
   Layout l = carve(device_arena, sh->N, sh->K, cam->width, cam->height, capacity);
   if (arena_bytes < l.bytes) return GABSPLAT_CAPACITY;
   l.scene.sh_degree = sh->sh_degree;
-  cudaStream_t st = (cudaStream_t)stream;
+  cudaStream_t st = (cudaStream_t)stream, cin = ctx->copy_in, cout = ctx->copy_out;
   const uint64_t n = (uint64_t)sh->N, k = (uint64_t)sh->K, hw = (uint64_t)cam->width * cam->height, f = sizeof(float);
-#define GS_H2D(dst, src, count) \
-  if ((count) && cudaMemcpyAsync((void*)(dst), (src), (count) * f, cudaMemcpyHostToDevice, st) != cudaSuccess) return GABSPLAT_CUDA
-#define GS_D2H(dst, src, count) \
-  if ((count) && cudaMemcpyAsync((dst), (const void*)(src), (count) * f, cudaMemcpyDeviceToHost, st) != cudaSuccess) return GABSPLAT_CUDA
+  // Uploads run on a copy stream in the order the kernels need them, downloads on another; the kernels wait for exactly
+  // the arrays they read:
+  //   means, scales, rotations (40 B per primitive)  -> the indexing track and the whole binning start
+  //   opacities, frequencies, weights, SH colours    -> the value track (side stream, beside the binning), the blends
+  //   dL/dimage                                      -> the backward
+  //   image                                          <- leaves while the backward runs
+#define GS_CK(call) if ((call) != cudaSuccess) return GABSPLAT_CUDA
+#define GS_H2D(dst, src, count) if (count) GS_CK(cudaMemcpyAsync((void*)(dst), (src), (count) * f, cudaMemcpyHostToDevice, cin))
+#define GS_D2H(dst, src, count, s) if (count) GS_CK(cudaMemcpyAsync((dst), (const void*)(src), (count) * f, cudaMemcpyDeviceToHost, s))
+  GS_CK(cudaEventRecord(ctx->ev_copy[0], st));          // whatever the caller queued before this call
+  GS_CK(cudaStreamWaitEvent(cin, ctx->ev_copy[0], 0));
+  GS_CK(cudaStreamWaitEvent(cout, ctx->ev_copy[0], 0));
   GS_H2D(l.scene.means, sh->means, n * 3);
   GS_H2D(l.scene.scales, sh->scales, n * 3);
   GS_H2D(l.scene.rotations, sh->rotations, n * 4);
+  GS_CK(cudaEventRecord(ctx->ev_copy[1], cin));
   GS_H2D(l.scene.opacities, sh->opacities, n);
-  GS_H2D(l.scene.sh, sh->sh, n * 48);
   GS_H2D(l.scene.freqs, sh->freqs, n * k * 3);
   GS_H2D(l.scene.weights, sh->weights, n * k);
-  if (dL_dimage_host) GS_H2D(l.dL, dL_dimage_host, 3 * hw);
-  uint64_t D = 0;
-  int32_t rc = gabsplat_preprocess_bin_sort(ctx, &l.scene, cam, &l.proj, &l.bin, &D, stream);
+  GS_H2D(l.scene.sh, sh->sh, n * 48);
+  GS_CK(cudaEventRecord(ctx->ev_copy[2], cin));
+  if (dL_dimage_host) {
+    GS_H2D(l.dL, dL_dimage_host, 3 * hw);
+    GS_CK(cudaEventRecord(ctx->ev_copy[3], cin));
+  }
+  l.scene.variant = sh->variant;
+  GS_CK(cudaStreamWaitEvent(st, ctx->ev_copy[1], 0));
+  int32_t rc = gabsplat_preprocess_bin_sort_ordered(ctx, &l.scene, cam, &l.proj, &l.bin, nullptr, stream, ctx->ev_copy[2]);
   if (rc != GABSPLAT_OK) return rc;
   if (!dL_dimage_host) l.fwd.blend_state = nullptr;  // inference: nothing to replay
   rc = gabsplat_render_forward(ctx, &l.scene, cam, &l.proj, &l.bin, &l.fwd, stream);
   if (rc != GABSPLAT_OK) return rc;
-  GS_D2H(image_host, l.fwd.image, 3 * hw);
+  GS_CK(cudaEventRecord(ctx->ev_copy[4], st));
+  GS_CK(cudaStreamWaitEvent(cout, ctx->ev_copy[4], 0));
+  GS_D2H(image_host, l.fwd.image, 3 * hw, cout);
+  uint32_t* count_slot = reinterpret_cast<uint32_t*>(ctx->pinned_count);
+  GS_CK(cudaMemcpyAsync(count_slot, l.bin.num_instances, sizeof(uint32_t), cudaMemcpyDeviceToHost, cout));
   if (dL_dimage_host) {
+    GS_CK(cudaStreamWaitEvent(st, ctx->ev_copy[3], 0));
     rc = gabsplat_render_backward(ctx, &l.scene, cam, &l.proj, &l.bin, &l.fwd, l.dL, &l.grads, l.grad_ws,
                                   l.grad_ws_bytes, stream);
     if (rc != GABSPLAT_OK) return rc;
-    GS_D2H(gh->d_means, l.grads.d_means, n * 3);
-    GS_D2H(gh->d_scales, l.grads.d_scales, n * 3);
-    GS_D2H(gh->d_rotations, l.grads.d_rotations, n * 4);
-    GS_D2H(gh->d_opacities, l.grads.d_opacities, n);
-    GS_D2H(gh->d_sh, l.grads.d_sh, n * 48);
-    GS_D2H(gh->d_freqs, l.grads.d_freqs, n * k * 3);
-    GS_D2H(gh->d_weights, l.grads.d_weights, n * k);
+    GS_D2H(gh->d_means, l.grads.d_means, n * 3, st);
+    GS_D2H(gh->d_scales, l.grads.d_scales, n * 3, st);
+    GS_D2H(gh->d_rotations, l.grads.d_rotations, n * 4, st);
+    GS_D2H(gh->d_opacities, l.grads.d_opacities, n, st);
+    GS_D2H(gh->d_sh, l.grads.d_sh, n * 48, st);
+    GS_D2H(gh->d_freqs, l.grads.d_freqs, n * k * 3, st);
+    GS_D2H(gh->d_weights, l.grads.d_weights, n * k, st);
   }
 #undef GS_H2D
 #undef GS_D2H
-  if (cudaStreamSynchronize(st) != cudaSuccess) return GABSPLAT_CUDA;
+  // the caller's stream ends after everything this call queued anywhere
+  GS_CK(cudaEventRecord(ctx->ev_copy[0], cout));
+  GS_CK(cudaStreamWaitEvent(st, ctx->ev_copy[0], 0));
+  GS_CK(cudaEventRecord(ctx->ev_copy[1], cin));
+  GS_CK(cudaStreamWaitEvent(st, ctx->ev_copy[1], 0));
+  GS_CK(cudaStreamSynchronize(st));
+#undef GS_CK
+  // an instance list larger than `capacity` renders the background only (every stage checks the count on the device)
+  if ((uint64_t)*count_slot > capacity) return GABSPLAT_CAPACITY;
   return GABSPLAT_OK;
 }
 
