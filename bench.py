@@ -209,7 +209,8 @@ def max_over_ranks(ms: float, dist, device=None) -> float:
 def workload_config(args, name, scene, cam) -> dict:
     return {"workload": "%s: N=%d primitives, K=%d, SH degree 3, %dx%d, 8 seeded views, %s" % (
                 name, scene.N, scene.K, cam.width, cam.height,
-                "forward" if args.forward_only else "forward+backward"),
+                "forward" if args.forward_only else "forward+backward") +
+                        "; the sorted 64-bit keys are not materialised in the timed step (no stage reads them)",
             "config_name": name, "N": scene.N, "K": scene.K, "width": cam.width, "height": cam.height,
             "zero_weights": bool(args.zero_weights),
             "l2_policy": "inputs larger than L2 (scene %.0f MB + gradients %.0f MB per step vs 126 MB L2)" % (
@@ -406,14 +407,29 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     dominant = max(per_stage, key=lambda s: per_stage[s]["ms"])
     roofline = {"kernel": dominant, **{k: per_stage[dominant][k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
                 "peak_kind": per_stage[dominant]["peak_kind"]}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")   # ncu-measured DRAM bytes per launch, if recorded
+    # ncu-measured per-launch figures of the stage's kernels, if recorded (profiles/traffic.json): DRAM bytes, and the
+    # executed warp instructions, from which the issue-slot utilisation of the live time follows (the numerators above
+    # are the METHOD's work; this is what the kernel as built executes)
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file):
         with open(traffic_file) as f:
             tr = json.load(f)
+        issue_slots_per_s = alu_peaks["sms"] * 4 * alu_peaks["sm_clock_hz"]
         for s in per_stage:
-            if s in tr.get(name, {}):
-                per_stage[s]["traffic"] = tr[name][s]
+            rec = tr.get(name, {}).get(s)
+            if isinstance(rec, dict):
+                per_stage[s]["traffic"] = rec.get("dram_bytes")
+                if rec.get("warp_instr") and K == 4 and not args.zero_weights:
+                    per_stage[s]["executed_warp_instr"] = rec["warp_instr"]
+                    per_stage[s]["issue_slot_utilisation"] = rec["warp_instr"] / (per_stage[s]["ms"] / 1e3 * issue_slots_per_s)
+            elif rec is not None:
+                per_stage[s]["traffic"] = rec
         roofline["traffic"] = per_stage[dominant]["traffic"]
+        for k in ("executed_warp_instr", "issue_slot_utilisation"):
+            if k in per_stage[dominant]:
+                roofline[k] = per_stage[dominant][k]
+    roofline["alu_peaks_measured"] = {k: alu_peaks[k] for k in ("ffma", "mufu_ex2", "mufu_cos", "mix_4ffma_1mufu", "alu_iadd",
+                                                                 "sm_clock_hz", "sms")}
 
     # end to end through the C ABI with HOST buffers (gabsplat_render_host): H2D of the scene and dL/dimage,
     # D2H of the image and the gradients, all inside the timed region

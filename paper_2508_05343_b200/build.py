@@ -4,6 +4,10 @@
 
 nvcc cross-compiles without a GPU.  The library lands next to this file so that it travels with the
 repository snapshot to the GPU box (it is git-ignored, not gpurun-ignored).
+
+GABSPLAT_NVCC_FLAGS (environment, optional): extra nvcc flags, e.g. the -D switches of the measured design alternatives
+kept in the sources (GS_FWD_STAGING_CPASYNC, GS_BWD_BRANCHFREE, GS_BWD_MINB, GS_BWD_REPLAY, GS_BWD_MAXROWS: DESIGN.md 7.4).
+Use --force with it; the default build is what the tests and bench.py measure.
 """
 from __future__ import annotations
 
@@ -43,7 +47,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         s = os.path.join(CSRC, src)
         o = os.path.join(OBJ, src.replace(".cu", ".o"))
         if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr_time):
-            cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
+            cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("GABSPLAT_NVCC_FLAGS", "").split() + \
+                  (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
             jobs.append(cmd)
 
     def run(cmd):

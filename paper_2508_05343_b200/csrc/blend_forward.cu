@@ -12,6 +12,28 @@ namespace {
 // entries examined / past the envelope test / blended is written to `counters` instead of the image.
 // SAVE = also record, per warp (half tile), the primitives blended at one of its pixels and the ballots of the
 // blending lanes (common.cuh BlendState): the backward replays exactly this list.
+#ifdef GS_FWD_STAGING_CPASYNC
+// The staging experiment north_star (3) asks for ("TMA bulk copies where they pay"), kept buildable so that its
+// measurement can be repeated (GABSPLAT_NVCC_FLAGS=-DGS_FWD_STAGING_CPASYNC python -m paper_2508_05343_b200.build --force):
+// the batches of a tile's list staged by a three-deep software pipeline of asynchronous copies (cp.async / LDGSTS; the
+// gathers are data-dependent 16-byte pieces of records, which the tensor form of TMA cannot address).  Measured at the
+// headline config: 0.552 ms (64-entry batches, 10 CTAs/SM) and 0.579 ms (128-entry batches, 7 CTAs/SM by shared memory)
+// against 0.527 ms for the synchronous staging below -- the loads it hides were already covered by the other CTAs of
+// the SM, and it costs occupancy and a batch of filtering past the point where the tile saturates.  DESIGN.md 7.4.
+// ---- asynchronous copies global -> shared (LDGSTS): the staging pipeline below keeps them in flight while a batch is blended
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+#ifndef GS_FWD_BATCH
+#define GS_FWD_BATCH 64
+#endif
+constexpr int kFwdBatch = GS_FWD_BATCH;              // list entries filtered per batch
+constexpr int kFwdPer = kFwdBatch / kBlendThreads;   // ... per thread
+#endif
+
 template <int K, bool COUNT, bool SAVE>
 __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam, const uint32_t* __restrict__ order,
                                                                       const uint2* __restrict__ ranges,
@@ -24,8 +46,15 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
   pdl_wait();
   constexpr int R4 = packed_floats(K) / 4;
   constexpr int TL = K > 0 ? 4 * ((3 * K + 3) / 4) : 1;
+#ifdef GS_FWD_STAGING_CPASYNC
+  __shared__ float4 s_rec[2][kFwdBatch * R4];
+  __shared__ float4 s_head[kFwdBatch * 2];
+  __shared__ uint32_t s_ids[kFwdBatch];
+  __shared__ uint32_t s_cnt[kFwdPer * (kBlendThreads / 32)];
+#else
   __shared__ float4 s_rec[kBatch * R4];
   __shared__ uint32_t s_cnt[8];
+#endif
   const TileGeom g = tile_geom(cam, order);
   const uint2 range = ranges[g.tile];
   const int n = (int)(range.y - range.x);
@@ -43,18 +72,127 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
     stop_pos[s] = 0;
   }
 
+#ifdef GS_FWD_STAGING_CPASYNC
+  const int tid = threadIdx.x;
+  // ids of batch b -> registers
+  auto load_ids = [&](int b, uint32_t (&idv)[kFwdPer]) {
+#pragma unroll
+    for (int r = 0; r < kFwdPer; ++r) {
+      const int p = b * kFwdBatch + r * kBlendThreads + tid;
+      idv[r] = p < n ? __ldg(ids + range.x + (uint32_t)p) : 0u;
+    }
+  };
+  // heads of batch b -> s_head, asynchronously; every thread copies (and later filters) its own candidates
+  auto issue_heads = [&](int b, const uint32_t (&idv)[kFwdPer]) {
+#pragma unroll
+    for (int r = 0; r < kFwdPer; ++r) {
+      const int c = r * kBlendThreads + tid;
+      if (b * kFwdBatch + c < n) {
+        const float4* src = packed + (size_t)idv[r] * R4;
+        cp_async16(&s_head[2 * c], src);
+        cp_async16(&s_head[2 * c + 1], src + 1);
+        s_ids[c] = idv[r];
+      }
+    }
+  };
+  // Filters batch b (its heads have landed in s_head), compacts the survivors in list order into s_rec[buf] -- heads by
+  // plain stores, tails by asynchronous copies -- and returns their number.  Contains one __syncthreads.
+  auto filter_compact = [&](int b, int buf) -> int {
+    float4 h0[kFwdPer], h1[kFwdPer];
+    uint32_t bal[kFwdPer];
+    bool keep[kFwdPer];
+#pragma unroll
+    for (int r = 0; r < kFwdPer; ++r) {
+      const int c = r * kBlendThreads + tid;
+      const int p = b * kFwdBatch + c;
+      keep[r] = false;
+      if (p < n) {
+        const float4 a = s_head[2 * c], l = s_head[2 * c + 1];
+        // mean relative to the tile origin: (hi - origin) + lo
+        const float mx = __fadd_rn(__fsub_rn(a.x, g.x0), a.z);
+        const float my = __fadd_rn(__fsub_rn(a.y, g.y0), a.w);
+        h0[r] = make_float4(mx, my, l.x, l.y);
+        h1[r] = make_float4(l.z, l.w, __uint_as_float((uint32_t)p + 1u), __uint_as_float(s_ids[c]));
+        keep[r] = tile_may_pass(mx, my, l.x, l.y, l.z, l.w);
+      }
+      bal[r] = __ballot_sync(kFull, keep[r]);
+      if (g.lane == 0) s_cnt[r * (kBlendThreads / 32) + g.warp] = __popc(bal[r]);
+    }
+    __syncthreads();
+    constexpr int kGroups = kFwdPer * (kBlendThreads / 32);
+    uint32_t total = 0;
+    uint32_t base[kFwdPer];
+#pragma unroll
+    for (int r = 0; r < kFwdPer; ++r) base[r] = 0;
+#pragma unroll
+    for (int q = 0; q < kGroups; ++q) {
+#pragma unroll
+      for (int r = 0; r < kFwdPer; ++r)
+        if (q == r * (kBlendThreads / 32) + g.warp) base[r] = total;
+      total += s_cnt[q];
+    }
+    const uint32_t lt = (1u << g.lane) - 1u;
+#pragma unroll
+    for (int r = 0; r < kFwdPer; ++r) {
+      if (keep[r]) {
+        const uint32_t slot = base[r] + __popc(bal[r] & lt);
+        float4* dst = &s_rec[buf][slot * R4];
+        dst[0] = h0[r];
+        dst[1] = h1[r];
+        const uint32_t pid = __float_as_uint(h1[r].w);
+        const float4* src = packed + (size_t)pid * R4;
+#pragma unroll
+        for (int ch = 2; ch < R4; ++ch) cp_async16(dst + ch, (ch == 2 && colour) ? colour + pid : src + ch);
+      }
+    }
+    return (int)total;
+  };
+
+#endif
   uint32_t n_saved = 0;                                        // warp-uniform
   const size_t save_at = 2 * (size_t)range.x + (size_t)g.warp * n;  // this warp's slice of save.ids / save.masks
   uint32_t* save_id = SAVE ? save.ids + save_at : nullptr;          // lane 0's write cursors
   uint4* save_mask = SAVE ? save.masks + save_at : nullptr;
+#ifdef GS_FWD_STAGING_CPASYNC
+  const int nbatch = (n + kFwdBatch - 1) / kFwdBatch;
+  uint32_t idn[kFwdPer];   // ids of the batch whose heads are issued next
+  int ns = 0;              // survivors of the batch about to be blended
+  if (nbatch > 0) {        // prologue: the only exposed latencies of the tile
+    load_ids(0, idn);
+    issue_heads(0, idn);
+    if (nbatch > 1) load_ids(1, idn);
+    cp_async_wait_all();
+    ns = filter_compact(0, 0);
+    if (nbatch > 1) issue_heads(1, idn);
+    if (nbatch > 2) load_ids(2, idn);
+    cp_async_wait_all();
+    __syncthreads();
+  }
+  for (int b = 0; b < nbatch; ++b) {
+    const bool all_done = done[0] && done[1] && done[2] && done[3];
+    if (__syncthreads_and(all_done)) break;
+    int ns_next = 0;
+    if (b + 1 < nbatch) {
+      ns_next = filter_compact(b + 1, (b + 1) & 1);
+      if (b + 2 < nbatch) issue_heads(b + 2, idn);
+      if (b + 3 < nbatch) load_ids(b + 3, idn);
+    }
+    const float4* __restrict__ recs = s_rec[b & 1];
+    const int nj = __all_sync(kFull, all_done) ? 0 : ns;  // warp-uniform: the votes below need every lane
+#define GS_FWD_RECS recs
+#define GS_FWD_NJ nj
+#else
   for (int b0 = 0; b0 < n; b0 += kBatch) {
     const bool all_done = done[0] && done[1] && done[2] && done[3];
     if (__syncthreads_and(all_done)) break;
     const int m = min(kBatch, n - b0);
     const int ns = stage_batch<K, false>(g, ids, packed, colour, range.x, b0, m, s_rec, s_cnt);
     if (__all_sync(kFull, all_done)) continue;  // warp-uniform: the votes below need every lane
-    for (int j = 0; j < ns; ++j) {
-      const float4 h0 = s_rec[j * R4], h1 = s_rec[j * R4 + 1];
+#define GS_FWD_RECS s_rec
+#define GS_FWD_NJ ns
+#endif
+    for (int j = 0; j < GS_FWD_NJ; ++j) {
+      const float4 h0 = GS_FWD_RECS[j * R4], h1 = GS_FWD_RECS[j * R4 + 1];
       const float dx = __fsub_rn(g.lx, h0.x);
       const float ux = __fmul_rn(h0.z, dx);
       float dy[kSlots], q[kSlots];
@@ -69,9 +207,9 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
         any = any || pass[s];
       }
       if (!__any_sync(kFull, any)) continue;  // warp-uniform
-      const float4 oc = s_rec[j * R4 + 2];
+      const float4 oc = GS_FWD_RECS[j * R4 + 2];
       float tail[TL];
-      if (K > 0) load_tail<K>(s_rec + j * R4, tail);
+      if (K > 0) load_tail<K>(GS_FWD_RECS + j * R4, tail);
       const uint32_t pos = __float_as_uint(h1.z);
       ModulationEntry<K> me;
       modulation_entry<K>(tail, dx, me);
@@ -125,6 +263,11 @@ __global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam
         }
       }
     }
+#ifdef GS_FWD_STAGING_CPASYNC
+    cp_async_wait_all();   // tails of batch b + 1, heads of batch b + 2: they had the whole batch to land
+    __syncthreads();
+    ns = ns_next;
+#endif
   }
   if (SAVE && g.lane == 0) save.counts[2 * g.tile + g.warp] = n_saved;
   const size_t HW = (size_t)cam.width * cam.height;
