@@ -8,15 +8,18 @@
 //                      separable 11-tap filter through shared memory, SSIM and its three partial derivatives
 //                      (dS/dmx, dS/dExx, dS/dExy) per pixel, per-CTA partial sums of |x - y| and SSIM
 //   loss_grad_kernel   the same separable filter over the three derivative maps, combined with x, y and sign(x - y)
-// The windowed sums are accumulated in fp64 (Exx - mx^2 cancels against C2 = 9e-4; the arithmetic is free next to
-// the memory traffic) and the partial sums are reduced in a fixed order, so the loss is deterministic.
+// The windowed sums are accumulated in fp64 (Exx - mx^2 cancels against C2 = 9e-4) and the partial sums are reduced in
+// a fixed order, so the loss is deterministic.  What the kernels spend is the fp64 filter arithmetic (11 + 11 DFMA per
+// quantity and pixel, plus the halo rows), so everything around it is kept off the instruction stream: a thread of
+// the horizontal pass converts and multiplies each input ONCE and feeds it to the 4 neighbouring outputs it owns; a
+// thread of the vertical pass owns two adjacent rows, whose 11-row windows share 10 rows.
 #include "common.cuh"
 
 namespace gabsplat {
 namespace {
 
 constexpr int kR = 5;             // window radius
-constexpr int kTX = 32, kTY = 16;  // output tile: two pixels per thread (rows ty and ty + 8)
+constexpr int kTX = 32, kTY = 16;  // output tile: two pixels per thread (rows 2 ty and 2 ty + 1)
 constexpr int kHX = kTX + 2 * kR, kHY = kTY + 2 * kR;
 constexpr int kLossThreads = 256;
 constexpr double kC1 = 0.01 * 0.01, kC2 = 0.03 * 0.03;
@@ -33,34 +36,65 @@ inline Taps make_taps() {
 
 // Separable filter of NQ quantities over one tile.  in(r, c, v) gives the NQ input values at halo position (r, c)
 // (zero outside the image); s_h[q][kHY][kTX] receives the horizontal sums; out[q][h] = the filtered value at the
-// thread's output pixels (tile rows ty + 8 h, column tx).
+// thread's output pixels (tile rows 2 ty + h, column tx).  Every sum adds its 11 terms in tap order.
+constexpr int kGroup = 4;                     // horizontal pass: adjacent outputs per thread
+constexpr int kGroupsPerRow = kTX / kGroup;
 template <int NQ, typename In>
 __device__ __forceinline__ void separable(const Taps& taps, In in, double (*s_h)[kHY][kTX], int tx, int ty, double (&out)[NQ][2]) {
-  for (int e = threadIdx.x; e < kHY * kTX; e += kLossThreads) {
-    const int r = e / kTX, c = e - r * kTX;
-    double acc[NQ];
+  if (threadIdx.x < kHY * kGroupsPerRow) {
+    const int r = threadIdx.x / kGroupsPerRow, c0 = kGroup * (threadIdx.x - r * kGroupsPerRow);
+    double acc[kGroup][NQ];
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
+    for (int o = 0; o < kGroup; ++o)
 #pragma unroll
-    for (int j = 0; j <= 2 * kR; ++j) {
+      for (int q = 0; q < NQ; ++q) acc[o][q] = 0.0;
+#pragma unroll
+    for (int j = 0; j < kGroup + 2 * kR; ++j) {
       double v[NQ];
-      in(r, c + j, v);
+      in(r, c0 + j, v);
 #pragma unroll
-      for (int q = 0; q < NQ; ++q) acc[q] += taps.g[j] * v[q];
+      for (int o = 0; o < kGroup; ++o) {
+        if (j - o >= 0 && j - o <= 2 * kR) {
+#pragma unroll
+          for (int q = 0; q < NQ; ++q) acc[o][q] += taps.g[j - o] * v[q];
+        }
+      }
     }
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) s_h[q][r][c] = acc[q];
+    for (int q = 0; q < NQ; ++q)
+#pragma unroll
+      for (int o = 0; o < kGroup; ++o) s_h[q][r][c0 + o] = acc[o][q];
   }
   __syncthreads();
 #pragma unroll
-  for (int q = 0; q < NQ; ++q)
+  for (int q = 0; q < NQ; ++q) {
+    double a0 = 0.0, a1 = 0.0;
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      double acc = 0.0;
-#pragma unroll
-      for (int i = 0; i <= 2 * kR; ++i) acc += taps.g[i] * s_h[q][ty + 8 * h + i][tx];
-      out[q][h] = acc;
+    for (int i = 0; i <= 2 * kR + 1; ++i) {
+      const double v = s_h[q][2 * ty + i][tx];
+      if (i <= 2 * kR) a0 += taps.g[i] * v;
+      if (i >= 1) a1 += taps.g[i - 1] * v;
     }
+    out[q][0] = a0;
+    out[q][1] = a1;
+  }
+}
+
+// the (kHY x kHX) halo of one channel of NI images -> shared memory (zero outside the image): a warp per row
+template <int NI>
+__device__ __forceinline__ void load_halo(int W, int H, int x0, int y0, const float* const (&src)[NI], float (*const (&dst)[NI])[kHX]) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int r = warp; r < kHY; r += kLossThreads / 32) {
+    const int gy = y0 + r;
+    const bool row_in = gy >= 0 && gy < H;
+    const size_t base = (size_t)gy * W;
+    for (int c = lane; c < kHX; c += 32) {
+      const int gx = x0 + c;
+      const bool ok = row_in && gx >= 0 && gx < W;
+#pragma unroll
+      for (int i = 0; i < NI; ++i) dst[i][r][c] = ok ? __ldg(src[i] + base + gx) : 0.f;
+    }
+  }
 }
 
 __global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, Taps taps, const float* __restrict__ image,
@@ -74,12 +108,10 @@ __global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, T
   const float* x = image + ch * HW;
   const float* y = target + ch * HW;
   const int x0 = blockIdx.x * kTX - kR, y0 = blockIdx.y * kTY - kR;
-  for (int e = threadIdx.x; e < kHY * kHX; e += kLossThreads) {
-    const int r = e / kHX, c = e - r * kHX;
-    const int gx = x0 + c, gy = y0 + r;
-    const bool in = gx >= 0 && gx < W && gy >= 0 && gy < H;
-    s_x[r][c] = in ? x[(size_t)gy * W + gx] : 0.f;
-    s_y[r][c] = in ? y[(size_t)gy * W + gx] : 0.f;
+  {
+    const float* const src[2] = {x, y};
+    float (*const dst[2])[kHX] = {s_x, s_y};
+    load_halo<2>(W, H, x0, y0, src, dst);
   }
   __syncthreads();
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
@@ -92,7 +124,7 @@ __global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, T
   const int gx = blockIdx.x * kTX + tx;
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
-    const int gy = blockIdx.y * kTY + ty + 8 * h;
+    const int gy = blockIdx.y * kTY + 2 * ty + h;
     if (gx >= W || gy >= H) continue;
     const double mx = f[0][h], my = f[1][h], exx = f[2][h], eyy = f[3][h], exy = f[4][h];
     const double a1 = 2.0 * mx * my + kC1, a2 = 2.0 * (exy - mx * my) + kC2;
@@ -104,7 +136,7 @@ __global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, T
     maps[(1 * 3 + ch) * HW + p] = (float)(-sv / b2);
     maps[(2 * 3 + ch) * HW + p] = (float)(2.0 * a1 * ib);
     sum_s += sv;
-    sum_l1 += fabs((double)s_x[ty + 8 * h + kR][tx + kR] - (double)s_y[ty + 8 * h + kR][tx + kR]);
+    sum_l1 += fabs((double)s_x[2 * ty + h + kR][tx + kR] - (double)s_y[2 * ty + h + kR][tx + kR]);
   }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) {
@@ -150,13 +182,10 @@ __global__ void __launch_bounds__(kLossThreads) loss_grad_kernel(int W, int H, T
   const int ch = blockIdx.z;
   const size_t HW = (size_t)W * H;
   const int x0 = blockIdx.x * kTX - kR, y0 = blockIdx.y * kTY - kR;
-  for (int e = threadIdx.x; e < kHY * kHX; e += kLossThreads) {
-    const int r = e / kHX, c = e - r * kHX;
-    const int gx = x0 + c, gy = y0 + r;
-    const bool in = gx >= 0 && gx < W && gy >= 0 && gy < H;
-    const size_t p = (size_t)gy * W + gx;
-#pragma unroll
-    for (int q = 0; q < 3; ++q) s_in[q][r][c] = in ? maps[(q * 3 + ch) * HW + p] : 0.f;
+  {
+    const float* const src[3] = {maps + (0 * 3 + ch) * HW, maps + (1 * 3 + ch) * HW, maps + (2 * 3 + ch) * HW};
+    float (*const dst[3])[kHX] = {s_in[0], s_in[1], s_in[2]};
+    load_halo<3>(W, H, x0, y0, src, dst);
   }
   __syncthreads();
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
@@ -169,7 +198,7 @@ __global__ void __launch_bounds__(kLossThreads) loss_grad_kernel(int W, int H, T
   const int gx = blockIdx.x * kTX + tx;
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
-    const int gy = blockIdx.y * kTY + ty + 8 * h;
+    const int gy = blockIdx.y * kTY + 2 * ty + h;
     if (gx >= W || gy >= H) continue;
     const size_t p = (size_t)gy * W + gx;
     const double xv = image[ch * HW + p], yv = target[ch * HW + p];

@@ -334,8 +334,11 @@ constexpr int kBwdThreads = 128;
 // there, compact, and keeps every lane of every live warp busy -- 10-20 % of the primitives are visible).  The
 // gradient arrays were zeroed by grad_zero_kernel (side stream, concurrently with the blend backward); rows of
 // culled primitives stay zero.
+#ifndef GS_PBWD_MINB
+#define GS_PBWD_MINB 3
+#endif
 template <bool VARIANT>
-__global__ void __launch_bounds__(kBwdThreads, 3) preprocess_backward_kernel(gabsplat_scene s, Camera c, const uint32_t* __restrict__ order,
+__global__ void __launch_bounds__(kBwdThreads, GS_PBWD_MINB) preprocess_backward_kernel(gabsplat_scene s, Camera c, const uint32_t* __restrict__ order,
                                                                          const uint32_t* __restrict__ n_vis,
                                                                          const uint8_t* __restrict__ rgb_clamped,
                                                                          float* grad2d, gabsplat_grads g) {
