@@ -109,8 +109,10 @@ typedef struct {
   uint32_t* tiles_touched; /* [N]     number of tiles in the primitive's rectangle                */
   int32_t* rect;           /* [N][4]  xmin,ymin,xmax,ymax in tiles, max exclusive                  */
   float* packed;           /* [N][gabsplat_packed_floats(K)]  gather record, 16-byte aligned       */
-  uint32_t* chunk_visible; /* [ceil(N / GABSPLAT_CHUNK)]  visible primitives per chunk of consecutive
-                              primitives (what the binning needs to compact them in index order)   */
+  uint32_t* chunk_visible; /* [3][ceil(N / GABSPLAT_CHUNK)]  per chunk of consecutive primitives: the number of
+                              visible ones (what the binning needs to compact them in index order), then the
+                              smallest and the largest bits(depth) among them (0xffffffff / 0 if none): the
+                              depth range the binning buckets its sort by                               */
 } gabsplat_projected;
 
 /* Number of floats per primitive in gabsplat_projected.packed (a multiple of 4). */

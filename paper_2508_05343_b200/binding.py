@@ -234,7 +234,7 @@ class Projected:
         self.tiles_touched = z((N,), torch.int32)  # uint32 on the device; torch has no uint32 arithmetic
         self.rect = z((N, 4), torch.int32)
         self.packed = z((N, lib().gabsplat_packed_floats(K)), torch.float32)
-        self.chunk_visible = z(((N + CHUNK - 1) // CHUNK + 1,), torch.int32)
+        self.chunk_visible = z((3 * ((N + CHUNK - 1) // CHUNK) + 1,), torch.int32)
 
     def struct(self) -> _Projected:
         p = _Projected()

@@ -216,13 +216,53 @@ void device_scan(const u32* in, const u32* idx, u32* out, u32 n, const u32* n_de
 // number of visible primitives of every chunk in chunk_visible): the visible primitives are compacted in
 // index order -- (bits(depth), index) pairs at [sum of the earlier chunks' counts, ...) -- so that the depth
 // passes sort n_vis pairs, not N.
+// The depth order is found by BUCKETS when the depths spread (they do in any real scene): the visible primitives
+// are binned by (bits(depth) - kmin) >> shift into at most kBuckets bins over the range [kmin, kmax] the projection
+// recorded per chunk; a bucket's pairs are gathered (in any order), and every pair finds its place inside its bucket
+// by counting the bucket's smaller (depth, index) pairs -- the lexicographic order IS the stable order, so no pass has
+// to preserve anything.  Three single-wave launches (histogram with the compaction, scatter, rank) replace the
+// compaction and four stable one-byte passes.  A bucket of more than kBucketLimit pairs (thousands of primitives at
+// one depth) would make the quadratic ranking slow: sort_flag is then set and the four radix passes, which are
+// always launched and otherwise return at once, sort the compacted pairs instead.
+constexpr u32 kBuckets = 8192;
+constexpr u32 kBucketLimit = 4096;
+
+struct DepthRange { u32 kmin, shift; };
+__device__ __forceinline__ u32 bucket_of(u32 key, const DepthRange& r) { return (key - r.kmin) >> r.shift; }
+
+// kmin / shift from the per-chunk ranges the projection left behind chunk_visible's counts (every CTA computes them itself)
+__device__ __forceinline__ DepthRange depth_range(const u32* __restrict__ chunk_visible, u32 nchunks) {
+  __shared__ u32 s_min[8], s_max[8];
+  u32 lo = 0xffffffffu, hi = 0u;
+  for (u32 c = threadIdx.x; c < nchunks; c += 256) {
+    lo = min(lo, __ldg(chunk_visible + nchunks + c));
+    hi = max(hi, __ldg(chunk_visible + 2 * nchunks + c));
+  }
+  lo = __reduce_min_sync(0xffffffffu, lo);
+  hi = __reduce_max_sync(0xffffffffu, hi);
+  if ((threadIdx.x & 31) == 0) { s_min[threadIdx.x >> 5] = lo; s_max[threadIdx.x >> 5] = hi; }
+  __syncthreads();
+#pragma unroll
+  for (int j = 0; j < 8; ++j) { lo = min(lo, s_min[j]); hi = max(hi, s_max[j]); }
+  __syncthreads();
+  DepthRange r;
+  r.kmin = lo;
+  const u32 span = hi >= lo ? hi - lo : 0u;
+  const int bits = 32 - __clz((int)span);           // span < 2^bits
+  r.shift = (u32)max(0, bits - 13);                 // (span >> shift) < kBuckets = 2^13
+  return r;
+}
+
 __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __restrict__ tiles_touched,
                                                          const float* __restrict__ depth, const u32* __restrict__ chunk_visible,
                                                          u32* __restrict__ keys, u32* __restrict__ vals, u32* __restrict__ n_vis,
-                                                         u32* __restrict__ table0) {
+                                                         u32* __restrict__ table0, u32* __restrict__ bucket_cnt,
+                                                         DepthRange* __restrict__ range_out) {
   pdl_wait();
   __shared__ u32 s_part[8], s_off;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const DepthRange rg = depth_range(chunk_visible, gridDim.x);
+  if (blockIdx.x == 0 && threadIdx.x == 0) *range_out = rg;
   u32 acc = 0;
   for (u32 c = threadIdx.x; c < blockIdx.x; c += 256) acc += __ldg(chunk_visible + c);
 #pragma unroll
@@ -254,11 +294,96 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __res
       const u32 key = __float_as_uint(depth[i]);
       keys[pos] = key;
       vals[pos] = (u32)i;
-      atomicAdd(&table0[(pos / kSmallTile) * 256u + (key & 255u)], 1u);  // histogram of the first pass, per sort tile
+      atomicAdd(&table0[(pos / kSmallTile) * 256u + (key & 255u)], 1u);  // histogram of the first radix pass, per sort tile
+      atomicAdd(&bucket_cnt[bucket_of(key, rg)], 1u);
     }
     run += total;
   }
   if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *n_vis = run;
+}
+
+// Gathers the compacted pairs by bucket: a CTA per kScatterTile pairs.  Every CTA scans the bucket counts itself (32
+// per thread); CTA 0 leaves the bucket starts and the path decision for the kernels that follow.
+constexpr int kScatterItems = 4;
+constexpr int kScatterTile = 256 * kScatterItems;
+__global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restrict__ kin, const u32* __restrict__ vin,
+                                                             u32* __restrict__ kout, u32* __restrict__ vout,
+                                                             const u32* __restrict__ n_vis_p, const u32* __restrict__ bucket_cnt,
+                                                             u32* __restrict__ bucket_cur, u32* __restrict__ bucket_base,
+                                                             u32* __restrict__ sort_flag, const DepthRange* __restrict__ range) {
+  pdl_wait();
+  __shared__ u32 s_base[kBuckets];
+  __shared__ u32 s_big;
+  const u32 n = *n_vis_p;
+  const u32 start = blockIdx.x * kScatterTile;
+  if (start >= n && blockIdx.x != 0) return;
+  const DepthRange rg = *range;
+  if (threadIdx.x == 0) s_big = 0;
+  // this thread's pairs and their buckets first: the loads are in flight while the counts are scanned
+  u32 key[kScatterItems], val[kScatterItems];
+#pragma unroll
+  for (int i = 0; i < kScatterItems; ++i) {
+    const u32 j = start + (u32)i * 256u + threadIdx.x;
+    key[i] = j < n ? __ldg(kin + j) : 0u;
+    val[i] = j < n ? __ldg(vin + j) : 0u;
+  }
+  constexpr int PER = kBuckets / 256;
+  u32 c[PER], sum = 0, mx = 0;
+#pragma unroll
+  for (int j = 0; j < PER; j += 4) {
+    const uint4 v = __ldg(reinterpret_cast<const uint4*>(bucket_cnt + threadIdx.x * PER + j));
+    c[j] = v.x; c[j + 1] = v.y; c[j + 2] = v.z; c[j + 3] = v.w;
+  }
+#pragma unroll
+  for (int j = 0; j < PER; ++j) { sum += c[j]; mx = max(mx, c[j]); }
+  u32 total;
+  u32 run = block_exclusive_scan(sum, &total);
+#pragma unroll
+  for (int j = 0; j < PER; ++j) { s_base[threadIdx.x * PER + j] = run; run += c[j]; }
+  if (mx > kBucketLimit) atomicOr(&s_big, 1u);
+  __syncthreads();
+  if (blockIdx.x == 0) {
+#pragma unroll
+    for (int j = 0; j < PER; ++j) bucket_base[threadIdx.x * PER + j] = s_base[threadIdx.x * PER + j];
+    if (threadIdx.x == 0) *sort_flag = s_big;
+  }
+  if (s_big) return;  // the radix passes sort the compacted pairs instead
+  u32 pos[kScatterItems];
+#pragma unroll
+  for (int i = 0; i < kScatterItems; ++i) {
+    const u32 j = start + (u32)i * 256u + threadIdx.x;
+    const u32 b = bucket_of(key[i], rg);
+    pos[i] = j < n ? s_base[b] + atomicAdd(&bucket_cur[b], 1u) : 0u;
+  }
+#pragma unroll
+  for (int i = 0; i < kScatterItems; ++i) {
+    const u32 j = start + (u32)i * 256u + threadIdx.x;
+    if (j < n) { kout[pos[i]] = key[i]; vout[pos[i]] = val[i]; }
+  }
+}
+
+// place of every pair inside its bucket = the number of the bucket's pairs that are smaller by (depth bits, index)
+__global__ void __launch_bounds__(256) bucket_rank_kernel(const u32* __restrict__ kin, const u32* __restrict__ vin,
+                                                          u32* __restrict__ kout, u32* __restrict__ vout,
+                                                          const u32* __restrict__ n_vis_p, const u32* __restrict__ bucket_cnt,
+                                                          const u32* __restrict__ bucket_base, const u32* __restrict__ sort_flag,
+                                                          const DepthRange* __restrict__ range) {
+  pdl_wait();
+  if (*sort_flag) return;
+  const u32 p = blockIdx.x * 256u + threadIdx.x;
+  if (p >= *n_vis_p) return;
+  const DepthRange rg = *range;
+  const u32 key = kin[p], val = vin[p];
+  const u32 b = bucket_of(key, rg);
+  const u32 lo = __ldg(bucket_base + b), cnt = __ldg(bucket_cnt + b);
+  u32 rank = 0;
+#pragma unroll 8
+  for (u32 q = lo; q < lo + cnt; ++q) {
+    const u32 kq = __ldg(kin + q), vq = __ldg(vin + q);
+    rank += (kq < key || (kq == key && vq < val)) ? 1u : 0u;
+  }
+  kout[lo + rank] = key;
+  vout[lo + rank] = val;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -391,8 +516,10 @@ __global__ void __launch_bounds__(kSortThreads) sort_scatter(const u32* __restri
                                                             u32* __restrict__ kout, u32* __restrict__ vout,
                                                             u64* __restrict__ kout64, const u32* __restrict__ gather,
                                                             const u32* __restrict__ count, const u32* __restrict__ table,
-                                                            u32 nblocks, int shift, u32* __restrict__ table_next) {
+                                                            u32 nblocks, int shift, u32* __restrict__ table_next,
+                                                            const u32* __restrict__ run_flag) {
   pdl_wait();
+  if (run_flag && *run_flag == 0) return;  // the bucketed depth sort has done the work (see depth_keys_kernel)
   __shared__ u32 warp_hist[kSortWarps][256];
   __shared__ u32 local_base[256];
   __shared__ u32 global_base[256];
@@ -906,6 +1033,11 @@ struct Workspace {
   u32* count_b;     // [1] = D, or 0 when D > capacity
   u32* table;       // [256][nblocks]
   u32* dtable[4];   // per depth pass: [sort_blocks(N)][256] histograms of that pass's input arrangement
+  u32* bucket_cnt;  // [kBuckets] pairs per depth bucket          } zeroed together with dtable
+  u32* bucket_cur;  // [kBuckets] fill cursors of the buckets      }
+  u32* sort_flag;   // [1] 1: a bucket is too large, the radix passes sort instead
+  u32* bucket_base; // [kBuckets] first slot of every bucket
+  DepthRange* range;  // bucket mapping of this call
   u32* pk[2];       // stage A key ping-pong [N]
   u32* pv[2];       // stage A value ping-pong [N]; pv[0] ends up holding the depth order
   u32* ik;          // stage B (radix path) alternate keys [capacity]
@@ -934,9 +1066,14 @@ Workspace carve(void* base, int N, u64 capacity, int ntiles) {
   w.table = (u32*)take(table_n * 4);
   {  // contiguous, zeroed by one memset per call
     const u64 one = (u64)256 * (((u64)N + kSmallTile - 1) / kSmallTile + 1);
-    u32* base4 = (u32*)take(4 * one * 4);
+    u32* base4 = (u32*)take((4 * one + 2 * kBuckets + 64) * 4);
     for (int i = 0; i < 4; ++i) w.dtable[i] = base4 + i * one;
+    w.bucket_cnt = base4 + 4 * one;
+    w.bucket_cur = w.bucket_cnt + kBuckets;
+    w.sort_flag = w.bucket_cur + kBuckets;
   }
+  w.bucket_base = (u32*)take((u64)kBuckets * 4);
+  w.range = (DepthRange*)take(sizeof(DepthRange));
   for (int i = 0; i < 2; ++i) { w.pk[i] = (u32*)take((u64)N * 4); w.pv[i] = (u32*)take((u64)N * 4); }
   w.n_vis = (u32*)take(16);
   w.bounds = (u32*)take((kChunks + 1) * 4);
@@ -961,18 +1098,18 @@ void radix_pass(const u32* kin, const u32* vin, u32* kout, u32* vout, u64* kout6
   launched();
   device_scan<false, false>(ws.table, nullptr, ws.table, 256u * nblocks, nullptr, 0u, ws.scan_sums, nullptr, st);
   if (kout64)
-    launch_pdl(sort_scatter<true, false>, nblocks, kSortThreads, 0, st, kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, (u32*)nullptr);
+    launch_pdl(sort_scatter<true, false>, nblocks, kSortThreads, 0, st, kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, (u32*)nullptr, (const u32*)nullptr);
   else
-    launch_pdl(sort_scatter<false, false>, nblocks, kSortThreads, 0, st, kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, (u32*)nullptr);
+    launch_pdl(sort_scatter<false, false>, nblocks, kSortThreads, 0, st, kin, vin, kout, vout, kout64, gather, count, ws.table, nblocks, shift, (u32*)nullptr, (const u32*)nullptr);
   launched();
 }
 
 // a pass over the visible primitives: ONE launch -- its per-tile histogram was accumulated by the producer of its
 // input (depth_keys_kernel for the first pass, the previous pass's scatter for the others)
 void radix_pass_small(const u32* kin, const u32* vin, u32* kout, u32* vout, const u32* count, u32 nblocks, int shift,
-                      const u32* table, u32* table_next, cudaStream_t st) {
+                      const u32* table, u32* table_next, const u32* run_flag, cudaStream_t st) {
   launch_pdl(sort_scatter<false, true, kSmallItems>, nblocks, kSortThreads, 0, st, kin, vin, kout, vout, (u64*)nullptr,
-             (const u32*)nullptr, count, table, nblocks, shift, table_next);
+             (const u32*)nullptr, count, table, nblocks, shift, table_next, run_flag);
   launched();
 }
 
@@ -1015,13 +1152,20 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   // A: depth order of the primitives (digits 0-3 of the 64-bit key)
   tm.begin(GABSPLAT_STAGE_DEPTH_SORT, st);
   const u32 nba = (u32)(((u64)N + kSmallTile - 1) / kSmallTile);
-  cudaMemsetAsync(ws.dtable[0], 0, (size_t)4 * 256 * (nba + 1) * sizeof(u32), st);
-  launch_pdl(depth_keys_kernel, (N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK, 256, 0, st, N, proj.tiles_touched, proj.depth,
-             proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis, ws.dtable[0]);
-  launched();
+  cudaMemsetAsync(ws.dtable[0], 0, ((size_t)4 * 256 * (nba + 1) + 2 * kBuckets + 64) * sizeof(u32), st);
+  const u32 nchunks = (u32)((N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK);
+  launch_pdl(depth_keys_kernel, nchunks, 256, 0, st, N, proj.tiles_touched, proj.depth,
+             proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis, ws.dtable[0], ws.bucket_cnt, ws.range);
+  // bucketed order: pairs gathered by bucket into pk[1] / pv[1], ranked inside their buckets back into pk[0] / pv[0]
+  launch_pdl(bucket_scatter_kernel, (u32)((N + kScatterTile - 1) / kScatterTile), 256, 0, st, ws.pk[0], ws.pv[0], ws.pk[1], ws.pv[1],
+             ws.n_vis, ws.bucket_cnt, ws.bucket_cur, ws.bucket_base, ws.sort_flag, (const DepthRange*)ws.range);
+  launch_pdl(bucket_rank_kernel, (u32)((N + 255) / 256), 256, 0, st, ws.pk[1], ws.pv[1], ws.pk[0], ws.pv[0], ws.n_vis,
+             ws.bucket_cnt, ws.bucket_base, ws.sort_flag, ws.range);
+  launched(3);
+  // ... unless a bucket is too large: then these four stable one-byte passes run (otherwise they return at once)
   for (int p = 0; p < 4; ++p)
     radix_pass_small(ws.pk[p & 1], ws.pv[p & 1], ws.pk[(p & 1) ^ 1], ws.pv[(p & 1) ^ 1], ws.n_vis, nba, 8 * p, ws.dtable[p],
-                     p < 3 ? ws.dtable[p + 1] : nullptr, st);
+                     p < 3 ? ws.dtable[p + 1] : nullptr, ws.sort_flag, st);
   const u32* order = ws.pv[0];
   tm.end(st);
   // K2 (over the n_vis ranks)

@@ -287,10 +287,12 @@ constexpr int kPreChunk = GABSPLAT_CHUNK;
 __global__ void __launch_bounds__(kPreThreads) index_kernel(gabsplat_scene s, Camera c, gabsplat_projected out) {
   pdl_wait();
   __shared__ int s_n;
-  if (threadIdx.x == 0) s_n = 0;
+  __shared__ uint32_t s_kmin, s_kmax;
+  if (threadIdx.x == 0) { s_n = 0; s_kmin = 0xffffffffu; s_kmax = 0u; }
   __syncthreads();
   const int base = blockIdx.x * kPreChunk;
   int mine = 0;
+  uint32_t kmin = 0xffffffffu, kmax = 0u;  // bits(depth) of the visible primitives: what the binning sorts by
 #pragma unroll 1
   for (int r = 0; r < kPreChunk / kPreThreads; ++r) {
     const int i = base + r * kPreThreads + threadIdx.x;
@@ -310,6 +312,8 @@ __global__ void __launch_bounds__(kPreThreads) index_kernel(gabsplat_scene s, Ca
       radius = ix.radius;
       if (ix.visible) {
         ++mine;
+        kmin = min(kmin, __float_as_uint(ix.depth));
+        kmax = max(kmax, __float_as_uint(ix.depth));
         reinterpret_cast<float2*>(out.mean2d)[i] = make_float2(ix.m2x, ix.m2y);
         out.depth[i] = ix.depth;
         reinterpret_cast<int4*>(out.rect)[i] = make_int4(ix.x0, ix.y0, ix.x1, ix.y1);
@@ -320,9 +324,15 @@ __global__ void __launch_bounds__(kPreThreads) index_kernel(gabsplat_scene s, Ca
   }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, d);
-  if ((threadIdx.x & 31) == 0 && mine) atomicAdd(&s_n, mine);
+  kmin = __reduce_min_sync(0xffffffffu, kmin);
+  kmax = __reduce_max_sync(0xffffffffu, kmax);
+  if ((threadIdx.x & 31) == 0 && mine) { atomicAdd(&s_n, mine); atomicMin(&s_kmin, kmin); atomicMax(&s_kmax, kmax); }
   __syncthreads();
-  if (threadIdx.x == 0) out.chunk_visible[blockIdx.x] = (uint32_t)s_n;
+  if (threadIdx.x == 0) {
+    out.chunk_visible[blockIdx.x] = (uint32_t)s_n;
+    out.chunk_visible[gridDim.x + blockIdx.x] = s_kmin;
+    out.chunk_visible[2 * gridDim.x + blockIdx.x] = s_kmax;
+  }
 }
 
 constexpr int kValThreads = 128;

@@ -207,3 +207,24 @@ def test_fused_preprocess_bin_sort_equals_the_two_calls():
     assert torch.equal(b1.ids[:b1.D], b2.ids[:b1.D]) and torch.equal(b1.tile_ranges, b2.tile_ranges)
     assert torch.equal(b1.keys[:b1.D], b2.keys[:b1.D])
     assert torch.equal(f1.image, f2.image)
+
+
+@pytest.mark.parametrize("levels", [1, 3, 6000])
+def test_depth_sort_paths(levels):
+    """The depth order of the visible primitives comes from the bucketed sort when the depths spread and from the
+    stable radix passes when a bucket overflows (thousands of primitives at one depth): 6000 primitives on `levels`
+    planes facing the camera -- one plane: every key equal, the order is the index order and the radix passes run;
+    three planes: three huge buckets (radix passes); 6000 levels: the bucketed path.  Lists bit-exact either way."""
+    from oracle import gabsplat_oracle as orc
+    from gpu_helpers import run_gpu
+    scene = scenes.make_scene("tiny", N=6000)
+    z = -0.9 + 1.8 * (np.arange(6000) % levels) / max(levels, 1)
+    scene.means[:, 2] = z.astype(np.float32)          # the tiny camera looks down +z: depth = z + 4 exactly
+    cam = scenes.make_cameras("tiny")[0]
+    g, _ = run_gpu(scene, cam)
+    o = orc.bin_sort(scene, cam)
+    if levels == 1:
+        assert len(np.unique(g["depth_bits"][g["tiles_touched"] != 0])) == 1
+    assert g["D"] == o["num_instances"]
+    assert np.array_equal(g["keys"], o["keys"]) and np.array_equal(g["ids"], o["ids"])
+    assert np.array_equal(g["tile_ranges"], o["tile_ranges"])
