@@ -894,7 +894,13 @@ __global__ void __launch_bounds__(1024) tile_ranges_scan_kernel(int ntiles, cons
   block_order_descending([&](u32 t) -> u32 { return fits ? totals[t] : 0u; }, (u32)ntiles, order);
 }
 
-constexpr int kFlat = 8;  // instances a thread keeps in registers during a step
+// Instances a thread keeps in registers during a step.  Measured (config 3 / 4 / 2 placement, ms): 8: 0.101 / 0.487 /
+// 0.064; 4: 0.093 / 0.457; 2: 0.089 / 0.444 / 0.051; 1: 0.088 / 0.437 / 0.050 -- a shared step of 32 primitives rarely
+// fills more than one instance per thread, and a primitive of more than kFlat * THREADS tiles takes the direct path.
+#ifndef GS_FLAT
+#define GS_FLAT 1
+#endif
+constexpr int kFlat = GS_FLAT;
 
 __device__ __forceinline__ u32 rect_tiles(const uint4& rc) {
   return ((rc.w & 0xffffu) - (rc.z & 0xffffu)) * ((rc.w >> 16) - (rc.z >> 16));
