@@ -34,8 +34,11 @@ constexpr int kFwdBatch = GS_FWD_BATCH;              // list entries filtered pe
 constexpr int kFwdPer = kFwdBatch / kBlendThreads;   // ... per thread
 #endif
 
+#ifndef GS_FWD_MINB
+#define GS_FWD_MINB 10
+#endif
 template <int K, bool COUNT, bool SAVE>
-__global__ void __launch_bounds__(kBlendThreads) blend_forward_kernel(Camera cam, const uint32_t* __restrict__ order,
+__global__ void __launch_bounds__(kBlendThreads, GS_FWD_MINB) blend_forward_kernel(Camera cam, const uint32_t* __restrict__ order,
                                                                       const uint2* __restrict__ ranges,
                                                                       const uint32_t* __restrict__ ids,
                                                                       const float4* __restrict__ packed,
