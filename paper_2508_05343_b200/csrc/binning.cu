@@ -222,10 +222,12 @@ void device_scan(const u32* in, const u32* idx, u32* out, u32 n, const u32* n_de
 // by counting the bucket's smaller (depth, index) pairs -- the lexicographic order IS the stable order, so no pass has
 // to preserve anything.  Three single-wave launches (histogram with the compaction, scatter, rank) replace the
 // compaction and four stable one-byte passes.  A bucket of more than kBucketLimit pairs (thousands of primitives at
-// one depth) would make the quadratic ranking slow: sort_flag is then set and the four radix passes, which are
-// always launched and otherwise return at once, sort the compacted pairs instead.
+// one depth), or buckets so uneven that the ranking would cost more than kRankBudget comparisons per pair, would make
+// the quadratic ranking slow: sort_flag is then set and the four radix passes, which are always launched and
+// otherwise return at once, sort the compacted pairs instead.
 constexpr u32 kBuckets = 8192;
 constexpr u32 kBucketLimit = 4096;
+constexpr u32 kRankBudget = 256;   // comparisons per pair, on average, the quadratic ranking may cost
 
 struct DepthRange { u32 kmin, shift; };
 __device__ __forceinline__ u32 bucket_of(u32 key, const DepthRange& r) { return (key - r.kmin) >> r.shift; }
@@ -314,11 +316,13 @@ __global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restri
   pdl_wait();
   __shared__ u32 s_base[kBuckets];
   __shared__ u32 s_big;
+  __shared__ unsigned long long s_sq;
   const u32 n = *n_vis_p;
   const u32 start = blockIdx.x * kScatterTile;
   if (start >= n && blockIdx.x != 0) return;
   const DepthRange rg = *range;
-  if (threadIdx.x == 0) s_big = 0;
+  if (threadIdx.x == 0) { s_big = 0; s_sq = 0; }
+  __syncthreads();
   // this thread's pairs and their buckets first: the loads are in flight while the counts are scanned
   u32 key[kScatterItems], val[kScatterItems];
 #pragma unroll
@@ -329,18 +333,25 @@ __global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restri
   }
   constexpr int PER = kBuckets / 256;
   u32 c[PER], sum = 0, mx = 0;
+  unsigned long long sq = 0;  // the ranking work: sum of the squared bucket sizes
 #pragma unroll
   for (int j = 0; j < PER; j += 4) {
     const uint4 v = __ldg(reinterpret_cast<const uint4*>(bucket_cnt + threadIdx.x * PER + j));
     c[j] = v.x; c[j + 1] = v.y; c[j + 2] = v.z; c[j + 3] = v.w;
   }
 #pragma unroll
-  for (int j = 0; j < PER; ++j) { sum += c[j]; mx = max(mx, c[j]); }
+  for (int j = 0; j < PER; ++j) { sum += c[j]; mx = max(mx, c[j]); sq += (unsigned long long)c[j] * c[j]; }
   u32 total;
   u32 run = block_exclusive_scan(sum, &total);
 #pragma unroll
   for (int j = 0; j < PER; ++j) { s_base[threadIdx.x * PER + j] = run; run += c[j]; }
+  // one huge bucket, or many large ones (more than kRankBudget comparisons per pair on average): the radix passes
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, d);
+  if ((threadIdx.x & 31) == 0) atomicAdd(&s_sq, sq);
   if (mx > kBucketLimit) atomicOr(&s_big, 1u);
+  __syncthreads();
+  if (threadIdx.x == 0 && s_sq > (unsigned long long)kRankBudget * n) s_big = 1u;
   __syncthreads();
   if (blockIdx.x == 0) {
 #pragma unroll

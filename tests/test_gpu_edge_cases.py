@@ -209,12 +209,13 @@ def test_fused_preprocess_bin_sort_equals_the_two_calls():
     assert torch.equal(f1.image, f2.image)
 
 
-@pytest.mark.parametrize("levels", [1, 3, 6000])
+@pytest.mark.parametrize("levels", [1, 3, 60, 6000])
 def test_depth_sort_paths(levels):
     """The depth order of the visible primitives comes from the bucketed sort when the depths spread and from the
     stable radix passes when a bucket overflows (thousands of primitives at one depth): 6000 primitives on `levels`
     planes facing the camera -- one plane: every key equal, the order is the index order and the radix passes run;
-    three planes: three huge buckets (radix passes); 6000 levels: the bucketed path.  Lists bit-exact either way."""
+    three planes: three huge buckets (radix passes); 60 planes: the bucketed path with 100-way ties inside a bucket;
+    6000 levels: the bucketed path.  Lists bit-exact either way."""
     from oracle import gabsplat_oracle as orc
     from gpu_helpers import run_gpu
     scene = scenes.make_scene("tiny", N=6000)
