@@ -724,11 +724,11 @@ __global__ void clamp_count_kernel(u32* sort_count, u32* num_instances, const un
 // B': the tile digit in ONE stable counting-sort pass.  The depth-ordered primitive sequence is cut into
 // kChunks chunks of equal estimated cost; because a primitive covers a tile at most once, the per-(chunk, tile)
 // histogram is simply the number of the chunk's primitives whose rectangle contains the tile:
-//   tile_count_kernel   table[tile][chunk] = that number                       (shared-memory histogram per CTA)
-//   tile_scan_kernel    table[tile][.] -> exclusive prefix over the chunks; totals[tile]
+//   tile_count_kernel   table[chunk][tile] = that number                       (shared-memory histogram per CTA)
+//   tile_scan_kernel    table[.][tile] -> exclusive prefix over the chunks; totals[tile]
 //   tile_ranges_scan    exclusive prefix of the totals over the tiles -> tile_ranges (+ launch order of the blend)
 //   tile_place_kernel   every CTA re-walks its chunk in depth order, kStep primitives at a time, and writes
-//                       (tile | depth, id) at  ranges[tile].x + table[tile][chunk] + (rank inside the chunk)
+//                       (tile | depth, id) at  ranges[tile].x + table[chunk][tile] + (rank inside the chunk)
 // The rank inside a step is the number of lower-ranked primitives of the step that cover the same tile: the
 // step's primitives OR their bit into mask[tile] (shared memory), then every instance counts the bits below
 // its own.  Result: exactly the order of a stable sort by tile of the depth-ordered instance sequence, i.e.
@@ -807,7 +807,7 @@ __device__ __forceinline__ void for_rect_tiles(u32 xy0, u32 xy1, int tiles_x, in
   }
 }
 
-// table[tile][chunk] = number of the chunk's primitives whose rectangle contains the tile, by a 2D difference
+// table[chunk][tile] = number of the chunk's primitives whose rectangle contains the tile, by a 2D difference
 // array in shared memory: four corner updates per primitive, then prefix sums along x and along y.
 __global__ void __launch_bounds__(kPlaceThreads) tile_count_kernel(int tiles_x, int tiles_y, const uint4* __restrict__ recs,
                                                                    const u32* __restrict__ bounds, u32* __restrict__ table) {
@@ -836,28 +836,39 @@ __global__ void __launch_bounds__(kPlaceThreads) tile_count_kernel(int tiles_x, 
     for (int y = 0; y < sy; ++y) { run += s_d[y * sx + x]; s_d[y * sx + x] = run; }
   }
   __syncthreads();
-  for (int t = threadIdx.x; t < tiles_x * tiles_y; t += kPlaceThreads) {
+  const int ntiles = tiles_x * tiles_y;
+  for (int t = threadIdx.x; t < ntiles; t += kPlaceThreads) {
     const int y = t / tiles_x, x = t - y * tiles_x;
-    table[(size_t)t * kChunks + blockIdx.x] = (u32)s_d[y * sx + x];
+    table[(size_t)blockIdx.x * ntiles + t] = (u32)s_d[y * sx + x];   // chunk-major: a coalesced row per CTA
   }
 }
 
-// a warp per tile: exclusive prefix of table[tile][0..kChunks) in place, total to totals[tile]
-__global__ void __launch_bounds__(256) tile_scan_kernel(int ntiles, u32* __restrict__ table, u32* __restrict__ totals) {
+// Exclusive prefix over the chunks of table[chunk][tile], in place, and the total of every tile.  A CTA takes 32
+// consecutive tiles (one coalesced 128-byte row segment per chunk) and cuts the chunks into kScanSegs segments, a warp
+// each: segment sums first, then the prefixes with the earlier segments' sums added.
+constexpr int kScanSegs = 16;
+static_assert(kChunks % kScanSegs == 0, "the chunk count must split evenly into scan segments");
+__global__ void __launch_bounds__(32 * kScanSegs) tile_scan_kernel(int ntiles, u32* __restrict__ table, u32* __restrict__ totals) {
   pdl_wait();
-  const int lane = threadIdx.x & 31;
-  const int t = blockIdx.x * 8 + (threadIdx.x >> 5);
-  if (t >= ntiles) return;
-  u32* row = table + (size_t)t * kChunks;
-  u32 carry = 0;
-  for (int c0 = 0; c0 < kChunks; c0 += 32) {
-    const int c = c0 + lane;
-    const u32 v = c < kChunks ? row[c] : 0u;
-    const u32 inc = warp_inclusive_scan(v, lane);
-    if (c < kChunks) row[c] = carry + inc - v;
-    carry += __shfl_sync(0xffffffffu, inc, 31);
+  constexpr int PER = kChunks / kScanSegs;
+  __shared__ u32 s_sum[kScanSegs][32];
+  const int lane = threadIdx.x & 31, seg = threadIdx.x >> 5;
+  const int t = blockIdx.x * 32 + lane;
+  const bool live = t < ntiles;
+  u32* col = table + (size_t)seg * PER * ntiles + t;
+  u32 v[PER], sum = 0;
+#pragma unroll
+  for (int i = 0; i < PER; ++i) { v[i] = live ? col[(size_t)i * ntiles] : 0u; sum += v[i]; }
+  s_sum[seg][lane] = sum;
+  __syncthreads();
+  u32 run = 0, all = 0;
+#pragma unroll
+  for (int j = 0; j < kScanSegs; ++j) { const u32 x = s_sum[j][lane]; run += j < seg ? x : 0u; all += x; }
+  if (live) {
+#pragma unroll
+    for (int i = 0; i < PER; ++i) { col[(size_t)i * ntiles] = run; run += v[i]; }
+    if (seg == 0) totals[t] = all;
   }
-  if (lane == 0) totals[t] = carry;
 }
 
 // one CTA: tile_ranges[t] = [start, start + totals[t]) by an exclusive prefix over the tiles ((0,0) for an empty
@@ -948,7 +959,7 @@ __global__ void __launch_bounds__(THREADS, THREADS == 1024 ? 2 : 4) tile_place_k
   __shared__ int s_m[2];               // primitives in the step
   if ((u64)*num_instances > capacity) return;
   for (u32 t = threadIdx.x; t < nband; t += THREADS) {
-    s_pos[t] = ranges[tile0 + t].x + table[(size_t)(tile0 + t) * kChunks + blockIdx.x];
+    s_pos[t] = ranges[tile0 + t].x + table[(size_t)blockIdx.x * ntiles + tile0 + t];
     s_mask[t] = 0;
   }
   const u32 b0 = bounds[blockIdx.x], b1 = bounds[blockIdx.x + 1];
@@ -1063,7 +1074,7 @@ struct Workspace {
   u32* bounds;      // [kChunks + 1] chunk boundaries (ranks in depth order)
   u32* totals;      // [ntiles] instances per tile
   uint4* recs;      // [N] records of the visible primitives in depth order
-  u32* chunk_table; // [ntiles][kChunks] per-(tile, chunk) counts, then exclusive prefixes over the chunks
+  u32* chunk_table; // [kChunks][ntiles] per-(chunk, tile) counts, then exclusive prefixes over the chunks
   u64 bytes;
 };
 
@@ -1212,7 +1223,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
     launched(2);
     tm.end(st);
     tm.begin(GABSPLAT_STAGE_RANGES, st);
-    launch_pdl(tile_scan_kernel, (ntiles + 7) / 8, 256, 0, st, ntiles, ws.chunk_table, ws.totals);
+    launch_pdl(tile_scan_kernel, (ntiles + 31) / 32, 32 * kScanSegs, 0, st, ntiles, ws.chunk_table, ws.totals);
     launch_pdl(tile_ranges_scan_kernel, 1, 1024, 0, st, ntiles, ws.totals, bin.num_instances, bin.capacity, ranges, bin.tile_order);
     launched(2);
     tm.end(st);
