@@ -877,41 +877,45 @@ __global__ void __launch_bounds__(1024) tile_ranges_scan_kernel(int ntiles, cons
                                                                u32* __restrict__ num_instances, u64 capacity,
                                                                uint2* __restrict__ ranges, u32* __restrict__ order) {
   pdl_wait();
-  __shared__ u32 s_warp[32], s_carry;
+  // every thread owns a run of consecutive tiles: one block-wide scan of the run sums (64-bit: D may exceed what the
+  // 32-bit positions can address), then the starts inside the run
+  __shared__ unsigned long long s_warp[32];
   __shared__ unsigned long long s_total;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  if (threadIdx.x == 0) { s_carry = 0; s_total = 0; }
-  __syncthreads();
-  {  // D = the number of instances (64-bit: it may exceed what the 32-bit positions can address)
-    unsigned long long acc = 0;
-    for (int t = threadIdx.x; t < ntiles; t += 1024) acc += totals[t];
+  const int per = (ntiles + 1023) / 1024;
+  const int t0 = min(ntiles, (int)threadIdx.x * per), t1 = min(ntiles, t0 + per);
+  unsigned long long sum = 0;
+  for (int t = t0; t < t1; ++t) sum += totals[t];
+  unsigned long long inc = sum;
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
-    if (lane == 0 && acc) atomicAdd(&s_total, acc);
+  for (int d = 1; d < 32; d <<= 1) {
+    const unsigned long long o = __shfl_up_sync(0xffffffffu, inc, d);
+    if (lane >= d) inc += o;
+  }
+  if (lane == 31) s_warp[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    const unsigned long long x = s_warp[lane];
+    unsigned long long xi = x;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const unsigned long long o = __shfl_up_sync(0xffffffffu, xi, d);
+      if (lane >= d) xi += o;
+    }
+    s_warp[lane] = xi - x;
+    if (lane == 31) s_total = xi;
   }
   __syncthreads();
   const unsigned long long D = s_total;
   const bool fits = D <= capacity && D <= 0xffffffffull;
   if (threadIdx.x == 0) *num_instances = (u32)min(D, 0xffffffffull);
-  __syncthreads();
-  for (int base = 0; base < ntiles; base += 1024) {
-    const int t = base + threadIdx.x;
-    const u32 v = t < ntiles ? totals[t] : 0u;
-    const u32 inc = warp_inclusive_scan(v, lane);
-    if (lane == 31) s_warp[w] = inc;
-    __syncthreads();
-    if (w == 0) {
-      const u32 x = s_warp[lane];
-      const u32 xi = warp_inclusive_scan(x, lane);
-      s_warp[lane] = xi - x;
-    }
-    __syncthreads();
-    const u32 start = s_carry + s_warp[w] + inc - v;
-    if (t < ntiles) ranges[t] = (fits && v) ? make_uint2(start, start + v) : make_uint2(0u, 0u);
-    __syncthreads();
-    if (threadIdx.x == 1023) s_carry = start + v;
-    __syncthreads();
+  u32 start = (u32)(s_warp[w] + inc - sum);
+  for (int t = t0; t < t1; ++t) {
+    const u32 v = totals[t];
+    ranges[t] = (fits && v) ? make_uint2(start, start + v) : make_uint2(0u, 0u);
+    start += v;
   }
+  __syncthreads();
   // launch order of the forward blend: tiles by descending list length
   block_order_descending([&](u32 t) -> u32 { return fits ? totals[t] : 0u; }, (u32)ntiles, order);
 }
