@@ -4,7 +4,8 @@
 // (reading C25).  It produces dL/dimage, the input of gabsplat_render_backward, without leaving the GPU.
 //
 // Two tiled passes, both HBM bound (26 MB in + 39 MB out, then 65 MB in + 13 MB out at 1297x840):
-//   ssim_maps_kernel   per 32x16 tile of one channel: the five windowed sums w*x, w*y, w*x^2, w*y^2, w*xy as a
+//   ssim_maps_kernel   per 32x16 tile of one channel: the four windowed sums w*x, w*y, w*(x^2 + y^2), w*xy (SSIM needs
+//                      the two second moments only through their sum) as a
 //                      separable 11-tap filter through shared memory, SSIM and its three partial derivatives
 //                      (dS/dmx, dS/dExx, dS/dExy) per pixel, per-CTA partial sums of |x - y| and SSIM
 //   loss_grad_kernel   the same separable filter over the three derivative maps, combined with x, y and sign(x - y)
@@ -97,11 +98,11 @@ __device__ __forceinline__ void load_halo(int W, int H, int x0, int y0, const fl
   }
 }
 
-__global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, Taps taps, const float* __restrict__ image,
+__global__ void __launch_bounds__(kLossThreads, 4) ssim_maps_kernel(int W, int H, Taps taps, const float* __restrict__ image,
                                                                 const float* __restrict__ target, float* __restrict__ maps,
                                                                 double* __restrict__ partials) {
   __shared__ float s_x[kHY][kHX], s_y[kHY][kHX];
-  __shared__ double s_h[5][kHY][kTX];
+  __shared__ double s_h[4][kHY][kTX];
   __shared__ double s_red[2][kLossThreads / 32];
   const int ch = blockIdx.z;
   const size_t HW = (size_t)W * H;
@@ -115,10 +116,10 @@ __global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, T
   }
   __syncthreads();
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-  double f[5][2];
-  separable<5>(taps, [&](int r, int c, double (&v)[5]) {
+  double f[4][2];
+  separable<4>(taps, [&](int r, int c, double (&v)[4]) {
     const double a = s_x[r][c], b = s_y[r][c];
-    v[0] = a; v[1] = b; v[2] = a * a; v[3] = b * b; v[4] = a * b;
+    v[0] = a; v[1] = b; v[2] = a * a + b * b; v[3] = a * b;
   }, s_h, tx, ty, f);
   double sum_l1 = 0.0, sum_s = 0.0;
   const int gx = blockIdx.x * kTX + tx;
@@ -126,9 +127,9 @@ __global__ void __launch_bounds__(kLossThreads) ssim_maps_kernel(int W, int H, T
   for (int h = 0; h < 2; ++h) {
     const int gy = blockIdx.y * kTY + 2 * ty + h;
     if (gx >= W || gy >= H) continue;
-    const double mx = f[0][h], my = f[1][h], exx = f[2][h], eyy = f[3][h], exy = f[4][h];
+    const double mx = f[0][h], my = f[1][h], exx_eyy = f[2][h], exy = f[3][h];
     const double a1 = 2.0 * mx * my + kC1, a2 = 2.0 * (exy - mx * my) + kC2;
-    const double b1 = mx * mx + my * my + kC1, b2 = (exx - mx * mx) + (eyy - my * my) + kC2;
+    const double b1 = mx * mx + my * my + kC1, b2 = exx_eyy - (mx * mx + my * my) + kC2;
     const double ib = 1.0 / (b1 * b2);
     const double sv = a1 * a2 * ib;
     const size_t p = (size_t)gy * W + gx;
