@@ -259,7 +259,7 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __res
                                                          const float* __restrict__ depth, const u32* __restrict__ chunk_visible,
                                                          u32* __restrict__ keys, u32* __restrict__ vals, u32* __restrict__ n_vis,
                                                          u32* __restrict__ table0, u32* __restrict__ bucket_cnt,
-                                                         DepthRange* __restrict__ range_out) {
+                                                         u32* __restrict__ slots, DepthRange* __restrict__ range_out) {
   pdl_wait();
   __shared__ u32 s_part[8], s_off;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -297,21 +297,22 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __res
       keys[pos] = key;
       vals[pos] = (u32)i;
       atomicAdd(&table0[(pos / kSmallTile) * 256u + (key & 255u)], 1u);  // histogram of the first radix pass, per sort tile
-      atomicAdd(&bucket_cnt[bucket_of(key, rg)], 1u);
+      slots[pos] = atomicAdd(&bucket_cnt[bucket_of(key, rg)], 1u);  // arrival number = the pair's slot in its bucket
     }
     run += total;
   }
   if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *n_vis = run;
 }
 
-// Gathers the compacted pairs by bucket: a CTA per kScatterTile pairs.  Every CTA scans the bucket counts itself (32
+// Gathers the compacted pairs by bucket (slot inside the bucket = the arrival number depth_keys_kernel's histogram
+// atomic returned): a CTA per kScatterTile pairs.  Every CTA scans the bucket counts itself (32
 // per thread); CTA 0 leaves the bucket starts and the path decision for the kernels that follow.
 constexpr int kScatterItems = 4;
 constexpr int kScatterTile = 256 * kScatterItems;
 __global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restrict__ kin, const u32* __restrict__ vin,
                                                              u32* __restrict__ kout, u32* __restrict__ vout,
                                                              const u32* __restrict__ n_vis_p, const u32* __restrict__ bucket_cnt,
-                                                             u32* __restrict__ bucket_cur, u32* __restrict__ bucket_base,
+                                                             const u32* __restrict__ slots, u32* __restrict__ bucket_base,
                                                              u32* __restrict__ sort_flag, const DepthRange* __restrict__ range) {
   pdl_wait();
   __shared__ u32 s_base[kBuckets];
@@ -324,12 +325,13 @@ __global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restri
   if (threadIdx.x == 0) { s_big = 0; s_sq = 0; }
   __syncthreads();
   // this thread's pairs and their buckets first: the loads are in flight while the counts are scanned
-  u32 key[kScatterItems], val[kScatterItems];
+  u32 key[kScatterItems], val[kScatterItems], slot[kScatterItems];
 #pragma unroll
   for (int i = 0; i < kScatterItems; ++i) {
     const u32 j = start + (u32)i * 256u + threadIdx.x;
     key[i] = j < n ? __ldg(kin + j) : 0u;
     val[i] = j < n ? __ldg(vin + j) : 0u;
+    slot[i] = j < n ? __ldg(slots + j) : 0u;
   }
   constexpr int PER = kBuckets / 256;
   u32 c[PER], sum = 0, mx = 0;
@@ -359,17 +361,14 @@ __global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restri
     if (threadIdx.x == 0) *sort_flag = s_big;
   }
   if (s_big) return;  // the radix passes sort the compacted pairs instead
-  u32 pos[kScatterItems];
 #pragma unroll
   for (int i = 0; i < kScatterItems; ++i) {
     const u32 j = start + (u32)i * 256u + threadIdx.x;
-    const u32 b = bucket_of(key[i], rg);
-    pos[i] = j < n ? s_base[b] + atomicAdd(&bucket_cur[b], 1u) : 0u;
-  }
-#pragma unroll
-  for (int i = 0; i < kScatterItems; ++i) {
-    const u32 j = start + (u32)i * 256u + threadIdx.x;
-    if (j < n) { kout[pos[i]] = key[i]; vout[pos[i]] = val[i]; }
+    if (j < n) {
+      const u32 pos = s_base[bucket_of(key[i], rg)] + slot[i];
+      kout[pos] = key[i];
+      vout[pos] = val[i];
+    }
   }
 }
 
@@ -1066,7 +1065,8 @@ struct Workspace {
   u32* table;       // [256][nblocks]
   u32* dtable[4];   // per depth pass: [sort_blocks(N)][256] histograms of that pass's input arrangement
   u32* bucket_cnt;  // [kBuckets] pairs per depth bucket          } zeroed together with dtable
-  u32* bucket_cur;  // [kBuckets] fill cursors of the buckets      }
+  u32* bucket_cur;  // [kBuckets] (unused)                         }
+  u32* slots;       // [N] slot of every compacted pair inside its bucket
   u32* sort_flag;   // [1] 1: a bucket is too large, the radix passes sort instead
   u32* bucket_base; // [kBuckets] first slot of every bucket
   DepthRange* range;  // bucket mapping of this call
@@ -1105,6 +1105,7 @@ Workspace carve(void* base, int N, u64 capacity, int ntiles) {
     w.sort_flag = w.bucket_cur + kBuckets;
   }
   w.bucket_base = (u32*)take((u64)kBuckets * 4);
+  w.slots = (u32*)take((u64)N * 4);
   w.range = (DepthRange*)take(sizeof(DepthRange));
   for (int i = 0; i < 2; ++i) { w.pk[i] = (u32*)take((u64)N * 4); w.pv[i] = (u32*)take((u64)N * 4); }
   w.n_vis = (u32*)take(16);
@@ -1187,10 +1188,10 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   cudaMemsetAsync(ws.dtable[0], 0, ((size_t)4 * 256 * (nba + 1) + 2 * kBuckets + 64) * sizeof(u32), st);
   const u32 nchunks = (u32)((N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK);
   launch_pdl(depth_keys_kernel, nchunks, 256, 0, st, N, proj.tiles_touched, proj.depth,
-             proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis, ws.dtable[0], ws.bucket_cnt, ws.range);
+             proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis, ws.dtable[0], ws.bucket_cnt, ws.slots, ws.range);
   // bucketed order: pairs gathered by bucket into pk[1] / pv[1], ranked inside their buckets back into pk[0] / pv[0]
   launch_pdl(bucket_scatter_kernel, (u32)((N + kScatterTile - 1) / kScatterTile), 256, 0, st, ws.pk[0], ws.pv[0], ws.pk[1], ws.pv[1],
-             ws.n_vis, ws.bucket_cnt, ws.bucket_cur, ws.bucket_base, ws.sort_flag, (const DepthRange*)ws.range);
+             ws.n_vis, ws.bucket_cnt, (const u32*)ws.slots, ws.bucket_base, ws.sort_flag, (const DepthRange*)ws.range);
   launch_pdl(bucket_rank_kernel, (u32)((N + 255) / 256), 256, 0, st, ws.pk[1], ws.pv[1], ws.pk[0], ws.pv[0], ws.n_vis,
              ws.bucket_cnt, ws.bucket_base, ws.sort_flag, ws.range);
   launched(3);
