@@ -315,9 +315,12 @@ __global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restri
                                                              const u32* __restrict__ slots, u32* __restrict__ bucket_base,
                                                              u32* __restrict__ sort_flag, const DepthRange* __restrict__ range) {
   pdl_wait();
-  __shared__ u32 s_base[kBuckets];
+  // bucket starts, one padding word per 32 (a thread scans a run of 32 consecutive counts: without the padding the 256
+  // runs start in the same bank)
+  __shared__ u32 s_base[kBuckets + kBuckets / 32];
   __shared__ u32 s_big;
   __shared__ unsigned long long s_sq;
+  auto at = [](u32 i) { return i + (i >> 5); };
   const u32 n = *n_vis_p;
   const u32 start = blockIdx.x * kScatterTile;
   if (start >= n && blockIdx.x != 0) return;
@@ -346,7 +349,7 @@ __global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restri
   u32 total;
   u32 run = block_exclusive_scan(sum, &total);
 #pragma unroll
-  for (int j = 0; j < PER; ++j) { s_base[threadIdx.x * PER + j] = run; run += c[j]; }
+  for (int j = 0; j < PER; ++j) { s_base[at(threadIdx.x * PER + j)] = run; run += c[j]; }
   // one huge bucket, or many large ones (more than kRankBudget comparisons per pair on average): the radix passes
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, d);
@@ -357,7 +360,7 @@ __global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restri
   __syncthreads();
   if (blockIdx.x == 0) {
 #pragma unroll
-    for (int j = 0; j < PER; ++j) bucket_base[threadIdx.x * PER + j] = s_base[threadIdx.x * PER + j];
+    for (int j = 0; j < PER; ++j) bucket_base[threadIdx.x * PER + j] = s_base[at(threadIdx.x * PER + j)];
     if (threadIdx.x == 0) *sort_flag = s_big;
   }
   if (s_big) return;  // the radix passes sort the compacted pairs instead
@@ -365,7 +368,7 @@ __global__ void __launch_bounds__(256) bucket_scatter_kernel(const u32* __restri
   for (int i = 0; i < kScatterItems; ++i) {
     const u32 j = start + (u32)i * 256u + threadIdx.x;
     if (j < n) {
-      const u32 pos = s_base[bucket_of(key[i], rg)] + slot[i];
+      const u32 pos = s_base[at(bucket_of(key[i], rg))] + slot[i];
       kout[pos] = key[i];
       vout[pos] = val[i];
     }
