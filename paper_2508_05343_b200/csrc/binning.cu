@@ -278,28 +278,46 @@ __global__ void __launch_bounds__(256) depth_keys_kernel(int N, const u32* __res
     s_off = t;
   }
   __syncthreads();
-  u32 run = s_off;
+  // the chunk's four rounds of 256 primitives at once: one vote and one exchange of the warp counts for all of them,
+  // then every load and every atomic of the thread is in flight before the first result is needed
+  constexpr int ROUNDS = GABSPLAT_CHUNK / 256;
+  __shared__ u32 s_cnt[ROUNDS][8];
   const int base = blockIdx.x * GABSPLAT_CHUNK;
-#pragma unroll 1
-  for (int r = 0; r < GABSPLAT_CHUNK / 256; ++r) {
+  bool vis[ROUNDS];
+  u32 bal[ROUNDS];
+#pragma unroll
+  for (int r = 0; r < ROUNDS; ++r) {
     const int i = base + r * 256 + (int)threadIdx.x;
-    const bool vis = i < N && tiles_touched[i] != 0;
-    const u32 bal = __ballot_sync(0xffffffffu, vis);
-    __syncthreads();  // s_part of the previous round consumed
-    if (lane == 0) s_part[w] = (u32)__popc(bal);
-    __syncthreads();
+    vis[r] = i < N && tiles_touched[i] != 0;
+  }
+#pragma unroll
+  for (int r = 0; r < ROUNDS; ++r) {
+    bal[r] = __ballot_sync(0xffffffffu, vis[r]);
+    if (lane == 0) s_cnt[r][w] = (u32)__popc(bal[r]);
+  }
+  __syncthreads();
+  u32 run = s_off, pos[ROUNDS], key[ROUNDS], slot[ROUNDS];
+#pragma unroll
+  for (int r = 0; r < ROUNDS; ++r) {
     u32 before = 0, total = 0;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) { const u32 c = s_part[j]; before += j < w ? c : 0u; total += c; }
-    if (vis) {
-      const u32 pos = run + before + (u32)__popc(bal & ((1u << lane) - 1u));
-      const u32 key = __float_as_uint(depth[i]);
-      keys[pos] = key;
-      vals[pos] = (u32)i;
-      atomicAdd(&table0[(pos / kSmallTile) * 256u + (key & 255u)], 1u);  // histogram of the first radix pass, per sort tile
-      slots[pos] = atomicAdd(&bucket_cnt[bucket_of(key, rg)], 1u);  // arrival number = the pair's slot in its bucket
-    }
+    for (int j = 0; j < 8; ++j) { const u32 c = s_cnt[r][j]; before += j < w ? c : 0u; total += c; }
+    pos[r] = run + before + (u32)__popc(bal[r] & ((1u << lane) - 1u));
     run += total;
+  }
+#pragma unroll
+  for (int r = 0; r < ROUNDS; ++r) key[r] = vis[r] ? __float_as_uint(depth[base + r * 256 + (int)threadIdx.x]) : 0u;
+#pragma unroll
+  for (int r = 0; r < ROUNDS; ++r)
+    slot[r] = vis[r] ? atomicAdd(&bucket_cnt[bucket_of(key[r], rg)], 1u) : 0u;  // arrival number = the pair's slot in its bucket
+#pragma unroll
+  for (int r = 0; r < ROUNDS; ++r) {
+    if (vis[r]) {
+      keys[pos[r]] = key[r];
+      vals[pos[r]] = (u32)(base + r * 256 + (int)threadIdx.x);
+      atomicAdd(&table0[(pos[r] / kSmallTile) * 256u + (key[r] & 255u)], 1u);  // histogram of the first radix pass, per sort tile
+      slots[pos[r]] = slot[r];
+    }
   }
   if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *n_vis = run;
 }
