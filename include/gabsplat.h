@@ -120,8 +120,9 @@ int32_t gabsplat_packed_floats(int32_t K);
 
 /* Tile binning state.  capacity = number of (key,id) slots the caller allocated. */
 typedef struct {
-  uint32_t* offsets;          /* [N]  inclusive prefix sum of tiles_touched over the visible primitives in
-                                 depth order (one entry per visible primitive; the rest is not written) */
+  uint32_t* offsets;          /* [N]  scratch of the binning, one entry per visible primitive in depth order:
+                                 the inclusive prefix of tiles_touched on images of more than 26000 tiles, of the
+                                 estimated placement cost otherwise; the rest is not written             */
   uint64_t* keys;             /* [capacity]  sorted on return: (tile_id << 32) | bits(depth).  No later stage
                                  reads the keys: for images of at most 26000 tiles the pointer may be NULL
                                  and the keys are then not materialised                                */

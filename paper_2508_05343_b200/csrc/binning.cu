@@ -3,8 +3,9 @@
 // ties by primitive index -- exactly what a stable LSD radix sort of the keys on one-byte digits gives -- plus
 // the [start,end) range of every tile.  The depth digits are sorted on the visible primitives, not on the D >> N
 // instances; the tile digit then takes one more stable pass:
-//   A   (bits(depth), index) of the n_vis visible primitives, compacted in index order; 4 stable one-byte
-//       passes over them -> `order`: visible primitives front to back, ties by index
+//   A   (bits(depth), index) of the n_vis visible primitives, compacted in index order, ordered by (depth, index):
+//       binned into depth buckets and ranked inside their bucket (3 launches), or -- a bucket too large -- by 4
+//       stable one-byte passes -> `order`: visible primitives front to back, ties by index
 //   K2  inclusive prefix over that order of the placement cost (B') or of tiles_touched (B) -> offsets (and D for B)
 //   B'  images of at most 26000 tiles: ONE stable counting pass on the whole tile id -- per-(tile, chunk) counts,
 //       their prefix (tile ranges and D fall out of it), then every instance id written once at its final slot;
