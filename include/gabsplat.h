@@ -134,6 +134,12 @@ typedef struct {
   uint32_t* num_instances;    /* [1]  device: D = total instance count                               */
   void* workspace;            /* device scratch, >= gabsplat_sort_workspace_bytes(N, capacity, W, H) bytes */
   uint64_t workspace_bytes;
+  const uint32_t* tile_work_hint; /* optional (NULL: none), [tiles_y*tiles_x]: gabsplat_fwd_out.tile_work of an
+                                 earlier render of (about) this view.  tile_order then follows min(hint, list
+                                 length) instead of the list length.  A tile's time is set by how far it walks
+                                 its list before its last pixel saturates, which the list length does not
+                                 predict; a trainer that revisits its views keeps one hint array per view.
+                                 It changes the launch order of the forward blend and nothing else          */
 } gabsplat_binning;
 
 uint64_t gabsplat_sort_workspace_bytes(int32_t N, uint64_t capacity, int32_t width, int32_t height);
@@ -150,6 +156,9 @@ typedef struct {
    * reverse and REQUIRES them: it neither re-walks the tile lists nor re-takes any skip/stop decision. */
   void* blend_state;
   uint64_t blend_state_bytes;
+  uint32_t* tile_work; /* optional (NULL: not written), [tiles_y*tiles_x]: list entries the tile consumed before all of
+                          its pixels were finished (a multiple of the staging batch, at most the list length):
+                          the tile_work_hint of a later gabsplat_bin_sort of the same view                      */
 } gabsplat_fwd_out;
 
 /* Bytes of gabsplat_fwd_out.blend_state for an image of this size and `capacity` instance slots

@@ -47,12 +47,12 @@ class _Projected(C.Structure):
 class _Binning(C.Structure):
     _fields_ = [("offsets", C.c_void_p), ("keys", C.c_void_p), ("ids", C.c_void_p), ("tile_ranges", C.c_void_p),
                 ("tile_order", C.c_void_p), ("capacity", C.c_uint64), ("num_instances", C.c_void_p), ("workspace", C.c_void_p),
-                ("workspace_bytes", C.c_uint64)]
+                ("workspace_bytes", C.c_uint64), ("tile_work_hint", C.c_void_p)]
 
 
 class _FwdOut(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("image", "final_T", "n_contrib", "blend_state")] + [
-        ("blend_state_bytes", C.c_uint64)]
+        ("blend_state_bytes", C.c_uint64), ("tile_work", C.c_void_p)]
 
 
 class _Grads(C.Structure):
@@ -260,6 +260,7 @@ class Binning:
         self.workspace_bytes = int(lib().gabsplat_sort_workspace_bytes(N, self.capacity, cam.width, cam.height))
         self.workspace = z((self.workspace_bytes + 256,), torch.uint8)
         self.D = None  # host copy of the instance count when the call read it back
+        self.tile_work_hint = None  # optional int32 [n_tiles]: FwdOut.tile_work of an earlier render of the view
 
     def struct(self) -> _Binning:
         b = _Binning()
@@ -271,6 +272,7 @@ class Binning:
         b.num_instances = self.num_instances.data_ptr()
         b.workspace = (self.workspace.data_ptr() + 255) // 256 * 256
         b.workspace_bytes = self.workspace_bytes
+        b.tile_work_hint = self.tile_work_hint.data_ptr() if self.tile_work_hint is not None else None
         return b
 
 
@@ -285,6 +287,7 @@ class FwdOut:
         self.n_contrib = torch.zeros((H, W), dtype=torch.int32, device=device)
         self.blend_state = None
         self.blend_state_bytes = 0
+        self.tile_work = None   # optional int32 [n_tiles] output: list entries every tile consumed (the next render's hint)
         if capacity is not None:
             self.blend_state_bytes = int(lib().gabsplat_blend_state_bytes(W, H, int(capacity)))
             self.blend_state = torch.empty((self.blend_state_bytes,), dtype=torch.uint8, device=device)
@@ -292,6 +295,7 @@ class FwdOut:
     def struct(self, save_state: bool = True) -> _FwdOut:
         o = _FwdOut()
         o.image, o.final_T, o.n_contrib = self.image.data_ptr(), self.final_T.data_ptr(), self.n_contrib.data_ptr()
+        o.tile_work = self.tile_work.data_ptr() if self.tile_work is not None else None
         if save_state and self.blend_state is not None:
             o.blend_state, o.blend_state_bytes = self.blend_state.data_ptr(), self.blend_state_bytes
         else:

@@ -45,7 +45,8 @@ __global__ void __launch_bounds__(kBlendThreads, GS_FWD_MINB) blend_forward_kern
                                                                       const float4* __restrict__ colour,
                                                                       float* __restrict__ image, float* __restrict__ final_T,
                                                                       uint32_t* __restrict__ n_contrib,
-                                                                      uint32_t* __restrict__ counters, BlendState save) {
+                                                                      uint32_t* __restrict__ counters, BlendState save,
+                                                                      uint32_t* __restrict__ tile_work) {
   pdl_wait();
   constexpr int R4 = packed_floats(K) / 4;
   constexpr int TL = K > 0 ? 4 * ((3 * K + 3) / 4) : 1;
@@ -152,6 +153,7 @@ __global__ void __launch_bounds__(kBlendThreads, GS_FWD_MINB) blend_forward_kern
   };
 
 #endif
+  int walked = n;                                              // list entries consumed when the tile finished
   uint32_t n_saved = 0;                                        // warp-uniform
   const size_t save_at = 2 * (size_t)range.x + (size_t)g.warp * n;  // this warp's slice of save.ids / save.masks
   uint32_t* save_id = SAVE ? save.ids + save_at : nullptr;          // lane 0's write cursors
@@ -173,7 +175,7 @@ __global__ void __launch_bounds__(kBlendThreads, GS_FWD_MINB) blend_forward_kern
   }
   for (int b = 0; b < nbatch; ++b) {
     const bool all_done = done[0] && done[1] && done[2] && done[3];
-    if (__syncthreads_and(all_done)) break;
+    if (__syncthreads_and(all_done)) { walked = b * kFwdBatch; break; }
     int ns_next = 0;
     if (b + 1 < nbatch) {
       ns_next = filter_compact(b + 1, (b + 1) & 1);
@@ -187,7 +189,7 @@ __global__ void __launch_bounds__(kBlendThreads, GS_FWD_MINB) blend_forward_kern
 #else
   for (int b0 = 0; b0 < n; b0 += kBatch) {
     const bool all_done = done[0] && done[1] && done[2] && done[3];
-    if (__syncthreads_and(all_done)) break;
+    if (__syncthreads_and(all_done)) { walked = b0; break; }
     const int m = min(kBatch, n - b0);
     const int ns = stage_batch<K, false>(g, ids, packed, colour, range.x, b0, m, s_rec, s_cnt);
     if (__all_sync(kFull, all_done)) continue;  // warp-uniform: the votes below need every lane
@@ -273,6 +275,7 @@ __global__ void __launch_bounds__(kBlendThreads, GS_FWD_MINB) blend_forward_kern
 #endif
   }
   if (SAVE && g.lane == 0) save.counts[2 * g.tile + g.warp] = n_saved;
+  if (tile_work && threadIdx.x == 0) tile_work[g.tile] = (uint32_t)walked;   // the launch-order hint of a later render
   const size_t HW = (size_t)cam.width * cam.height;
 #pragma unroll
   for (int s = 0; s < kSlots; ++s) {
@@ -295,11 +298,11 @@ __global__ void __launch_bounds__(kBlendThreads, GS_FWD_MINB) blend_forward_kern
 template <int K, bool COUNT, bool SAVE>
 cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, const float4* colour,
                      float* image, float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save,
-                     cudaStream_t st) {
+                     uint32_t* tile_work, cudaStream_t st) {
   const int ntiles = cam.tiles_x * cam.tiles_y;
   launch_pdl(blend_forward_kernel<K, COUNT, SAVE>, ntiles, kBlendThreads, 0, st, cam, (const uint32_t*)bin.tile_order,
              reinterpret_cast<const uint2*>(bin.tile_ranges), (const uint32_t*)bin.ids, reinterpret_cast<const float4*>(proj.packed),
-             colour, image, final_T, n_contrib, counters, save ? *save : BlendState{nullptr, nullptr, nullptr, nullptr});
+             colour, image, final_T, n_contrib, counters, save ? *save : BlendState{nullptr, nullptr, nullptr, nullptr}, tile_work);
   launched();
   return cudaGetLastError();
 }
@@ -307,17 +310,17 @@ cudaError_t launch_k(const Camera& cam, const gabsplat_projected& proj, const ga
 template <bool COUNT, bool SAVE>
 cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin, const float4* colour,
                      float* image, float* final_T, uint32_t* n_contrib, uint32_t* counters, const BlendState* save,
-                     cudaStream_t st) {
+                     uint32_t* tile_work, cudaStream_t st) {
   switch (K) {
-    case 0: return launch_k<0, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
-    case 1: return launch_k<1, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
-    case 2: return launch_k<2, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
-    case 3: return launch_k<3, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
-    case 4: return launch_k<4, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
-    case 5: return launch_k<5, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
-    case 6: return launch_k<6, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
-    case 7: return launch_k<7, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
-    case 8: return launch_k<8, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, st);
+    case 0: return launch_k<0, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, tile_work, st);
+    case 1: return launch_k<1, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, tile_work, st);
+    case 2: return launch_k<2, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, tile_work, st);
+    case 3: return launch_k<3, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, tile_work, st);
+    case 4: return launch_k<4, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, tile_work, st);
+    case 5: return launch_k<5, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, tile_work, st);
+    case 6: return launch_k<6, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, tile_work, st);
+    case 7: return launch_k<7, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, tile_work, st);
+    case 8: return launch_k<8, COUNT, SAVE>(cam, proj, bin, colour, image, final_T, n_contrib, counters, save, tile_work, st);
   }
   return cudaErrorInvalidValue;
 }
@@ -327,8 +330,8 @@ cudaError_t dispatch(int K, const Camera& cam, const gabsplat_projected& proj, c
 cudaError_t launch_blend_forward(int K, const Camera& cam, const gabsplat_projected& proj,
                                  const gabsplat_binning& bin, const gabsplat_fwd_out& out, const BlendState* save,
                                  cudaStream_t st) {
-  return save ? dispatch<false, true>(K, cam, proj, bin, nullptr, out.image, out.final_T, out.n_contrib, nullptr, save, st)
-              : dispatch<false, false>(K, cam, proj, bin, nullptr, out.image, out.final_T, out.n_contrib, nullptr, nullptr, st);
+  return save ? dispatch<false, true>(K, cam, proj, bin, nullptr, out.image, out.final_T, out.n_contrib, nullptr, save, out.tile_work, st)
+              : dispatch<false, false>(K, cam, proj, bin, nullptr, out.image, out.final_T, out.n_contrib, nullptr, nullptr, out.tile_work, st);
 }
 
 namespace {
@@ -362,12 +365,12 @@ cudaError_t launch_blend_aux(int N, int K, const float* weights, const Camera& c
   }
   Camera c = cam;
   c.bg[0] = c.bg[1] = c.bg[2] = 0.f;
-  return dispatch<false, false>(K, c, proj, bin, aux, image, final_T, n_contrib, nullptr, nullptr, st);
+  return dispatch<false, false>(K, c, proj, bin, aux, image, final_T, n_contrib, nullptr, nullptr, nullptr, st);
 }
 
 cudaError_t launch_count_pairs(int K, const Camera& cam, const gabsplat_projected& proj, const gabsplat_binning& bin,
                                uint32_t* counters, cudaStream_t st) {
-  return dispatch<true, false>(K, cam, proj, bin, nullptr, nullptr, nullptr, nullptr, counters, nullptr, st);
+  return dispatch<true, false>(K, cam, proj, bin, nullptr, nullptr, nullptr, nullptr, counters, nullptr, nullptr, st);
 }
 
 }  // namespace gabsplat

@@ -62,11 +62,13 @@ Layout carve(void* base, int N, int K, int width, int height, uint64_t capacity)
   l.bin.num_instances = a.take<uint32_t>(4);
   l.bin.workspace_bytes = sort_workspace_bytes(N, capacity, (int)tiles);
   l.bin.workspace = a.take<char>(l.bin.workspace_bytes);
+  l.bin.tile_work_hint = nullptr;
   l.fwd.image = a.take<float>(3 * hw);
   l.fwd.final_T = a.take<float>(hw);
   l.fwd.n_contrib = a.take<uint32_t>(hw);
   l.fwd.blend_state_bytes = blend_state_bytes(tiles, capacity);
   l.fwd.blend_state = a.take<char>(l.fwd.blend_state_bytes);
+  l.fwd.tile_work = nullptr;
   l.dL = a.take<float>(3 * hw);
   l.grads.d_means = a.take<float>(n * 3);
   l.grads.d_scales = a.take<float>(n * 3);
