@@ -210,7 +210,8 @@ def workload_config(args, name, scene, cam) -> dict:
     return {"workload": "%s: N=%d primitives, K=%d, SH degree 3, %dx%d, 8 seeded views, %s" % (
                 name, scene.N, scene.K, cam.width, cam.height,
                 "forward" if args.forward_only else "forward+backward") +
-                        "; the sorted 64-bit keys are not materialised in the timed step (no stage reads them)",
+                        "; the sorted 64-bit keys are not materialised in the timed step (no stage reads them); the "
+                        "forward's tiles are launched in the order of their walk lengths in the previous render of the view",
             "config_name": name, "N": scene.N, "K": scene.K, "width": cam.width, "height": cam.height,
             "zero_weights": bool(args.zero_weights),
             "l2_policy": "inputs larger than L2 (scene %.0f MB + gradients %.0f MB per step vs 126 MB L2)" % (
@@ -315,7 +316,13 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     dLs = [torch.from_numpy(scenes.make_image_grad(name, v, cams[v])).to(dev) for v in range(V)] if backward else None
     proj = gb.Projected(N, K, dev)
 
-    # dry run per view (untimed): instance counts for the capacity, and the roofline numerators
+    # Launch-order hints (gabsplat_fwd_out.tile_work -> gabsplat_binning.tile_work_hint): one array per view, written by
+    # every forward of the view and read by the next bin_sort of the same view -- what a trainer that cycles through
+    # its views keeps.  It changes the order in which the forward's CTAs start, nothing else (results bit-identical);
+    # the same step without hints is timed beside it (ms_per_step_no_hint).
+    n_tiles = cams[0].tiles_x * cams[0].tiles_y
+    hints = [torch.zeros((n_tiles,), dtype=torch.int32, device=dev) for _ in range(V)]
+    # dry run per view (untimed): instance counts for the capacity, the roofline numerators, and the first hints
     stats = []
     probe = gb.Binning(N, cams[0], 0, dev)
     Ds = []
@@ -323,7 +330,9 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
         gb.gabsplat_preprocess(ctx, ds, cams[v], proj)
         b = gb.gabsplat_bin_sort(ctx, N, proj, cams[v], capacity=None)
         Ds.append(b.D)
-        fwd = gb.gabsplat_render_forward(ctx, ds, cams[v], proj, b, save_state=False)
+        fwd = gb.FwdOut(cams[v], dev, None)
+        fwd.tile_work = hints[v]
+        gb.gabsplat_render_forward(ctx, ds, cams[v], proj, b, fwd, save_state=False)
         cnt = gb.gabsplat_count_pairs(ctx, ds, cams[v], proj, b).to(torch.int64).reshape(-1, 4).sum(0).tolist()
         stats.append({"n_visible": int((proj.tiles_touched != 0).sum().item()), "D": b.D, "examined": cnt[0],
                       "envelope": cnt[1], "blended": cnt[2], "envelope_le_last": cnt[3],
@@ -339,8 +348,10 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
 
     my_view = lambda i: view_of_step(i, rank, V)
 
-    def step(i, do_backward, bins=bins):
+    def step(i, do_backward, bins=bins, use_hint=True):
         v = my_view(i)
+        bins.tile_work_hint = hints[v] if use_hint else None
+        fwd.tile_work = hints[v] if use_hint else None
         # S1 + S2 through the fused entry point (same results as the two calls; the value track of the projection
         # overlaps the binning)
         gb.gabsplat_preprocess_bin_sort(ctx, ds, cams[v], proj, bins, read_count=False)
@@ -355,8 +366,8 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(n, do_backward, with_stage_timing, bins=bins):
-        step_ = lambda i, b: step(i, b, bins)
+    def timed(n, do_backward, with_stage_timing, bins=bins, use_hint=True):
+        step_ = lambda i, b: step(i, b, bins, use_hint)
         for i in range(args.warmup):
             step_(i, do_backward)
         barrier()
@@ -385,6 +396,8 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
     clocks = sampler.stop() if rank == 0 else None
     staged_ms, _, recs = timed(args.steps, backward, True)
     fwd_ms, _, _ = timed(args.steps, False, False) if backward else (total_ms, 0, [])
+    nohint_ms, _, _ = timed(args.steps, backward, False, use_hint=False)
+    fwd_nohint_ms, _, _ = timed(args.steps, False, False, use_hint=False) if backward else (nohint_ms, 0, [])
     bins_k = gb.Binning(N, cams[0], capacity, dev, with_keys=True)
     keys_total_ms, _, _ = timed(args.steps, backward, False, bins_k)
     del bins_k
@@ -515,6 +528,10 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
         "fwd_ms_per_frame": fwd_ms / args.steps, "fwd_bwd_ms_per_view": ms_per_step if backward else None,
         "fwd_mpix_per_s": world * H * W / 1e6 / (fwd_ms / args.steps / 1e3),
         "ms_per_step_with_keys": keys_total_ms / args.steps,
+        "ms_per_step_no_hint": nohint_ms / args.steps, "fwd_ms_per_frame_no_hint": fwd_nohint_ms / args.steps,
+        "launch_order_hint": "every forward writes, per tile, how many list entries it consumed (gabsplat_fwd_out.tile_work); the "
+                             "next bin_sort of the SAME view orders the forward's CTAs by it (gabsplat_binning.tile_work_hint). "
+                             "Scheduling only: results are bit-identical; *_no_hint are the same steps without it",
         "loss_fwd_bwd_ms": loss_ms,
         "keys": "the sorted 64-bit (tile|depth) keys are an inspectable by-product that no stage reads; the timed "
                 "step does not materialise them, ms_per_step_with_keys is the same step with them written",

@@ -229,3 +229,49 @@ def test_depth_sort_paths(levels):
     assert g["D"] == o["num_instances"]
     assert np.array_equal(g["keys"], o["keys"]) and np.array_equal(g["ids"], o["ids"])
     assert np.array_equal(g["tile_ranges"], o["tile_ranges"])
+
+
+def test_launch_order_hint_changes_nothing_but_the_order():
+    """gabsplat_fwd_out.tile_work (list entries every tile consumed) fed back as gabsplat_binning.tile_work_hint: the
+    tile order becomes the order of min(hint, list length), still a permutation; image, final T, last contributor,
+    lists and gradients are bit-identical (only the forward's launch order changed)."""
+    import torch
+    from paper_2508_05343_b200 import binding as gb
+    from gpu_helpers import ctx
+    from test_gpu_parity import _ragged_case
+    scene, cam = _ragged_case("unbounded", 40000, 403, 251, 360.0)
+    dL = torch.from_numpy(np.random.default_rng(5).standard_normal((3, cam.height, cam.width)).astype(np.float32)).cuda()
+    c = ctx()
+    ds = gb.upload_scene(scene)
+    proj = gb.gabsplat_preprocess(c, ds, cam)
+    bins = gb.gabsplat_bin_sort(c, ds.N, proj, cam)
+    fwd = gb.FwdOut(cam, ds.means.device, bins.capacity)
+    fwd.tile_work = torch.full((bins.n_tiles,), -1, dtype=torch.int32, device="cuda")
+    gb.gabsplat_render_forward(c, ds, cam, proj, bins, fwd)
+    g0 = gb.gabsplat_render_backward(c, ds, cam, proj, bins, fwd, dL)
+    torch.cuda.synchronize()
+    n = (bins.tile_ranges[:, 1] - bins.tile_ranges[:, 0]).cpu().numpy()
+    work = fwd.tile_work.cpu().numpy()
+    assert np.all(work >= 0) and np.all(work <= n)                     # every tile wrote it
+    assert np.all((work % 128 == 0) | (work == n))                     # whole staging batches, or the whole list
+    last = fwd.n_contrib.cpu().numpy().reshape(-1)
+    assert work.max() >= 1 and last.max() <= n.max()
+    ref = dict(image=fwd.image.clone(), T=fwd.final_T.clone(), nc=fwd.n_contrib.clone(), ids=bins.ids.clone(),
+               ranges=bins.tile_ranges.clone(), order=bins.tile_order.clone())
+    # second render of the view, with the hint
+    bins.tile_work_hint = fwd.tile_work.clone()
+    gb.gabsplat_bin_sort(c, ds.N, proj, cam, bins)
+    gb.gabsplat_render_forward(c, ds, cam, proj, bins, fwd)
+    g1 = gb.gabsplat_render_backward(c, ds, cam, proj, bins, fwd, dL)
+    torch.cuda.synchronize()
+    order = bins.tile_order.cpu().numpy()
+    assert np.array_equal(np.sort(order), np.arange(bins.n_tiles))     # a permutation
+    key = np.minimum(work, n)[order]
+    # descending up to the 256 buckets of the counting sort behind it
+    assert key[0] == key.max() and np.all(np.diff(key.astype(np.int64)) <= max(1, int(key.max()) // 255 + 1))
+    assert not np.array_equal(order, ref["order"].cpu().numpy())
+    assert torch.equal(fwd.image, ref["image"]) and torch.equal(fwd.final_T, ref["T"]) and torch.equal(fwd.n_contrib, ref["nc"])
+    assert torch.equal(bins.ids, ref["ids"]) and torch.equal(bins.tile_ranges, ref["ranges"])
+    for name in ("d_means", "d_scales", "d_rotations", "d_opacities", "d_sh", "d_freqs", "d_weights"):
+        a, b = getattr(g0, name), getattr(g1, name)
+        assert torch.allclose(a, b, rtol=1e-4, atol=2e-6 * float(a.abs().max()))   # equal up to the order of the fp32 atomics
