@@ -53,8 +53,8 @@ def test_struct_sizes_match_header():
     assert C.sizeof(gb._Camera) == 4 * (2 + 4 + 12 + 1 + 3)
     assert C.sizeof(gb._Scene) == 16 + 7 * 8
     assert C.sizeof(gb._Projected) == 11 * 8
-    assert C.sizeof(gb._Binning) == 9 * 8
-    assert C.sizeof(gb._FwdOut) == 5 * 8
+    assert C.sizeof(gb._Binning) == 10 * 8      # ... + tile_work_hint
+    assert C.sizeof(gb._FwdOut) == 6 * 8        # ... + tile_work
     assert C.sizeof(gb._Grads) == 9 * 8
 
 
