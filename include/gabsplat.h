@@ -128,8 +128,8 @@ typedef struct {
                                  and the keys are then not materialised                                */
   uint32_t* ids;              /* [capacity]  primitive index of each instance, same order            */
   uint32_t* tile_ranges;      /* [tiles_y*tiles_x][2]  [start,end) into keys/ids; (0,0) if empty     */
-  uint32_t* tile_order;       /* [tiles_y*tiles_x]  the tiles by descending list length: the order in
-                                 which the forward blend launches its CTAs (longest first)            */
+  uint32_t* tile_order;       /* [tiles_y*tiles_x]  the order in which the forward blend launches its CTAs:
+                                 the tiles by descending list length, or by tile_work_hint (below)      */
   uint64_t capacity;
   uint32_t* num_instances;    /* [1]  device: D = total instance count                               */
   void* workspace;            /* device scratch, >= gabsplat_sort_workspace_bytes(N, capacity, W, H) bytes */
