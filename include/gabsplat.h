@@ -240,6 +240,36 @@ uint64_t gabsplat_loss_workspace_bytes(int32_t width, int32_t height);
 int32_t gabsplat_loss(gabsplat_ctx* ctx, int32_t width, int32_t height, const float* image, const float* target, float lambda,
                       float* loss_out, float* dL_dimage, void* workspace, uint64_t workspace_bytes, void* stream);
 
+/* gabsplat_loss_static -- the loss above for callers that cannot allocate device memory.
+ *
+ * gabsplat_loss wants a workspace, and somebody has to cudaMalloc it.  Not every caller can: code that runs as a
+ * plugin inside another engine and is given only its input and output buffers; a real-time loop whose rules forbid
+ * allocator calls once it is running (cudaMalloc serialises the whole process and may stall the GPU); a process that
+ * shares a nearly full GPU and cannot count on a free block being there.  This entry point needs no workspace, no
+ * context and no gabsplat_create: its scratch (the nine derivative maps and the per-block partial sums of Eq.14 :171)
+ * is a fixed array compiled into the library.  It never calls cudaMalloc, cudaFree or any routine that allocates.
+ *
+ * Same arithmetic, same kernels, same results bit for bit as gabsplat_loss; same arguments minus ctx and workspace.
+ * image, target, loss_out [3], dL_dimage (may be NULL) are DEVICE pointers owned by the caller, on the device that is
+ * CURRENT on the calling thread, which must also be the device of `stream`.
+ *
+ * Limit: width * height <= gabsplat_loss_static_max_pixels() = 262 144 (512 x 512) and each side <= 2048.  A larger
+ *   image returns GABSPLAT_CAPACITY and launches nothing; use gabsplat_loss for it.
+ * Cost: the array is 9 MiB and is resident on EVERY GPU on which this library's module is loaded, from then until
+ *   the process exits, whether or not this function is ever called.
+ * First call on each device: looks up the array's address on that device (cudaGetSymbolAddress; host-side, cached
+ *   afterwards).  Make that first call before starting any stream capture on the device.
+ * Sharing: all calls on one GPU use the same array.  It keeps whatever the previous call left; that is harmless here
+ *   because each call writes every scratch value before reading it, so nothing has to be cleared.  But two calls whose
+ *   kernels can overlap on the GPU -- different streams without an ordering between them, or two host threads -- race
+ *   on it and both results are garbage.  Order such calls yourself (one stream, or events).
+ * Errors: GABSPLAT_INVALID_ARG / GABSPLAT_CAPACITY / GABSPLAT_CUDA; gabsplat_loss_static_last_error() returns the
+ *   text of the calling thread's last non-OK status (never NULL).  Asynchronous like gabsplat_loss. */
+uint64_t gabsplat_loss_static_max_pixels(void);
+const char* gabsplat_loss_static_last_error(void);
+int32_t gabsplat_loss_static(int32_t width, int32_t height, const float* image, const float* target, float lambda,
+                             float* loss_out, float* dL_dimage, void* stream);
+
 /* Convenience for callers with HOST buffers (bench.py's end-to-end leg): one forward (and, if
  * dL_dimage_host != NULL, backward) pass with host->device copies of the scene / image gradient and
  * device->host copies of the image / gradients inside the call; synchronises.  All pointers in

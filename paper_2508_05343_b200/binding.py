@@ -110,6 +110,12 @@ def lib():
         L.gabsplat_loss_workspace_bytes.restype = C.c_uint64
         L.gabsplat_loss.argtypes = [P, C.c_int32, C.c_int32, P, P, C.c_float, P, P, P, C.c_uint64, P]
         L.gabsplat_loss.restype = C.c_int32
+        L.gabsplat_loss_static_max_pixels.argtypes = []
+        L.gabsplat_loss_static_max_pixels.restype = C.c_uint64
+        L.gabsplat_loss_static_last_error.argtypes = []
+        L.gabsplat_loss_static_last_error.restype = C.c_char_p
+        L.gabsplat_loss_static.argtypes = [C.c_int32, C.c_int32, P, P, C.c_float, P, P, P]
+        L.gabsplat_loss_static.restype = C.c_int32
         L.gabsplat_kernel_launches.argtypes = []
         L.gabsplat_kernel_launches.restype = C.c_uint64
         L.gabsplat_timing_enable.argtypes = [P, C.c_int32]
@@ -445,6 +451,32 @@ def gabsplat_loss(ctx: Context, image: torch.Tensor, target: torch.Tensor, lam: 
     ctx.check(lib().gabsplat_loss(ctx._h, W, H, _ptr(image), _ptr(target), float(lam), _ptr(out),
                                   _ptr(grad) if want_grad else None, _ptr(workspace), workspace.numel(), _stream(stream)))
     return out, grad
+
+
+def gabsplat_loss_static_max_pixels() -> int:
+    return int(lib().gabsplat_loss_static_max_pixels())
+
+
+def gabsplat_loss_static(image: torch.Tensor, target: torch.Tensor, lam: float = 0.2, out: torch.Tensor | None = None,
+                         grad: torch.Tensor | None = None, want_grad: bool = True, stream=None):
+    """gabsplat_loss without a workspace and without a context, for callers that may not allocate device memory
+    (plugins that only own their inputs and outputs, loops that must stay off the allocator): the scratch is a fixed
+    array inside the library, one per GPU, shared by all calls.  Pass `out` ([3]) and `grad` (like image) to keep this
+    wrapper from allocating them with torch; images beyond gabsplat_loss_static_max_pixels() raise (status CAPACITY).
+    Calls that may overlap on the GPU race on the shared scratch: keep them on one stream."""
+    assert image.dtype == torch.float32 and target.dtype == torch.float32 and image.shape == target.shape
+    assert image.is_contiguous() and target.is_contiguous() and image.dim() == 3 and image.shape[0] == 3
+    H, W = int(image.shape[1]), int(image.shape[2])
+    if out is None:
+        out = torch.empty((3,), dtype=torch.float32, device=image.device)
+    if want_grad and grad is None:
+        grad = torch.empty_like(image)
+    with torch.cuda.device(image.device):      # the scratch that is used is the current device's
+        rc = lib().gabsplat_loss_static(W, H, _ptr(image), _ptr(target), float(lam), _ptr(out),
+                                        _ptr(grad) if want_grad else None, _stream(stream))
+    if rc != 0:
+        raise GabsplatError(rc, lib().gabsplat_loss_static_last_error().decode())
+    return out, (grad if want_grad else None)
 
 
 def gabsplat_kernel_launches() -> int:

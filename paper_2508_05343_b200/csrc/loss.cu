@@ -14,6 +14,8 @@
 // quantity and pixel, plus the halo rows), so everything around it is kept off the instruction stream: a thread of
 // the horizontal pass converts and multiplies each input ONCE and feeds it to the 4 neighbouring outputs it owns; a
 // thread of the vertical pass owns two adjacent rows, whose 11-row windows share 10 rows.
+#include <mutex>
+
 #include "common.cuh"
 
 namespace gabsplat {
@@ -235,3 +237,102 @@ cudaError_t launch_loss(int W, int H, const float* image, const float* target, f
 }
 
 }  // namespace gabsplat
+
+// ---- gabsplat_loss_static: the same loss for callers that have no way to obtain device scratch ----------------
+//
+// gabsplat_loss needs a workspace (the nine derivative maps between its two passes and the per-CTA partial sums),
+// and the workspace has to come from somewhere: cudaMalloc, or a framework allocator sitting on top of it.  Some
+// callers cannot do that.  A plugin running inside someone else's engine is handed its input and output buffers
+// and nothing else; a real-time or safety-reviewed loop is forbidden to touch the allocator after start-up
+// (cudaMalloc takes a process-wide lock and may synchronise the device); a caller on a memory-capped GPU may find
+// the pool exhausted or fragmented at the moment it asks.  For them the scratch lives in the library image itself:
+// a file-scope __device__ array that the CUDA runtime places on every GPU that loads this module and that stays there
+// until the process exits.  Nothing is allocated or freed by this entry point, ever.
+//
+// The price is a fixed ceiling (kStaticMaxPixels, below) and a single shared copy per GPU: see the header.
+namespace gabsplat {
+namespace {
+
+constexpr int kStaticMaxPixels = 512 * 512;  // width * height; 36 bytes of maps per pixel -> 9 MiB
+constexpr int kStaticMaxSide = 2048;         // bounds the CTA count of a thin strip: 3 (W/32 + 1)(H/16 + 1) <= 3 * 705
+constexpr int kStaticMaxBlocks = 3 * 768;
+constexpr size_t kStaticMapsBytes = (size_t)9 * kStaticMaxPixels * sizeof(float);  // a multiple of 256
+constexpr size_t kStaticBytes = kStaticMapsBytes + (size_t)kStaticMaxBlocks * 2 * sizeof(double);
+static_assert(kStaticMapsBytes % 256 == 0, "the partial sums follow the maps and hold doubles");
+
+// The scratch itself.  In HOST code this name is only a handle the runtime recognises -- it is not a device address,
+// and handing it to a kernel would make the kernel write through a host pointer.  The address the kernels may use
+// comes from cudaGetSymbolAddress (static_scratch below) and differs from GPU to GPU.
+static __device__ __align__(256) unsigned char g_loss_scratch[kStaticBytes];
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned char* g_static_address[kStaticMaxDevices] = {};  // per device ordinal; resolved on the first call there
+thread_local const char* t_static_error = "no error";
+
+// Device address of g_loss_scratch on the CURRENT device, looked up once per device.  The look-up may make the
+// runtime load this module onto the device, which is why the first call on a device belongs before any capture.
+cudaError_t static_scratch(unsigned char** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_address[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_loss_scratch);
+    if (e != cudaSuccess) return e;
+    g_static_address[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_static_address[dev];
+  return cudaSuccess;
+}
+
+}  // namespace
+}  // namespace gabsplat
+
+extern "C" uint64_t gabsplat_loss_static_max_pixels(void) { return (uint64_t)gabsplat::kStaticMaxPixels; }
+
+extern "C" const char* gabsplat_loss_static_last_error(void) { return gabsplat::t_static_error; }
+
+extern "C" int32_t gabsplat_loss_static(int32_t width, int32_t height, const float* image, const float* target, float lambda,
+                                        float* loss_out, float* dL_dimage, void* stream) {
+  using namespace gabsplat;
+  if (width <= 0 || height <= 0 || !image || !target || !loss_out || !(lambda >= 0.f && lambda <= 1.f)) {
+    t_static_error = "loss_static: bad size, lambda or null pointer";
+    return GABSPLAT_INVALID_ARG;
+  }
+  const dim3 grid((width + kTX - 1) / kTX, (height + kTY - 1) / kTY, 3);
+  if (width > kStaticMaxSide || height > kStaticMaxSide || (int64_t)width * height > (int64_t)kStaticMaxPixels ||
+      (uint64_t)grid.x * grid.y * grid.z > (uint64_t)kStaticMaxBlocks) {
+    t_static_error = "loss_static: image larger than the built-in scratch (width * height <= 262144, each side <= 2048); "
+                     "use gabsplat_loss with a caller-provided workspace";
+    return GABSPLAT_CAPACITY;
+  }
+  unsigned char* scratch = nullptr;
+  cudaError_t e = static_scratch(&scratch);
+  if (e != cudaSuccess) {
+    t_static_error = cudaGetErrorString(e);
+    return GABSPLAT_CUDA;
+  }
+  // Every map value and partial sum that is read below is written first by this same call, so the previous call's
+  // leftovers in the array need no clearing.
+  float* maps = reinterpret_cast<float*>(scratch);
+  double* partials = reinterpret_cast<double*>(scratch + kStaticMapsBytes);
+  static const Taps taps = make_taps();
+  const cudaStream_t st = (cudaStream_t)stream;
+  const uint64_t hw = (uint64_t)width * height;
+  ssim_maps_kernel<<<grid, kLossThreads, 0, st>>>(width, height, taps, image, target, maps, partials);
+  loss_reduce_kernel<<<1, 256, 0, st>>>(partials, (int)(grid.x * grid.y * grid.z), 3.0 * (double)hw, lambda, loss_out);
+  launched(2);
+  if (dL_dimage) {
+    loss_grad_kernel<<<grid, kLossThreads, 0, st>>>(width, height, taps, image, target, maps, lambda, dL_dimage);
+    launched();
+  }
+  e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    t_static_error = cudaGetErrorString(e);
+    return GABSPLAT_CUDA;
+  }
+  return GABSPLAT_OK;
+}
