@@ -6,7 +6,7 @@ nvcc cross-compiles without a GPU.  The library lands next to this file so that 
 repository snapshot to the GPU box (it is git-ignored, not gpurun-ignored).
 
 GABSPLAT_NVCC_FLAGS (environment, optional): extra nvcc flags, e.g. the -D switches of the measured design alternatives
-kept in the sources (GS_FWD_STAGING_CPASYNC, GS_BWD_BRANCHFREE, GS_BWD_MINB, GS_BWD_REPLAY, GS_BWD_MAXROWS: DESIGN.md 7.4).
+kept in the sources (GS_FWD_STAGING_CPASYNC, GS_BWD_BRANCHFREE, GS_BWD_MINB, GS_BWD_REPLAY, GS_BWD_MAXROWS, GS_BWD_LOWPHASE: DESIGN.md 7.2, 7.4).
 Use --force with it; the default build is what the tests and bench.py measure.
 """
 from __future__ import annotations

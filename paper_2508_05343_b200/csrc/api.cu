@@ -8,7 +8,22 @@
 
 namespace gabsplat {
 std::atomic<unsigned long long> g_kernel_launches{0};
+
+// argument checks shared with host_api.cu (which must refuse a bad scene before it queues the first copy)
+bool camera_ok(const gabsplat_camera* c) {
+  // z_near > 0 (also rejects NaN): the depth key orders bits(t_z) as unsigned integers, valid for positive floats only
+  return c && c->width > 0 && c->height > 0 && c->fx > 0.f && c->fy > 0.f && c->z_near > 0.f &&
+         (int64_t)((c->width + kTile - 1) / kTile) * ((c->height + kTile - 1) / kTile) < (1 << 30);
 }
+
+bool scene_ok(const gabsplat_scene* s) {
+  if (!s || s->N < 0 || s->K < 0 || s->K > kMaxK || s->sh_degree < 0 || s->sh_degree > 3 || s->variant < 0 || s->variant > 3) return false;
+  if (s->N == 0) return true;
+  if (!s->means || !s->scales || !s->rotations || !s->opacities || !s->sh) return false;
+  if (s->K > 0 && (!s->freqs || !s->weights)) return false;
+  return true;
+}
+}  // namespace gabsplat
 
 namespace {
 
@@ -25,20 +40,6 @@ int32_t fail(gabsplat_ctx* ctx, int32_t code, const char* msg) {
 int32_t cuda_fail(gabsplat_ctx* ctx, cudaError_t e, const char* where) {
   if (ctx) std::snprintf(ctx->error, sizeof(ctx->error), "%s: %s", where, cudaGetErrorString(e));
   return GABSPLAT_CUDA;
-}
-
-bool camera_ok(const gabsplat_camera* c) {
-  // z_near > 0 (also rejects NaN): the depth key orders bits(t_z) as unsigned integers, valid for positive floats only
-  return c && c->width > 0 && c->height > 0 && c->fx > 0.f && c->fy > 0.f && c->z_near > 0.f &&
-         (int64_t)((c->width + kTile - 1) / kTile) * ((c->height + kTile - 1) / kTile) < (1 << 30);
-}
-
-bool scene_ok(const gabsplat_scene* s) {
-  if (!s || s->N < 0 || s->K < 0 || s->K > kMaxK || s->sh_degree < 0 || s->sh_degree > 3 || s->variant < 0 || s->variant > 3) return false;
-  if (s->N == 0) return true;
-  if (!s->means || !s->scales || !s->rotations || !s->opacities || !s->sh) return false;
-  if (s->K > 0 && (!s->freqs || !s->weights)) return false;
-  return true;
 }
 
 bool projected_ok(const gabsplat_projected* p, int N, int K) {

@@ -40,6 +40,10 @@ __host__ __device__ constexpr int group_rows(int NV) { return NV > kMaxRows ? NV
 #define GS_BWD_REPLAY 32
 #endif
 constexpr int kReplay = GS_BWD_REPLAY;  // saved entries staged per warp and batch
+#ifndef GS_BWD_LOWPHASE
+#define GS_BWD_LOWPHASE 0.0625f
+#endif
+constexpr float kLowPhase = GS_BWD_LOWPHASE;  // radians: below it 1 - cos and sin come from the phase itself (0 = never)
 
 __device__ __forceinline__ float rcp_fast(float x) {  // x in [0.01, 1]: no denormal, no special case
   float r;
@@ -158,6 +162,23 @@ __global__ void __launch_bounds__(32, GS_BWD_MINB) blend_backward_kernel(Camera 
       }
     }
     __syncwarp();
+    // Small phases (see the second pass below): lane j bounds |phase_k| over the pixels of this half tile that staged
+    // entry j can have been blended at -- the envelope test confines them to the ellipse u^2 + v^2 <= -qmin, whose
+    // half extents are sqrt(-qmin) sqrt(L21^2 + L22^2) / (L11 L22) in x and sqrt(-qmin) / L22 in y -- and sets bit k when the bound is
+    // below kLowPhase.
+    uint32_t my_low = 0u;
+    if (K > 0 && g.lane < m) {
+      const float4 a = rec[g.lane * R4], l = rec[g.lane * R4 + 1];
+      const float sq = sqrtf(fmaxf(-l.w, 0.f)), i22 = 1.0f / l.z;
+      const float rx = sq * sqrtf(fmaf(l.y, l.y, l.z * l.z)) * i22 / l.x, ry = sq * i22;
+      const float cy = 8.0f * (float)g.warp + 3.5f;
+      const float ex = fminf(fabsf(a.x - 7.5f) + 7.5f, rx), ey = fminf(fabsf(a.y - cy) + 3.5f, ry);
+      float tail[TL];
+      load_tail<K>(rec + g.lane * R4, tail);
+#pragma unroll
+      for (int k = 0; k < K; ++k)
+        if (fmaf(fabsf(tail[2 * k]), ex, fabsf(tail[2 * k + 1]) * ey) < kLowPhase) my_low |= 1u << k;
+    }
     int pend = 0, j0 = 0;
     for (int j = 0; j < m; ++j) {
       const uint4 mk = s_mask1[j];
@@ -176,6 +197,7 @@ __global__ void __launch_bounds__(32, GS_BWD_MINB) blend_backward_kernel(Camera 
       float Sc[KK], St[KK], Sty[KK];                                 // sums of -dL/dM cos_k, -dL/dM sin_k, -dL/dM sin_k dy
       float Sax = 0.f, Say = 0.f;                                    // AbsGS
       float wfx[KK], wfy[KK];
+      float ngMs[kSlots] = {0.f, 0.f, 0.f, 0.f};                     // -dL/dM per pixel, kept for the small-phase pass
 #pragma unroll
       for (int k = 0; k < K; ++k) {
         Sc[k] = St[k] = Sty[k] = 0.f;
@@ -225,6 +247,7 @@ __global__ void __launch_bounds__(32, GS_BWD_MINB) blend_backward_kernel(Camera 
           Suu = fmaf(gqu, u, Suu); Suv = fmaf(gqu, v, Suv); Svv = fmaf(gqv, v, Svv);
           Squ += gqu; Sqv += gqv;
           Sm += ngM;
+          ngMs[s] = ngM;
           float pdx = 0.f, pdy = 0.f;       // per-pixel d/d(dx), d/d(dy) through the phases (AbsGS only)
 #pragma unroll
           for (int k = 0; k < K; ++k) {
@@ -241,6 +264,34 @@ __global__ void __launch_bounds__(32, GS_BWD_MINB) blend_backward_kernel(Camera 
           }
         }
       }
+      float dw[KK];                                                  // -sum dL/dM (cos_k - 1)
+#pragma unroll
+      for (int k = 0; k < K; ++k) dw[k] = Sm - Sc[k];
+      // Small phases.  Next to 1 the fp32 cosine carries an absolute error of ~1e-7, so 1 - cos_k has no correct digit at
+      // |phase| ~ 1e-3, and the fp32 sine loses its relative accuracy the same way: d omega_k and d f2D_k of a component
+      // that is still near its initial value (the paper starts every primitive at f = 0.001) would be
+      // rounding noise.  Where every pixel the entry was blended at has |phase_k| < kLowPhase (bit k of the entry's mask,
+      // warp-uniform) the three phase sums of component k are taken again from the phase itself:
+      // 1 - cos = ph^2 (1/2 - ph^2/24), sin = ph (1 - ph^2/6), both to 2e-7 relative below 1/16.
+      const uint32_t lowk = K > 0 ? __shfl_sync(kFull, my_low, j) : 0u;
+      if (lowk != 0u) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+          if (!((lowk >> k) & 1u)) continue;
+          float d = 0.f, t0 = 0.f, ty = 0.f;
+#pragma unroll
+          for (int s = 0; s < kSlots; ++s) {
+            const float dy = __fsub_rn(g.ly[s], a.y);
+            const float ph = __fmaf_rn(tail[2 * k + 1], dy, me.phx[k]);
+            const float ph2 = ph * ph;
+            d = fmaf(ngMs[s] * ph2, fmaf(ph2, -1.0f / 24.0f, 0.5f), d);
+            const float t = ngMs[s] * (ph * fmaf(ph2, -1.0f / 6.0f, 1.0f));
+            t0 += t;
+            ty = fmaf(t, dy, ty);
+          }
+          dw[k] = d; St[k] = t0; Sty[k] = ty;
+        }
+      }
       {
         float* col = s_red + pend * (NV * kRowStride) + g.lane;
         // mean: d = p - mu2D, so dL/dmu2D = -dL/dd;  dL/dd = dL/dq ln 2 (-2 u L11, -2 (u L21 + v L22)) + sum_k gph_k 2 pi f2D_k
@@ -254,7 +305,7 @@ __global__ void __launch_bounds__(32, GS_BWD_MINB) blend_backward_kernel(Camera 
           gdy = fmaf(sg, tail[2 * k + 1], gdy);
           col[(9 + 2 * k) * kRowStride] = sg * dx;
           col[(9 + 2 * k + 1) * kRowStride] = w * Sty[k];
-          col[(9 + 2 * K + k) * kRowStride] = Sm - Sc[k];   // -sum dL/dM (cos_k - 1)
+          col[(9 + 2 * K + k) * kRowStride] = dw[k];
         }
         col[0] = -gdx; col[kRowStride] = -gdy;
         // conic, in whitened form: S = sum dL/d(ln G) w w^T  (the projection backward maps it to dL/dU)

@@ -178,6 +178,10 @@ cudaError_t launch_trace_pixels(int K, const Camera& cam, const gabsplat_project
 cudaError_t launch_probe_sincos(int n, const float* phase, float* c, float* s, cudaStream_t st);
 cudaError_t measure_peaks(float* results_host, void* scratch, cudaStream_t st);
 
+// argument checks of the ABI (api.cu): the INVALID_ARG conditions of gabsplat.h on a camera / a scene of device or host pointers
+bool camera_ok(const gabsplat_camera* c);
+bool scene_ok(const gabsplat_scene* s);
+
 uint64_t sort_workspace_bytes(int N, uint64_t capacity, int ntiles);
 bool keys_optional(int ntiles);  // true when the binning never reads gabsplat_binning.keys itself
 

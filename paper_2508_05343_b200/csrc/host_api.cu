@@ -1,5 +1,7 @@
 // gabsplat_render_host: the four calls of the ABI chained for a caller whose buffers live in HOST memory
 // (the end-to-end leg of bench.py).  Only copies and calls of the public entry points; no kernels here.
+#include <cstdio>
+
 #include "common.cuh"
 
 namespace {
@@ -98,8 +100,15 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* sh, const 
                              uint64_t capacity, float* image_host, const float* dL_dimage_host,
                              gabsplat_grads* gh, void* device_arena, uint64_t arena_bytes, void* stream) {
   if (!ctx || !sh || !cam || !image_host || !device_arena) return GABSPLAT_INVALID_ARG;
-  if (sh->N < 0 || sh->K < 0 || sh->K > kMaxK || cam->width <= 0 || cam->height <= 0) return GABSPLAT_INVALID_ARG;
+  // everything the calls below would refuse is refused here, before a single copy has been queued
+  if (!scene_ok(sh) || !camera_ok(cam)) {
+    std::snprintf(ctx->error, sizeof(ctx->error), "render_host: bad %s", scene_ok(sh) ? "camera" : "scene");
+    return GABSPLAT_INVALID_ARG;
+  }
   if (dL_dimage_host && !gh) return GABSPLAT_INVALID_ARG;
+  if (dL_dimage_host && sh->N > 0 &&
+      (!gh->d_means || !gh->d_scales || !gh->d_rotations || !gh->d_opacities || !gh->d_sh || (sh->K > 0 && (!gh->d_freqs || !gh->d_weights))))
+    return GABSPLAT_INVALID_ARG;
   if (((uintptr_t)device_arena & 255) != 0) return GABSPLAT_INVALID_ARG;
   Layout l = carve(device_arena, sh->N, sh->K, cam->width, cam->height, capacity);
   if (arena_bytes < l.bytes) return GABSPLAT_CAPACITY;
@@ -112,7 +121,15 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* sh, const 
   //   opacities, frequencies, weights, SH colours    -> the value track (side stream, beside the binning), the blends
   //   dL/dimage                                      -> the backward
   //   image                                          <- leaves while the backward runs
-#define GS_CK(call) if ((call) != cudaSuccess) return GABSPLAT_CUDA
+  // A failure after this point leaves with copies from / to the caller's host buffers possibly still in flight on the two
+  // internal streams, which the caller cannot wait for: every error return drains them (and the caller's stream) first.
+  auto bail = [&](int32_t rc) {
+    cudaStreamSynchronize(cin);
+    cudaStreamSynchronize(cout);
+    cudaStreamSynchronize(st);
+    return rc;
+  };
+#define GS_CK(call) if ((call) != cudaSuccess) return bail(GABSPLAT_CUDA)
 #define GS_H2D(dst, src, count) if (count) GS_CK(cudaMemcpyAsync((void*)(dst), (src), (count) * f, cudaMemcpyHostToDevice, cin))
 #define GS_D2H(dst, src, count, s) if (count) GS_CK(cudaMemcpyAsync((dst), (const void*)(src), (count) * f, cudaMemcpyDeviceToHost, s))
   GS_CK(cudaEventRecord(ctx->ev_copy[0], st));          // whatever the caller queued before this call
@@ -134,10 +151,10 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* sh, const 
   l.scene.variant = sh->variant;
   GS_CK(cudaStreamWaitEvent(st, ctx->ev_copy[1], 0));
   int32_t rc = gabsplat_preprocess_bin_sort_ordered(ctx, &l.scene, cam, &l.proj, &l.bin, nullptr, stream, ctx->ev_copy[2]);
-  if (rc != GABSPLAT_OK) return rc;
+  if (rc != GABSPLAT_OK) return bail(rc);
   if (!dL_dimage_host) l.fwd.blend_state = nullptr;  // inference: nothing to replay
   rc = gabsplat_render_forward(ctx, &l.scene, cam, &l.proj, &l.bin, &l.fwd, stream);
-  if (rc != GABSPLAT_OK) return rc;
+  if (rc != GABSPLAT_OK) return bail(rc);
   GS_CK(cudaEventRecord(ctx->ev_copy[4], st));
   GS_CK(cudaStreamWaitEvent(cout, ctx->ev_copy[4], 0));
   GS_D2H(image_host, l.fwd.image, 3 * hw, cout);
@@ -147,7 +164,7 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* sh, const 
     GS_CK(cudaStreamWaitEvent(st, ctx->ev_copy[3], 0));
     rc = gabsplat_render_backward(ctx, &l.scene, cam, &l.proj, &l.bin, &l.fwd, l.dL, &l.grads, l.grad_ws,
                                   l.grad_ws_bytes, stream);
-    if (rc != GABSPLAT_OK) return rc;
+    if (rc != GABSPLAT_OK) return bail(rc);
     GS_D2H(gh->d_means, l.grads.d_means, n * 3, st);
     GS_D2H(gh->d_scales, l.grads.d_scales, n * 3, st);
     GS_D2H(gh->d_rotations, l.grads.d_rotations, n * 4, st);

@@ -136,6 +136,41 @@ def test_render_host_matches_device_path():
         assert np.allclose(grads[n].numpy(), ref[n], rtol=1e-4, atol=1e-6 * np.abs(ref[n]).max())
 
 
+def test_render_host_refuses_bad_arguments_before_copying():
+    """A scene or camera the device calls would refuse (z_near <= 0, unknown variant) is refused by gabsplat_render_host
+    itself, before any copy is queued on its internal streams: INVALID_ARG, the host image untouched, and the same
+    buffers render correctly in the next call."""
+    import copy
+    torch, gb, ctx, run_gpu = _mods()
+    scene = scenes.make_scene("tiny")
+    cam = scenes.make_cameras("tiny")[0]
+    ref, _ = run_gpu(scene, cam)
+
+    class H:
+        pass
+    h = H()
+    for n in ("means", "scales", "rotations", "opacities", "sh", "freqs", "weights"):
+        setattr(h, n, torch.from_numpy(getattr(scene, n)).pin_memory())
+    h.sh_degree = 3
+    cap = ref["D"] + 10
+    arena = torch.zeros(gb.host_arena_bytes(scene.N, scene.K, cam, cap), dtype=torch.uint8, device="cuda")
+    img = torch.full((3, cam.height, cam.width), -1.0, dtype=torch.float32).pin_memory()
+    bad_cam = copy.copy(cam)
+    bad_cam.z_near = 0.0
+    with pytest.raises(gb.GabsplatError) as err:
+        gb.gabsplat_render_host(ctx, h, bad_cam, cap, img, None, None, arena)
+    assert err.value.code == gb.INVALID_ARG and "camera" in str(err.value)
+    h.variant = 7
+    with pytest.raises(gb.GabsplatError) as err:
+        gb.gabsplat_render_host(ctx, h, cam, cap, img, None, None, arena)
+    assert err.value.code == gb.INVALID_ARG and "scene" in str(err.value)
+    torch.cuda.synchronize()
+    assert float(img.min()) == -1.0 and float(img.max()) == -1.0
+    h.variant = 0
+    gb.gabsplat_render_host(ctx, h, cam, cap, img, None, None, arena)
+    assert np.array_equal(img.numpy(), ref["image"])
+
+
 def test_inference_forward_has_no_blend_state():
     """A forward run without blend_state (inference) gives the same image bit for bit, and the backward refuses
     it with INVALID_ARG instead of silently re-deciding anything."""
