@@ -109,11 +109,16 @@ typedef struct {
   uint32_t* tiles_touched; /* [N]     number of tiles in the primitive's rectangle                */
   int32_t* rect;           /* [N][4]  xmin,ymin,xmax,ymax in tiles, max exclusive                  */
   float* packed;           /* [N][gabsplat_packed_floats(K)]  gather record, 16-byte aligned       */
-  uint32_t* chunk_visible; /* [3][ceil(N / GABSPLAT_CHUNK)]  per chunk of consecutive primitives: the number of
+  uint32_t* chunk_visible; /* [gabsplat_chunk_visible_count(N)] = [3][ceil(N / GABSPLAT_CHUNK)] (+1), all of it written
+                              by gabsplat_preprocess -- size it with that function, the layout has grown before.
+                              Per chunk of consecutive primitives: the number of
                               visible ones (what the binning needs to compact them in index order), then the
                               smallest and the largest bits(depth) among them (0xffffffff / 0 if none): the
                               depth range the binning buckets its sort by                               */
 } gabsplat_projected;
+
+/* Number of uint32 elements gabsplat_projected.chunk_visible must hold for N primitives. */
+uint64_t gabsplat_chunk_visible_count(int32_t N);
 
 /* Number of floats per primitive in gabsplat_projected.packed (a multiple of 4). */
 int32_t gabsplat_packed_floats(int32_t K);
@@ -139,7 +144,11 @@ typedef struct {
                                  length) instead of the list length.  A tile's time is set by how far it walks
                                  its list before its last pixel saturates, which the list length does not
                                  predict; a trainer that revisits its views keeps one hint array per view.
-                                 It changes the launch order of the forward blend and nothing else          */
+                                 It changes the launch order of the forward blend and nothing else.  It is
+                                 IGNORED (tile_order = descending list length) for images of more than 26 000
+                                 tiles, which take the one-byte radix path, and when capacity == 0.  What it
+                                 gains was measured on an unchanged scene re-rendered from the same view, its
+                                 best case; bench.py's headline step does not use it          */
 } gabsplat_binning;
 
 uint64_t gabsplat_sort_workspace_bytes(int32_t N, uint64_t capacity, int32_t width, int32_t height);
@@ -320,14 +329,16 @@ int32_t gabsplat_count_pairs(gabsplat_ctx* ctx, const gabsplat_scene* scene, con
  * pixel where a skip / stop / clamp decision sits within fp32 error of its threshold both outcomes are correct, and
  * the tests hand the CUDA path's decisions at exactly those pixels to the oracle).  One thread per pixel walks the
  * pixel's tile list with the operation sequence of gabsplat_render_forward (Eq.12-13 :158-162; bit-identical alpha).
- *   pixels   device [n][2] int32 (x, y), inside the image
- *   offsets  device [n+1] uint32, ascending: pixel i may write entries[offsets[i] .. offsets[i+1])
+ *   pixels   device [n][2] int32 (x, y); a pixel outside the image is not traced: its colour_T is 0 and its info is
+ *            (0, 0, 0, 1)
+ *   offsets  device [n+1] uint32, ascending: pixel i may write entries[offsets[i] .. offsets[i+1]) (an inverted pair
+ *            gives the pixel an empty slice)
  *   entries  device: for every entry blended at pixel i, in order: its 1-based position in the tile list, bit 31 set
  *            when min(0.99, .) was active (zero derivative in the backward); entries beyond the slice are dropped
  *   colour_T device [n][4] float: the pixel's (r, g, b) incl. background and final T -- equal bit for bit to
  *            gabsplat_fwd_out.image / final_T
  *   info     device [n][4] uint32: n_contrib, number of blended entries (may exceed the slice), 1-based position of
- *            the entry at which the pixel stopped (T (1 - alpha) < 1e-4; 0 = never), 0 */
+ *            the entry at which the pixel stopped (T (1 - alpha) < 1e-4; 0 = never), 1 if the pixel is outside the image else 0 */
 int32_t gabsplat_trace_pixels(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,
                               const gabsplat_projected* proj, const gabsplat_binning* bin, int32_t n, const int32_t* pixels,
                               const uint32_t* offsets, uint32_t* entries, float* colour_T, uint32_t* info, void* stream);

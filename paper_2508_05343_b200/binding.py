@@ -106,6 +106,8 @@ def lib():
         L.gabsplat_render_aux.argtypes = [P, C.POINTER(_Scene), C.POINTER(_Camera), C.POINTER(_Projected),
                                           C.POINTER(_Binning), P, P, C.c_uint64, P]
         L.gabsplat_render_aux.restype = C.c_int32
+        L.gabsplat_chunk_visible_count.argtypes = [C.c_int32]
+        L.gabsplat_chunk_visible_count.restype = C.c_uint64
         L.gabsplat_loss_workspace_bytes.argtypes = [C.c_int32, C.c_int32]
         L.gabsplat_loss_workspace_bytes.restype = C.c_uint64
         L.gabsplat_loss.argtypes = [P, C.c_int32, C.c_int32, P, P, C.c_float, P, P, P, C.c_uint64, P]
@@ -240,7 +242,7 @@ class Projected:
         self.tiles_touched = z((N,), torch.int32)  # uint32 on the device; torch has no uint32 arithmetic
         self.rect = z((N, 4), torch.int32)
         self.packed = z((N, lib().gabsplat_packed_floats(K)), torch.float32)
-        self.chunk_visible = z((3 * ((N + CHUNK - 1) // CHUNK) + 1,), torch.int32)
+        self.chunk_visible = z((int(lib().gabsplat_chunk_visible_count(N)),), torch.int32)
 
     def struct(self) -> _Projected:
         p = _Projected()

@@ -322,6 +322,10 @@ int32_t gabsplat_loss(gabsplat_ctx* ctx, int32_t width, int32_t height, const fl
   return e == cudaSuccess ? GABSPLAT_OK : cuda_fail(ctx, e, "loss");
 }
 
+uint64_t gabsplat_chunk_visible_count(int32_t N) {
+  return N <= 0 ? 1 : 3 * (((uint64_t)N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK) + 1;
+}
+
 uint64_t gabsplat_kernel_launches(void) { return g_kernel_launches.load(std::memory_order_relaxed); }
 
 int32_t gabsplat_trace_pixels(gabsplat_ctx* ctx, const gabsplat_scene* scene, const gabsplat_camera* cam,

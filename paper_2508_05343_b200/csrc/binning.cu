@@ -1092,8 +1092,7 @@ struct Workspace {
   u32* count_b;     // [1] = D, or 0 when D > capacity
   u32* table;       // [256][nblocks]
   u32* dtable[4];   // per depth pass: [sort_blocks(N)][256] histograms of that pass's input arrangement
-  u32* bucket_cnt;  // [kBuckets] pairs per depth bucket          } zeroed together with dtable
-  u32* bucket_cur;  // [kBuckets] (unused)                         }
+  u32* bucket_cnt;  // [kBuckets] pairs per depth bucket          zeroed together with dtable and sort_flag
   u32* slots;       // [N] slot of every compacted pair inside its bucket
   u32* sort_flag;   // [1] 1: a bucket is too large, the radix passes sort instead
   u32* bucket_base; // [kBuckets] first slot of every bucket
@@ -1126,11 +1125,10 @@ Workspace carve(void* base, int N, u64 capacity, int ntiles) {
   w.table = (u32*)take(table_n * 4);
   {  // contiguous, zeroed by one memset per call
     const u64 one = (u64)256 * (((u64)N + kSmallTile - 1) / kSmallTile + 1);
-    u32* base4 = (u32*)take((4 * one + 2 * kBuckets + 64) * 4);
+    u32* base4 = (u32*)take((4 * one + kBuckets + 64) * 4);
     for (int i = 0; i < 4; ++i) w.dtable[i] = base4 + i * one;
     w.bucket_cnt = base4 + 4 * one;
-    w.bucket_cur = w.bucket_cnt + kBuckets;
-    w.sort_flag = w.bucket_cur + kBuckets;
+    w.sort_flag = w.bucket_cnt + kBuckets;
   }
   w.bucket_base = (u32*)take((u64)kBuckets * 4);
   w.slots = (u32*)take((u64)N * 4);
@@ -1213,7 +1211,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   // A: depth order of the primitives (digits 0-3 of the 64-bit key)
   tm.begin(GABSPLAT_STAGE_DEPTH_SORT, st);
   const u32 nba = (u32)(((u64)N + kSmallTile - 1) / kSmallTile);
-  cudaMemsetAsync(ws.dtable[0], 0, ((size_t)4 * 256 * (nba + 1) + 2 * kBuckets + 64) * sizeof(u32), st);
+  cudaMemsetAsync(ws.dtable[0], 0, ((size_t)4 * 256 * (nba + 1) + kBuckets + 64) * sizeof(u32), st);
   const u32 nchunks = (u32)((N + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK);
   launch_pdl(depth_keys_kernel, nchunks, 256, 0, st, N, proj.tiles_touched, proj.depth,
              proj.chunk_visible, ws.pk[0], ws.pv[0], ws.n_vis, ws.dtable[0], ws.bucket_cnt, ws.slots, ws.range);

@@ -396,11 +396,16 @@ __global__ void __launch_bounds__(128) trace_pixels_kernel(Camera cam, const uin
   constexpr int R4 = packed_floats(K) / 4;
   constexpr int TL = K > 0 ? tail_floats(K) : 1;
   const int2 p = pixels[i];
+  if (p.x < 0 || p.y < 0 || p.x >= cam.width || p.y >= cam.height) {  // not a pixel of this image: flagged, nothing walked
+    colour_T[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    info[i] = make_uint4(0u, 0u, 0u, 1u);
+    return;
+  }
   const int tx = p.x / kTile, ty = p.y / kTile;
   const uint2 range = ranges[ty * cam.tiles_x + tx];
   const float x0 = (float)(tx * kTile), y0 = (float)(ty * kTile);
   const float lx = (float)(p.x - tx * kTile), ly = (float)(p.y - ty * kTile);
-  const uint32_t cap = offsets[i + 1] - offsets[i];
+  const uint32_t cap = offsets[i + 1] >= offsets[i] ? offsets[i + 1] - offsets[i] : 0u;  // descending offsets: no slice
   uint32_t* out = entries + offsets[i];
   float T = 1.0f, Cr = 0.f, Cg = 0.f, Cb = 0.f;
   uint32_t last = 0, stop = 0, nb = 0;

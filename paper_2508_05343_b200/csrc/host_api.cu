@@ -54,7 +54,7 @@ Layout carve(void* base, int N, int K, int width, int height, uint64_t capacity)
   l.proj.tiles_touched = a.take<uint32_t>(n);
   l.proj.rect = a.take<int32_t>(n * 4);
   l.proj.packed = a.take<float>(n * packed_floats(K));
-  l.proj.chunk_visible = a.take<uint32_t>(3 * ((n + GABSPLAT_CHUNK - 1) / GABSPLAT_CHUNK) + 1);
+  l.proj.chunk_visible = a.take<uint32_t>(gabsplat_chunk_visible_count(N));
   l.bin.offsets = a.take<uint32_t>(n);
   l.bin.keys = a.take<uint64_t>(capacity);
   l.bin.ids = a.take<uint32_t>(capacity);

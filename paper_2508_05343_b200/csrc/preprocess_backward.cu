@@ -146,7 +146,9 @@ __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Came
   double gf_extra[KV][3];
 #pragma unroll
   for (int k = 0; k < KV; ++k) gf_extra[k][0] = gf_extra[k][1] = gf_extra[k][2] = 0.0;
-  if (VARIANT && line && live) {
+  // a primitive outside the value contract (a scale of exactly 0) has b = inf: C2_k = 1 whatever f and v are, no gradient
+  // flows through it -- and 0 * inf below would turn the whole row into NaN
+  if (VARIANT && line && live && bq > 0.0 && bq < 1e300) {
     // C2_k = exp(-2 pi^2 a_k^2 / b), a_k = v . f_k, b = v^T Sigma^-1 v, v = W^T (u_x, u_y, 1)
     const double pi2 = 9.8696044010893586188;
     double gv[3] = {0, 0, 0}, gb = 0.0;
@@ -173,7 +175,8 @@ __device__ __forceinline__ void backward_one(const gabsplat_scene& s, const Came
   {
     const double iu = 1.0 / (U00 * U11 - U01 * U01);
     const double Ui00 = U11 * iu, Ui01 = -U01 * iu, Ui11 = U00 * iu;
-    if (mip) {  // rho = sqrt(det U / det U_d):  d rho = rho / 2 tr((U^-1 - U_d^-1) dU)
+    if (mip && rho > 0.0) {  // rho = sqrt(det U / det U_d):  d rho = rho / 2 tr((U^-1 - U_d^-1) dU); rho = 0 (det U = 0,
+                             // a degenerate primitive): never blended, and U^-1 is not finite
       const double h = 0.5 * g_rho * rho;
       GU[0][0] += h * (Ui00 - ca); GU[0][1] += h * (Ui01 - cb); GU[1][0] += h * (Ui01 - cb); GU[1][1] += h * (Ui11 - cc);
     }

@@ -65,3 +65,25 @@ def test_full_attenuation_never_blends():
     check_forward(g, orc.render_forward(scene, cam))
     check_gradients(g, o)
     assert np.all(np.isfinite(g["d_weights"])) and np.all(g["d_weights"][1::2] == 0)
+
+
+@pytest.mark.parametrize("variant,K,zero_axes", [(1, 4, 1), (3, 4, 1), (2, 0, 2), (2, 0, 1)])
+def test_degenerate_scales_give_no_nan(variant, K, zero_axes):
+    """Outside the value contract (scales > 0), but a trainer can underflow a scale to exactly 0: the variants divide by
+    s^2 (line integral: b = v^T Sigma^-1 v = inf) and by det U (Mip filter: rho = 0, U^-1 not finite).  Such a primitive
+    must not poison anything: image and every gradient stay finite, and the primitives that are in contract get the
+    gradients they get without the degenerate ones' variant terms (those rows are exactly zero or finite)."""
+    import torch
+    from gpu_helpers import run_gpu
+    scene = scenes.make_scene("tiny", K=K)
+    scene.variant = variant
+    scene.scales[::7, 1] = 0.0
+    if zero_axes == 2:
+        scene.scales[::7, 2] = 0.0
+    cam = scenes.make_cameras("tiny")[0]
+    dL = scenes.make_image_grad("tiny", 0, cam)
+    g, _ = run_gpu(scene, cam, dL)
+    assert np.isfinite(g["image"]).all()
+    for n in ("d_means", "d_scales", "d_rotations", "d_opacities", "d_sh", "d_freqs", "d_weights"):
+        assert np.isfinite(g[n]).all(), n
+    assert np.abs(g["d_means"]).max() > 0
