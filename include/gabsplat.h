@@ -298,14 +298,15 @@ int32_t gabsplat_render_host(gabsplat_ctx* ctx, const gabsplat_scene* scene_host
  * events, writes up to max_records (stage id, elapsed milliseconds) pairs in launch order, stores the
  * number of records that existed in *n_records, and clears the record list.  Host calls. */
 #define GABSPLAT_STAGE_PREPROCESS 0      /* S1  projection kernel                                   */
-#define GABSPLAT_STAGE_SCAN 1            /* S2a prefix sum of tiles_touched                          */
-#define GABSPLAT_STAGE_DUPLICATE 2       /* S2b key emission                                        */
-#define GABSPLAT_STAGE_SORT 3            /* S2c radix passes on the tile digits (over the instances) */
-#define GABSPLAT_STAGE_RANGES 4          /* S2d tile ranges (incl. clearing them)                   */
+#define GABSPLAT_STAGE_SCAN 1            /* S2a prefix sum of tiles_touched over the depth-ordered visible primitives */
+#define GABSPLAT_STAGE_DUPLICATE 2       /* S2b chunk bounds + per-(chunk, tile) counts (<= 26 000 tiles); key emission (radix path) */
+#define GABSPLAT_STAGE_SORT 3            /* S2c the tile digit: one counting placement pass; one-byte radix passes over the
+                                            instances on the radix path                                          */
+#define GABSPLAT_STAGE_RANGES 4          /* S2d tile ranges (prefix of the count table; from the sorted keys on the radix path) */
 #define GABSPLAT_STAGE_BLEND_FORWARD 5   /* S3                                                      */
 #define GABSPLAT_STAGE_BLEND_BACKWARD 6  /* S4a (incl. zeroing the 2D gradient records)             */
 #define GABSPLAT_STAGE_PREPROCESS_BACKWARD 7 /* S4b (incl. zeroing the gradient outputs)             */
-#define GABSPLAT_STAGE_DEPTH_SORT 8      /* S2c radix passes on the depth digits (over the primitives) */
+#define GABSPLAT_STAGE_DEPTH_SORT 8      /* S2c depth order of the visible primitives (bucketed; radix passes as fallback) */
 #define GABSPLAT_STAGE_COUNT 9
 int32_t gabsplat_timing_enable(gabsplat_ctx* ctx, int32_t on);
 int32_t gabsplat_timing_read(gabsplat_ctx* ctx, int32_t* stage_ids_host, float* ms_host, int32_t max_records,

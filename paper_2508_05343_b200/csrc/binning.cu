@@ -795,7 +795,7 @@ __device__ __forceinline__ void chunk_bound(const u32* __restrict__ offsets, con
 // record r of the depth-ordered visible primitives: (id, bits(depth), x0 | y0 << 16, x1 | y1 << 16): what the two
 // walks below read, coalesced, instead of chasing order -> rect / depth per primitive
 // One launch for two independent jobs: CTAs 0..kChunks compute the chunk boundaries, the others write the records.
-constexpr int kRecordCtas = 148 * 4;
+inline int record_ctas() { return sm_count() * 4; }
 __global__ void __launch_bounds__(256) bounds_records_kernel(const u32* __restrict__ offsets, const u32* __restrict__ order,
                                                              const int4* __restrict__ rect, const float* __restrict__ depth,
                                                              const u32* __restrict__ n_vis_p, u32* __restrict__ bounds,
@@ -803,7 +803,7 @@ __global__ void __launch_bounds__(256) bounds_records_kernel(const u32* __restri
   pdl_wait();
   if (blockIdx.x <= kChunks) { chunk_bound(offsets, n_vis_p, bounds, blockIdx.x); return; }
   const u32 n_vis = *n_vis_p;
-  for (u32 r = (blockIdx.x - kChunks - 1) * blockDim.x + threadIdx.x; r < n_vis; r += kRecordCtas * blockDim.x) {
+  for (u32 r = (blockIdx.x - kChunks - 1) * blockDim.x + threadIdx.x; r < n_vis; r += (gridDim.x - kChunks - 1) * blockDim.x) {
     const u32 id = __ldg(order + r);
     const int4 rc = __ldg(rect + id);
     recs[r] = make_uint4(id, __float_as_uint(__ldg(depth + id)), (u32)rc.x | ((u32)rc.y << 16), (u32)rc.z | ((u32)rc.w << 16));
@@ -1248,7 +1248,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
     const int4* rect = reinterpret_cast<const int4*>(proj.rect);
     uint2* ranges = reinterpret_cast<uint2*>(bin.tile_ranges);
     tm.begin(GABSPLAT_STAGE_DUPLICATE, st);
-    launch_pdl(bounds_records_kernel, kChunks + 1 + kRecordCtas, 256, 0, st, bin.offsets, order, rect, proj.depth, ws.n_vis,
+    launch_pdl(bounds_records_kernel, kChunks + 1 + record_ctas(), 256, 0, st, bin.offsets, order, rect, proj.depth, ws.n_vis,
                ws.bounds, ws.recs);
     launch_pdl(tile_count_kernel, kChunks, kPlaceThreads, smem_count, st, cam.tiles_x, cam.tiles_y, ws.recs, ws.bounds, ws.chunk_table);
     launched(2);
@@ -1284,7 +1284,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   // tile id over the duplicated instances
   unsigned long long* total64 = reinterpret_cast<unsigned long long*>(ws.count_a);
   cudaMemsetAsync(total64, 0, sizeof(unsigned long long), st);
-  instance_total_kernel<<<148 * 4, 256, 0, st>>>(N, proj.tiles_touched, total64);
+  instance_total_kernel<<<sm_count() * 4, 256, 0, st>>>(N, proj.tiles_touched, total64);
   clamp_count_kernel<<<1, 1, 0, st>>>(ws.count_b, bin.num_instances, total64, bin.capacity);
   launched(2);
   // stage B passes: one per byte of the tile id.  The last pass reads the alternate buffers and writes
@@ -1315,7 +1315,7 @@ cudaError_t launch_bin_sort(int N, const gabsplat_projected& proj, const Camera&
   // K5
   tm.begin(GABSPLAT_STAGE_RANGES, st);
   cudaMemsetAsync(bin.tile_ranges, 0, (size_t)ntiles * 2 * sizeof(u32), st);
-  tile_ranges_kernel<<<148 * 8, 256, 0, st>>>(bin.keys, bin.num_instances, bin.capacity,
+  tile_ranges_kernel<<<sm_count() * 8, 256, 0, st>>>(bin.keys, bin.num_instances, bin.capacity,
                                               reinterpret_cast<uint2*>(bin.tile_ranges));
   launched();
   const cudaError_t eo = launch_tile_order(bin.tile_ranges, false, ntiles, bin.tile_order, st);

@@ -1,6 +1,7 @@
 // S4a / K7: the blend in reverse (gradients of sum_p <dL/dC(p), C(p)> with respect to the projected
 // quantities of every primitive, including f2D and omega; PAPER.md:48, :129 -- derivation in DESIGN.md).
-// Same CTA / pixel mapping as the forward kernel (blend_common.cuh): 64 threads per tile, 4 pixels per thread.
+// Same pixel mapping as the forward kernel (blend_common.cuh): a warp per half tile (16 x 8 pixels), 4 pixels per thread;
+// here every half tile is a CTA of its own (one warp), launched by descending saved-list length.
 // Each warp replays the list of blended primitives the forward saved for its half tile, back to front, and
 // recovers the transmittance in front of each primitive by division.  Per primitive a thread first sums the
 // gradient contributions of its 4 pixels in registers; the 9+3K (+2) sums are then reduced over the warp through

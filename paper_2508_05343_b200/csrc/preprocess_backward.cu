@@ -377,7 +377,7 @@ __global__ void __launch_bounds__(256) grad_zero_kernel(int N, int K, gabsplat_g
 
 cudaError_t launch_grad_zero(const gabsplat_scene& s, const gabsplat_grads& g, cudaStream_t st) {
   if (s.N == 0) return cudaSuccess;
-  grad_zero_kernel<<<148 * 8, 256, 0, st>>>(s.N, s.K, g);
+  grad_zero_kernel<<<sm_count() * 8, 256, 0, st>>>(s.N, s.K, g);
   launched();
   return cudaGetLastError();
 }
