@@ -439,11 +439,16 @@ def run_ours(args, name, scene, cams, rank, world, local_rank) -> dict | None:
         with open(traffic_file) as f:
             tr = json.load(f)
         issue_slots_per_s = alu_peaks["sms"] * 4 * alu_peaks["sm_clock_hz"]
+        # the file holds one capture: config `name`, K = 4, non-zero weights; every other workload says so
+        profiled = K == 4 and not args.zero_weights and name in tr
         for s in per_stage:
+            if not profiled:
+                per_stage[s]["traffic"] = "not profiled"
+                continue
             rec = tr.get(name, {}).get(s)
             if isinstance(rec, dict):
                 per_stage[s]["traffic"] = rec.get("dram_bytes")
-                if rec.get("warp_instr") and K == 4 and not args.zero_weights:
+                if rec.get("warp_instr"):
                     per_stage[s]["executed_warp_instr"] = rec["warp_instr"]
                     per_stage[s]["issue_slot_utilisation"] = rec["warp_instr"] / (per_stage[s]["ms"] / 1e3 * issue_slots_per_s)
             elif rec is not None:

@@ -1,6 +1,7 @@
 """-m gpu parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times: every view of configs 3
-(unbounded, 1M primitives, 1297x840) and 2 (object, 300k, 800x800), views of config 4 (large, 3M, 1957x1266), and
-config 5 (K in {1, 2, 8} and the all-omega-zero case at 1M / 1297x840) -- the whole image, final T, last
+(unbounded, 1M primitives, 1297x840) and 2 (object, 300k, 800x800), four views of config 4 (large, 3M, 1957x1266),
+config 5 (K in {1, 2, 8} and the all-omega-zero case at 1M / 1297x840, two views each) and the primitive variants (f4) at
+config 3's size -- the whole image, final T, last
 contributor and EVERY gradient tensor against the oracle, UNMASKED, at north_star's tolerances.
 
 The image (and so its gradient) is discontinuous where a skip / stop / clamp decision crosses its threshold; within
@@ -114,7 +115,8 @@ def test_unbounded_every_view(view):
     full_compare("unbounded/view%d" % view, scene, cam, scenes.make_image_grad("unbounded", view, cam))
 
 
-@pytest.mark.parametrize("K,zero,view", [(1, False, 1), (2, False, 2), (8, False, 3), (4, True, 4)])
+@pytest.mark.parametrize("K,zero,view", [(1, False, 1), (2, False, 2), (8, False, 3), (4, True, 4),
+                                         (1, False, 5), (2, False, 6), (8, False, 7), (4, True, 0)])
 def test_filter_bank_sweep_full_size(K, zero, view):
     """BASELINE.json config 5: the K sweep and the all-omega-zero case at 1M primitives / 1297x840 (the synthetic
     stand-in for the paper's F ablation, Table 3)."""
@@ -134,7 +136,19 @@ def test_zero_weights_equals_k0_full_size():
     assert np.array_equal(g4["n_contrib"], g0["n_contrib"])
 
 
-@pytest.mark.parametrize("view", [0, 3])
+@pytest.mark.parametrize("variant,view", [(1, 1), (2, 2), (3, 5)])
+def test_variants_full_size(variant, view):
+    """SURVEY 8(f) f4 at the headline size: the line-integral amplitude, the Mip 2D filter (:224) and
+    both, on 1M primitives / 1297x840 -- whole-screen rectangles, |phase| up to ~300 rad, the fp64 value track and the
+    variant chain rule of the projection backward on every visible primitive; same unmasked comparison as the plain
+    primitive (the injected decisions are taken on the folded records the blend kernels see)."""
+    scene = scenes.make_scene("unbounded")
+    scene.variant = variant
+    cam = scenes.make_cameras("unbounded")[view]
+    full_compare("unbounded/variant%d/view%d" % (variant, view), scene, cam, scenes.make_image_grad("unbounded", view, cam))
+
+
+@pytest.mark.parametrize("view", [0, 3, 5, 6])
 def test_large_views(view):
     """BASELINE.json config 4: 3M primitives, 1957x1266, ~50 M instances, forward + backward."""
     scene = scenes.make_scene("large")
@@ -142,7 +156,7 @@ def test_large_views(view):
     full_compare("large/view%d" % view, scene, cam, scenes.make_image_grad("large", view, cam))
 
 
-@pytest.mark.parametrize("view", [0, 3, 6])
+@pytest.mark.parametrize("view", range(8))
 def test_object_views(view):
     """BASELINE.json config 2 (300k primitives in the unit ball, 800x800, white background).  The config is forward
     only; the backward is compared as well since it costs nothing extra here."""
